@@ -1,0 +1,227 @@
+/* qcf.h — C ABI of the B200-native QCFuse selective-recompute layer step.
+ *
+ * What the library computes is defined by arxiv 2606.05875 (cited below as PAPER.md:<line>, the text
+ * under /root/reference/PAPER.md, plus section / equation).  One call of `qcf_layer_step` is one layer of the
+ * "pipeline cache fusion" stage of Fig. 9 for a batch of independent RAG requests
+ * C = [c_1..c_m] + U (Eq. 1):
+ *
+ *   a1  qcf_rope_reposition   Eq. 4   re-position per-chunk PIC K caches (RoPE at chunk-local positions)
+ *                                     to request positions, stitch K and V
+ *   a2  qcf_score             Eq. 18/20 user-query -> context attention mass per context position,
+ *                                     aggregated over query tokens and heads
+ *   a3  qcf_select_topk       Eq. 11  P = TopK(I(t), floor(rho N))
+ *   a4+a5 qcf_recompute_attn  Eq. 7   scatter refreshed K/V of rows P (+ the query's own K/V) into the fused
+ *                                     cache, then causal GQA attention of rows P u U over the fused cache
+ *
+ *       qcf_full_prefill_attn Eq. 2   dense causal GQA over all N+Lq rows: the rho = 1 comparator
+ *
+ *
+ * Conventions (every entry point):
+ *   - All tensors are bf16 unless stated, token-major: caches [T][Hkv][d], queries/outputs [T][Hq][d];
+ *     q-head h reads kv-head g = h / (Hq/Hkv).  RoPE pairs are half-split (j, j+d/2), angle
+ *     pos * theta^(-2j/d) (reading (a)).
+ *   - "dev" = device pointer (16-byte aligned), "host" = host pointer.  The caller owns every buffer; the
+ *     library allocates only in qcf_create / qcf_batch_create and never on the hot path.
+ *   - Hot-path calls are asynchronous on `stream` (a cudaStream_t passed as void*), launch kernels only, do
+ *     no host<->device copies and no synchronisation; they may be captured in a CUDA graph.
+ *   - Per-request device arrays are strided by the batch's strides (qcf_batch_get_info):
+ *       t_stride = max_b (N_b + Lq_b) rows  — fused caches, position-indexed fresh rows, outputs
+ *       n_stride = max_b N_b               — scores, selections
+ *   - Errors: every call returns a qcf_status; nothing throws or aborts.  Arguments are validated on the
+ *     host before any launch.  qcf_last_error(ctx) gives the message of the last failure on that ctx.
+ *   - A ctx and its batches are not thread-safe; use one ctx per host thread / stream.
+ *   - There is no CPU fallback: without an sm_100 device qcf_create fails with QCF_ERR_UNSUPPORTED.
+ */
+#ifndef QCF_H_
+#define QCF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QCF_API __attribute__((visibility("default")))
+
+typedef struct qcf_ctx qcf_ctx;       /* opaque: device properties, workspace                           */
+typedef struct qcf_batch qcf_batch;   /* opaque: device-resident description of a batch of requests     */
+
+typedef enum {
+  QCF_OK = 0,
+  QCF_ERR_INVALID_ARG = 1,  /* null pointer, negative size, ratio outside [0,1], mis-ordered offsets     */
+  QCF_ERR_UNSUPPORTED = 2,  /* head_dim not in {64,128}, Hq % Hkv != 0, G not in {1,2,4,8,16}, no sm_100 */
+  QCF_ERR_WORKSPACE = 3,    /* batch exceeds the limits given to qcf_create                              */
+  QCF_ERR_CUDA = 4          /* a CUDA runtime call failed; message holds cudaGetErrorString              */
+} qcf_status;
+
+/* Head layout of one attention layer (BASELINE.json: "head layout"). */
+typedef struct {
+  int32_t n_q_heads;     /* Hq                                                     */
+  int32_t n_kv_heads;    /* Hkv, divides Hq                                        */
+  int32_t head_dim;      /* d, 64 or 128                                           */
+  float rope_theta;      /* RoPE base theta (1e6 in the BASELINE configs)          */
+  float softmax_scale;   /* 0 -> 1/sqrt(d)                                         */
+} qcf_layout;
+
+/* One request C = [c_1..c_m] + U (Eq. 1).  All pointers are HOST pointers, read only during
+ * qcf_batch_create.  Chunk i's PIC cache (Eq. 3) is `chunk_len[i]` consecutive rows of the
+ * layer's PIC pool starting at row `chunk_row[i]` (the pool is a [pool_rows][Hkv][d] bf16 array whose base
+ * pointers, one for K and one for V, are given per call because they change per layer while the chunk
+ * geometry does not).  The chunk's request offset off_i is the exclusive prefix sum of chunk_len
+ * (PAPER.md:112-117), N = sum chunk_len.  A chunk may be shared by many requests (BASELINE config 4). */
+typedef struct {
+  int32_t n_chunks;            /* m >= 0                                                               */
+  int32_t n_query;             /* Lq = |U| >= 0                                                        */
+  const int32_t* chunk_len;    /* host [m], each >= 0                                                  */
+  const int64_t* chunk_row;    /* host [m], first pool row of chunk i's PIC cache, >= 0                */
+} qcf_request;
+
+typedef struct {
+  int32_t batch;       /* B                                                                             */
+  int32_t t_stride;    /* max_b (N_b + Lq_b)                                                            */
+  int32_t n_stride;    /* max_b N_b                                                                     */
+  int32_t q_stride;    /* max_b Lq_b                                                                    */
+  int64_t total_ctx;   /* sum_b N_b                                                                     */
+} qcf_batch_info;
+
+/* ---------------------------------------------------------------------------------------------- lifetime */
+
+/* Creates a context on the current CUDA device for one head layout.  max_batch / max_ctx / max_query bound
+ * the batches that may be created on it (they size the internal workspace: score statistics, tile counters).
+ * Fails with QCF_ERR_UNSUPPORTED if the device is not compute capability 10.x or the layout is unsupported. */
+QCF_API qcf_status qcf_create(qcf_ctx** out, const qcf_layout* layout, int32_t max_batch, int32_t max_ctx,
+                              int32_t max_query);
+QCF_API void qcf_destroy(qcf_ctx* ctx);
+/* Message of the last failure on ctx ("" if none).  With ctx == NULL returns the message of the last failed
+ * qcf_create on this thread.  The pointer stays valid until the next call on the same ctx. */
+QCF_API const char* qcf_last_error(const qcf_ctx* ctx);
+/* Library version string, and the SM architecture the kernels were compiled for (100). */
+QCF_API const char* qcf_version(void);
+
+/* Validates `reqs[0..batch)`, computes chunk offsets off_i, the per-chunk rotation tables
+ * (cos, sin)(off_i * theta^(-2j/d)) in double precision on the host (Eq. 4's Pi_i), and uploads them.
+ * Synchronous (one blocking upload); not a hot-path call: a batch is built once per request set and reused by
+ * all L layers.  batch == 0 is legal (every later call on it is a no-op). */
+QCF_API qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch, qcf_batch** out);
+QCF_API void qcf_batch_destroy(qcf_batch* b);
+QCF_API qcf_status qcf_batch_get_info(const qcf_batch* b, qcf_batch_info* info);
+
+/* |P| = floor(rho * N + 1e-6) evaluated in double (Eq. 8 constraint |P| = floor(rho N), PAPER.md:195;
+ * DESIGN.md reading (g)).  Returns -1 if n_ctx < 0 or ratio is outside [0,1] or NaN. */
+QCF_API int32_t qcf_n_select(int32_t n_ctx, double ratio);
+
+/* ------------------------------------------------------------------------------------------------ a1 */
+
+/* Eq. 4.  For every request b, chunk i, chunk row r, kv-head g, pair j < d/2:
+ *     phi = off_i * theta^(-2j/d);  (a, b) = K_pic[r][g][j], K_pic[r][g][j+d/2]
+ *     k_fused[b][off_i+r][g][j]     = bf16(a cos phi - b sin phi)
+ *     k_fused[b][off_i+r][g][j+d/2] = bf16(b cos phi + a sin phi)
+ *     v_fused[b][off_i+r][g][:]     = V_pic[r][g][:]                       (byte copy)
+ * fp32 arithmetic, one bf16 rounding (RNE) on store.  A chunk at off_i = 0 is copied bit-exactly.
+ *   k_pool, v_pool : dev, [pool_rows][Hkv][d] bf16, read-only (the layer's PIC pool)
+ *   k_fused,v_fused: dev, [B][t_stride][Hkv][d] bf16; rows 0..N_b-1 of each request are written, the rest
+ *                    (the Lq query rows and padding) are left untouched. */
+QCF_API qcf_status qcf_rope_reposition(qcf_ctx* ctx, const qcf_batch* b, const void* k_pool, const void* v_pool,
+                                       void* k_fused, void* v_fused, void* stream);
+
+/* ------------------------------------------------------------------------------------------------ a2 */
+
+/* Eq. 18 with Attn^l(.)_t as defined at PAPER.md:208.  For request b, context position
+ * t < N_b:
+ *     I(t) = 1/(Hq Lq) * sum_{i<Lq} sum_{h<Hq} softmax_{t' < N_b}( q_probe[i][h] . k_fused[t'][h/G] * scale )_t
+ * (context keys only, no mask: DESIGN.md readings (b), (c), (d), (e)).  bf16 operands, fp32 accumulation and
+ * softmax.  accumulate == 0: scores[b][t] = I(t);  accumulate != 0: scores[b][t] += I(t)  (Eq. 20, the sum
+ * over critical layers).
+ *   q_probe : dev, [B][q_stride][Hq][d] bf16 — the anchor-conditioned query states Q_U^l(C_A) (Eq. 17), RoPE
+ *             at positions N_b..N_b+Lq_b-1; rows >= Lq_b of a request are ignored
+ *   k_fused : dev, [B][t_stride][Hkv][d] bf16 — output of qcf_rope_reposition (rows 0..N_b-1 are read)
+ *   scores  : dev, [B][n_stride] fp32; entries t >= N_b are left untouched
+ * A request with Lq_b == 0 or N_b == 0 contributes nothing (its scores are zeroed when accumulate == 0). */
+QCF_API qcf_status qcf_score(qcf_ctx* ctx, const qcf_batch* b, const void* q_probe, const void* k_fused,
+                             float* scores, int32_t accumulate, void* stream);
+
+/* ------------------------------------------------------------------------------------------------ a3 */
+
+/* Eq. 11: per request, the k_b = qcf_n_select(N_b, ratio) context positions with the
+ * largest scores over ALL context positions of the request (global budget, reading (i)); ties are broken
+ * towards the lower position (reading (h)); positions are emitted in ascending order.
+ *   scores : dev, [B][n_stride] fp32 (any finite values; -0 == +0; NaN unsupported)
+ *   sel    : dev, [B][n_stride] int32; sel[b][0..k_b) written
+ *   n_sel  : dev, [B] int32; n_sel[b] = k_b written
+ * Exact (integer radix select on the order-preserving key of the fp32 score): bit-identical across runs. */
+QCF_API qcf_status qcf_select_topk(qcf_ctx* ctx, const qcf_batch* b, const float* scores, double ratio,
+                                   int32_t* sel, int32_t* n_sel, void* stream);
+
+/* --------------------------------------------------------------------------------------------- a4 + a5 */
+
+/* Eq. 7 + PAPER.md:134.  With R_b = sel[b][0..n_sel[b]) followed by the query positions N_b..N_b+Lq_b-1:
+ *   a4: for p in R_b:  k_fused[b][p] = k_new[.], v_fused[b][p] = v_new[.]      (row copy; the query's own
+ *       K/V are appended at N_b..)
+ *   a5: for row index r (position p_r = R_b[r]) and head h:
+ *       out[b][r][h] = sum_{j <= p_r} softmax_j( q_new[.][h] . k_fused[b][j][h/G] * scale ) v_fused[b][j][h/G]
+ *       over the FUSED cache (unselected prefix = PIC, selected prefix = new; reading (k): all rows are
+ *       independent given the fused cache).  bf16 operands, fp32 softmax/accumulate, bf16 output (RNE).
+ *   sel, n_sel : dev, as written by qcf_select_topk (sel ascending, distinct, < N_b)
+ *   q_new/k_new/v_new : dev bf16, fresh rows under the current request order and positions;
+ *       rows_by_position != 0: [B][t_stride][H][d] indexed by request position p (only rows in R_b are read)
+ *       rows_by_position == 0: [B][t_stride][H][d] compact, row r <-> R_b[r]
+ *   k_fused, v_fused : dev, in/out
+ *   out : dev, [B][t_stride][Hq][d] bf16, rows 0..|R_b|-1 written (compact, P ascending then U)
+ *   lse : dev or NULL, [B][t_stride][Hq] fp32 natural-log-sum-exp of each output row's logits */
+QCF_API qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                                      const void* q_new, const void* k_new, const void* v_new,
+                                      int32_t rows_by_position, void* k_fused, void* v_fused, void* out,
+                                      float* lse, void* stream);
+
+/* Eq. 2 at one layer: dense causal GQA attention of all T_b = N_b + Lq_b rows over
+ * themselves — the rho = 1 endpoint and the "library's own full-prefill attention" comparator.
+ *   q : dev [B][t_stride][Hq][d];  k, v : dev [B][t_stride][Hkv][d];  out : dev [B][t_stride][Hq][d] */
+QCF_API qcf_status qcf_full_prefill_attn(qcf_ctx* ctx, const qcf_batch* b, const void* q, const void* k,
+                                         const void* v, void* out, float* lse, void* stream);
+
+/* ------------------------------------------------------------------------------------------------ a6 */
+
+/* Everything one layer needs, by name.  Pointers as documented at the stage entry points. */
+typedef struct {
+  const void* k_pool;      /* a1 in  */
+  const void* v_pool;      /* a1 in  */
+  void* k_fused;           /* a1 out, a2 in, a4/a5 in-out */
+  void* v_fused;
+  const void* q_probe;     /* a2 in (critical layers only; may be NULL otherwise) */
+  float* scores;           /* a2 in-out, a3 in */
+  int32_t* sel;            /* a3 out / a4,a5 in */
+  int32_t* n_sel;
+  const void* q_new;       /* a4/a5 in */
+  const void* k_new;
+  const void* v_new;
+  void* out;               /* a5 out */
+  float* lse;              /* a5 out, optional */
+  double ratio;            /* rho, used when select_now != 0 */
+  int32_t rows_by_position;
+  int32_t is_critical_layer; /* != 0: run a2 on this layer (l in L*, Eq. 20) */
+  int32_t accumulate;        /* a2: add to `scores` instead of overwriting */
+  int32_t select_now;        /* != 0: run a3 after a2 (once, after the last critical layer) */
+} qcf_layer_args;
+
+/* Fig. 9 / PAPER.md:337-344, one layer: a1 -> [a2 if is_critical_layer] -> [a3 if select_now] -> a4 -> a5,
+ * chained on `stream` with no host synchronisation. */
+QCF_API qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* args, void* stream);
+
+/* Same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe
+ * and fresh rows, runs qcf_layer_step on the context's internal device buffers, downloads `out`, `sel`,
+ * `n_sel` (and the fused cache if k_fused / v_fused are non-NULL), and synchronises `stream` before
+ * returning.  Pointer fields of `host` are host pointers with the same shapes; `pool_rows` is the number of
+ * rows of host->k_pool / v_pool.  Device staging buffers are allocated on first use and kept by the ctx. */
+QCF_API qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* host,
+                                       int64_t pool_rows, void* stream);
+
+/* Per-stage device time of the most recent qcf_layer_step issued with profiling enabled.
+ * qcf_set_profiling(ctx, 1) makes qcf_layer_step record CUDA events between stages (still asynchronous);
+ * qcf_get_stage_ms synchronises on the last event and fills ms[5] = {a1, a2, a3, a4, a5}. */
+QCF_API qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable);
+QCF_API qcf_status qcf_get_stage_ms(qcf_ctx* ctx, float* ms5);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QCF_H_ */

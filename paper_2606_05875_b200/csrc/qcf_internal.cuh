@@ -1,0 +1,157 @@
+// Internal declarations shared by the qcf translation units (not part of the C ABI).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "qcf.h"
+
+namespace qcf {
+
+// Device-resident description of a batch (arrays live in one allocation owned by qcf_batch).
+struct BatchDev {
+  int32_t batch;
+  int32_t n_chunks;        // total over the batch
+  int32_t t_stride;        // rows per request in fused caches / fresh rows / outputs
+  int32_t n_stride;        // entries per request in scores / sel
+  int32_t q_stride;        // rows per request in q_probe
+  // per request [batch]
+  const int32_t* n_ctx;    // N_b
+  const int32_t* n_query;  // Lq_b
+  // per chunk [n_chunks]
+  const int32_t* chunk_req;    // owning request
+  const int32_t* chunk_off;    // off_i: first request position
+  const int32_t* chunk_len;
+  const int64_t* chunk_row;    // first row in the PIC pool
+  const int32_t* chunk_blk;    // [n_chunks+1] exclusive prefix of ceil(len / kRepoRows): reposition work list
+  const float2* rot;           // [n_chunks][d/2] (cos, sin)(off_i * theta^(-2j/d))
+};
+
+struct Layout {
+  int hq, hkv, d, g;
+  float theta;
+  float scale;        // softmax scale
+};
+
+constexpr int kRepoRows = 8;        // rows per reposition work item
+
+}  // namespace qcf
+
+struct qcf_ctx {
+  qcf::Layout lay;
+  int device;
+  int n_sm;
+  int max_batch, max_ctx, max_query;
+  // workspace (device)
+  float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]
+  float* stats_l;        // score pass-1 partial row sum-exp
+  float* score_part;     // score pass-2 per-kv-head partial column sums [max_batch][Hkv][max_ctx]
+  unsigned int* counters;  // tile counters (zeroed, self-resetting)
+  size_t n_counters;
+  // host staging for qcf_layer_step_host
+  struct HostStage* stage;
+  // profiling
+  int profiling;
+  cudaEvent_t ev[6];
+  bool ev_valid;
+  mutable std::string err;
+};
+
+struct qcf_batch {
+  qcf_ctx* ctx;
+  qcf::BatchDev dev;       // pointers into `blob`
+  void* blob;              // one device allocation
+  // host copies for validation / grid sizing
+  int32_t batch;
+  int32_t n_chunks;
+  int32_t t_stride, n_stride, q_stride;
+  int32_t max_ctx, max_query;
+  int64_t total_ctx;
+  int32_t repo_blocks;     // total reposition work items
+  int32_t* h_n_ctx;        // [batch]
+  int32_t* h_n_query;      // [batch]
+};
+
+namespace qcf {
+
+constexpr int kScoreSplits = 8;     // key-range splits of the score statistics pass
+
+// Stage launchers (each validates nothing: arguments were checked by the API layer). Return cudaGetLastError().
+cudaError_t launch_reposition(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool,
+                              const __nv_bfloat16* v_pool, __nv_bfloat16* k_f, __nv_bfloat16* v_f, cudaStream_t);
+cudaError_t launch_score(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* q_probe, const __nv_bfloat16* k_f,
+                         float* scores, int accumulate, cudaStream_t);
+cudaError_t launch_topk(const qcf_ctx*, const qcf_batch*, const float* scores, double ratio, int32_t* sel,
+                        int32_t* n_sel, cudaStream_t);
+cudaError_t launch_scatter(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
+                           const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, int rows_by_position,
+                           __nv_bfloat16* k_f, __nv_bfloat16* v_f, cudaStream_t);
+// sel == nullptr: dense mode (rows 0..N+Lq-1 at their own positions, q indexed by position).
+cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
+                        const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
+                        const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
+
+// ------------------------------------------------------------------------------------------- device helpers
+#ifdef __CUDACC__
+
+__device__ __forceinline__ uint4 ld_nc_v4(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_na_v4(void* p, const uint4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
+               "r"(v.w)
+               : "memory");
+}
+__device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+// pack two fp32 -> bf16x2 (RNE), lo in the low half
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(addr));
+}
+__device__ __forceinline__ void ldmatrix_x4_trans(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(addr));
+}
+// D(16x8,f32) += A(16x16,bf16,row) * B(16x8,bf16,col)
+__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+// Shared-memory tile of bf16 rows of D elements, 16-byte chunks XOR-swizzled by (row & 7) so that ldmatrix
+// (8 rows x 16 B) and row-wise 16-byte stores are both conflict-free.  Returns the byte offset.
+template <int D>
+__device__ __forceinline__ uint32_t swz(int row, int chunk) {
+  return static_cast<uint32_t>(row * (D * 2) + ((chunk ^ (row & 7)) << 4));
+}
+
+#endif  // __CUDACC__
+
+}  // namespace qcf

@@ -1,0 +1,142 @@
+// a1 — Eq. 4: re-position per-chunk PIC keys to request positions and stitch K, V.
+//
+// HBM-bound stream: every K and V row is read once and written once (4 * Hkv * d * 2 bytes per context token).
+// A thread owns one "pair slot" of a row — 8 consecutive pairs (j..j+7, j+d/2..j+d/2+7) of one kv-head, i.e. two
+// 16-byte vectors — and keeps that slot's 8 (cos, sin) values of the chunk's rotation in registers while it walks
+// the rows of its work item, so the only memory traffic in the loop is 128-bit coalesced K/V loads and stores.
+#include "qcf_internal.cuh"
+
+namespace qcf {
+
+namespace {
+
+__device__ __forceinline__ void rotate8(const uint4& a, const uint4& b, const float (&c)[8], const float (&s)[8],
+                                        uint4& oa, uint4& ob) {
+  const uint32_t aw[4] = {a.x, a.y, a.z, a.w};
+  const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+  uint32_t ow_a[4], ow_b[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float a0 = bf16lo(aw[i]), a1 = bf16hi(aw[i]);
+    const float b0 = bf16lo(bw[i]), b1 = bf16hi(bw[i]);
+    // out_j = a cos - b sin ; out_{j+d/2} = b cos + a sin     (fp32, one rounding to bf16 on store)
+    const float ra0 = fmaf(a0, c[2 * i], -b0 * s[2 * i]);
+    const float ra1 = fmaf(a1, c[2 * i + 1], -b1 * s[2 * i + 1]);
+    const float rb0 = fmaf(b0, c[2 * i], a0 * s[2 * i]);
+    const float rb1 = fmaf(b1, c[2 * i + 1], a1 * s[2 * i + 1]);
+    ow_a[i] = pack_bf16(ra0, ra1);
+    ow_b[i] = pack_bf16(rb0, rb1);
+  }
+  oa = make_uint4(ow_a[0], ow_a[1], ow_a[2], ow_a[3]);
+  ob = make_uint4(ow_b[0], ow_b[1], ow_b[2], ow_b[3]);
+}
+
+// grid.x = number of work items (kRepoRows rows of one chunk); blockDim.x = slots * rows_per_pass where
+// slots = Hkv * d / 16 pair slots per row.
+template <int D>
+__global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, const __nv_bfloat16* __restrict__ k_pool,
+                                                         const __nv_bfloat16* __restrict__ v_pool,
+                                                         __nv_bfloat16* __restrict__ k_f,
+                                                         __nv_bfloat16* __restrict__ v_f) {
+  constexpr int kSlotsPerHead = D / 16;
+  const int slots = hkv * kSlotsPerHead;
+  const int row_elems = hkv * D;
+  // locate the chunk of this work item (chunk_blk is an exclusive prefix sum; a handful of chunks per batch)
+  const int item = blockIdx.x;
+  int lo = 0, hi = bd.n_chunks;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (bd.chunk_blk[mid] <= item) lo = mid; else hi = mid;
+  }
+  const int c = lo;
+  const int row0 = (item - bd.chunk_blk[c]) * kRepoRows;
+  const int len = bd.chunk_len[c];
+  const int rows = min(kRepoRows, len - row0);
+  const int off = bd.chunk_off[c];
+  const int req = bd.chunk_req[c];
+  const size_t src_row = static_cast<size_t>(bd.chunk_row[c]) + row0;
+  const size_t dst_row = static_cast<size_t>(req) * bd.t_stride + off + row0;
+
+  const int slot = threadIdx.x % slots;
+  const int rsub = threadIdx.x / slots;
+  const int rows_per_pass = blockDim.x / slots;
+  const int head = slot / kSlotsPerHead;
+  const int jc = slot % kSlotsPerHead;           // which group of 8 pairs
+  const int e0 = head * D + jc * 8;              // first-half vector (elements), second half at + D/2
+
+  // ---- K: rotate by the chunk's offset angle.  off == 0 is the identity and is copied bit-exactly.
+  const __nv_bfloat16* ks = k_pool + src_row * row_elems;
+  __nv_bfloat16* kd = k_f + dst_row * row_elems;
+  if (off == 0) {
+    for (int r = rsub; r < rows; r += rows_per_pass) {
+      const uint4 a = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0);
+      const uint4 b = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0 + D / 2);
+      st_na_v4(kd + static_cast<size_t>(r) * row_elems + e0, a);
+      st_na_v4(kd + static_cast<size_t>(r) * row_elems + e0 + D / 2, b);
+    }
+  } else {
+    float cs[8], sn[8];
+    const float4* rt = reinterpret_cast<const float4*>(bd.rot + static_cast<size_t>(c) * (D / 2) + jc * 8);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float4 t = __ldg(rt + i);
+      cs[2 * i] = t.x; sn[2 * i] = t.y; cs[2 * i + 1] = t.z; sn[2 * i + 1] = t.w;
+    }
+    // rows of this thread: rsub, rsub + rpp, ...  — at most kRepoRows / rpp, all loads issued before use
+    constexpr int kMaxIter = kRepoRows;
+    uint4 a[kMaxIter], b[kMaxIter];
+    const int n_it = (rows - rsub + rows_per_pass - 1) / rows_per_pass;   // may be <= 0
+#pragma unroll
+    for (int it = 0; it < kMaxIter; ++it) {
+      if (it < n_it) {
+        const size_t r = rsub + it * rows_per_pass;
+        a[it] = ld_nc_v4(ks + r * row_elems + e0);
+        b[it] = ld_nc_v4(ks + r * row_elems + e0 + D / 2);
+      }
+    }
+#pragma unroll
+    for (int it = 0; it < kMaxIter; ++it) {
+      if (it < n_it) {
+        const size_t r = rsub + it * rows_per_pass;
+        uint4 oa, ob;
+        rotate8(a[it], b[it], cs, sn, oa, ob);
+        st_na_v4(kd + r * row_elems + e0, oa);
+        st_na_v4(kd + r * row_elems + e0 + D / 2, ob);
+      }
+    }
+  }
+
+  // ---- V: stitched in the same token order (byte copy)
+  const uint4* vs = reinterpret_cast<const uint4*>(v_pool + src_row * row_elems);
+  uint4* vd = reinterpret_cast<uint4*>(v_f + dst_row * row_elems);
+  const int n_vec = rows * (row_elems / 8);
+  for (int i = threadIdx.x; i < n_vec; i += blockDim.x * 4) {
+    uint4 t[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i + u * blockDim.x < n_vec) t[u] = ld_nc_v4(vs + i + u * blockDim.x);
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (i + u * blockDim.x < n_vec) st_na_v4(vd + i + u * blockDim.x, t[u]);
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_reposition(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* k_pool,
+                              const __nv_bfloat16* v_pool, __nv_bfloat16* k_f, __nv_bfloat16* v_f,
+                              cudaStream_t stream) {
+  if (b->repo_blocks == 0) return cudaSuccess;
+  const int slots = ctx->lay.hkv * ctx->lay.d / 16;
+  int rpp = 256 / slots;
+  if (rpp < 1) rpp = 1;
+  if (rpp > kRepoRows) rpp = kRepoRows;
+  const int threads = slots * rpp;     // slots <= 512 is enforced at qcf_create
+  if (ctx->lay.d == 128)
+    reposition_kernel<128><<<b->repo_blocks, threads, 0, stream>>>(b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
+  else
+    reposition_kernel<64><<<b->repo_blocks, threads, 0, stream>>>(b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
+  return cudaGetLastError();
+}
+
+}  // namespace qcf

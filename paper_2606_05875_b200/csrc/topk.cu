@@ -1,0 +1,127 @@
+// a3 — Eq. 11: P = TopK(I(t), floor(rho N)) over all context positions of a request.
+//
+// Exact integer selection: the fp32 score is mapped to an order-preserving uint32 key, a 4-pass MSB-first 8-bit
+// radix select finds the k-th largest key T and how many elements equal to T belong to the top-k, then one ordered
+// sweep emits the selected positions in ascending order (ties at T go to the lowest positions — reading (h)).
+// One CTA per request: N <= 32768 scores are 128 KB, L1/L2-resident after the first pass; the stage is latency-
+// bound, not bandwidth-bound.
+#include "qcf_internal.cuh"
+
+namespace qcf {
+
+namespace {
+
+constexpr int kThreads = 1024;
+
+__device__ __forceinline__ uint32_t order_key(float f) {
+  uint32_t u = __float_as_uint(f);
+  if (u == 0x80000000u) u = 0u;                                  // -0 == +0
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);             // ascending in the value
+}
+
+__global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float* __restrict__ scores, double ratio,
+                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel) {
+  __shared__ unsigned int hist[256];
+  __shared__ unsigned int s_prefix, s_remaining;
+  __shared__ unsigned int warp_cnt[32];                          // packed (gt << 16) | eq per warp
+  const int b = blockIdx.x;
+  const int N = bd.n_ctx[b];
+  const int k = static_cast<int>(floor(ratio * static_cast<double>(N) + 1e-6));    // reading (g)
+  const float* s = scores + static_cast<size_t>(b) * bd.n_stride;
+  int32_t* out = sel + static_cast<size_t>(b) * bd.n_stride;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) n_sel[b] = k;
+  if (k <= 0) return;
+  if (k >= N) {
+    for (int i = tid; i < N; i += kThreads) out[i] = i;
+    return;
+  }
+
+  // ---- radix select: after pass p the top 8(p+1) bits of the k-th largest key are known
+  if (tid == 0) { s_prefix = 0u; s_remaining = static_cast<unsigned int>(k); }
+#pragma unroll 1
+  for (int pass = 0; pass < 4; ++pass) {
+    const int shift = 24 - 8 * pass;
+    if (tid < 256) hist[tid] = 0u;
+    __syncthreads();
+    const uint32_t prefix = s_prefix;
+    const uint32_t mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
+    for (int i = tid; i < N; i += kThreads) {
+      const uint32_t key = order_key(s[i]);
+      if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 0xffu], 1u);
+    }
+    __syncthreads();
+    if (warp == 0) {
+      // bins from the top: find the digit where the cumulative count reaches `remaining`
+      const unsigned int remaining = s_remaining;
+      unsigned int cnt[8], tot = 0;
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { cnt[j] = hist[255 - (lane * 8 + j)]; tot += cnt[j]; }
+      unsigned int incl = tot;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      unsigned int run = incl - tot;                             // elements in higher bins than this lane's
+      if (run < remaining && incl >= remaining) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          if (run + cnt[j] >= remaining) {
+            s_prefix = prefix | (static_cast<uint32_t>(255 - (lane * 8 + j)) << shift);
+            s_remaining = remaining - run;
+            break;
+          }
+          run += cnt[j];
+        }
+      }
+    }
+    __syncthreads();
+  }
+  const uint32_t T = s_prefix;
+  const unsigned int need = s_remaining;                         // elements equal to T that are selected (>= 1)
+
+  // ---- ordered emission: position of element i = #(key > T before i) + min(#(key == T before i), need)
+  unsigned int run_gt = 0, run_eq = 0;
+  for (int base = 0; base < N; base += kThreads) {
+    const int i = base + tid;
+    uint32_t key = 0u;
+    const bool valid = i < N;
+    if (valid) key = order_key(s[i]);
+    const bool gt = valid && key > T, eq = valid && key == T;
+    const unsigned int bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
+    if (lane == 0) warp_cnt[warp] = (static_cast<unsigned int>(__popc(bg)) << 16) | static_cast<unsigned int>(__popc(be));
+    __syncthreads();
+    unsigned int before = 0, total = 0;
+    {
+      const unsigned int v = warp_cnt[lane];
+      unsigned int incl = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int u = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += u;
+      }
+      const unsigned int excl = incl - v;
+      before = __shfl_sync(0xffffffffu, excl, warp);
+      total = __shfl_sync(0xffffffffu, incl, 31);
+    }
+    const unsigned int lt_mask = (1u << lane) - 1u;
+    const unsigned int gt_before = run_gt + (before >> 16) + __popc(bg & lt_mask);
+    const unsigned int eq_before = run_eq + (before & 0xffffu) + __popc(be & lt_mask);
+    if (gt || (eq && eq_before < need)) out[gt_before + min(eq_before, need)] = i;
+    run_gt += total >> 16;
+    run_eq += total & 0xffffu;
+    __syncthreads();
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_topk(const qcf_ctx*, const qcf_batch* b, const float* scores, double ratio, int32_t* sel,
+                        int32_t* n_sel, cudaStream_t stream) {
+  if (b->batch == 0) return cudaSuccess;
+  topk_kernel<<<b->batch, kThreads, 0, stream>>>(b->dev, scores, ratio, sel, n_sel);
+  return cudaGetLastError();
+}
+
+}  // namespace qcf

@@ -1,0 +1,73 @@
+"""CPU-side checks of the boundary: libqcf.so builds for sm_100a, loads without a GPU, exports every symbol that
+include/qcf.h declares, and its host-only entry points behave (no compute calls here)."""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_05875_b200 import binding, build
+    build.build()
+    return binding.load_library()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "qcf.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"QCF_API\s+[\w\s\*]+?\b(qcf_\w+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    from paper_2606_05875_b200 import binding
+    declared = _declared_symbols()
+    assert len(declared) >= 15
+    assert sorted(binding.EXPORTS) == declared, "binding.EXPORTS must list exactly what qcf.h declares"
+    for name in declared:
+        assert hasattr(lib, name), name
+    # and nothing else leaks out of the shared object
+    out = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True).stdout
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l and not l.split()[-1].startswith("_"))
+    assert exported == declared
+
+
+def test_header_compiles_as_plain_c(tmp_path):
+    src = tmp_path / "t.c"
+    src.write_text('#include "qcf.h"\nint main(void) { qcf_layout l; qcf_layer_args a; (void)l; (void)a; return 0; }\n')
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-c", str(src), "-o",
+                    str(tmp_path / "t.o")], check=True)
+
+
+def test_library_is_sm100a_with_expected_kernels():
+    from paper_2606_05875_b200 import binding
+    out = subprocess.run(["cuobjdump", "-lelf", binding.LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_n_select_floor_rule(lib):
+    # DESIGN.md reading (g): floor(rho N + 1e-6) in double; the BASELINE configs' values
+    cases = [(128, 0.3, 38), (5120, 0.3, 1536), (10240, 0.3, 3072), (8192, 0.1, 819), (8192, 0.3, 2457),
+             (8192, 0.5, 4096), (32768, 0.15, 4915), (10, 0.0, 0), (10, 1.0, 10), (0, 0.5, 0)]
+    for n, r, k in cases:
+        assert lib.qcf_n_select(n, r) == k
+    assert lib.qcf_n_select(-1, 0.5) == -1 and lib.qcf_n_select(5, 1.5) == -1 and lib.qcf_n_select(5, float("nan")) == -1
+
+
+def test_create_fails_loudly_without_device_or_on_bad_layout(lib):
+    from paper_2606_05875_b200 import binding
+    import torch
+    h = ctypes.c_void_p()
+    lay = binding.qcf_layout(8, 3, 128, 1e6, 0.0)                  # Hkv does not divide Hq
+    assert lib.qcf_create(ctypes.byref(h), ctypes.byref(lay), 1, 128, 8) == binding.QCF_ERR_UNSUPPORTED
+    assert b"divide" in lib.qcf_last_error(None)
+    if not torch.cuda.is_available():
+        lay = binding.qcf_layout(8, 2, 128, 1e6, 0.0)
+        st = lib.qcf_create(ctypes.byref(h), ctypes.byref(lay), 1, 128, 8)
+        assert st == binding.QCF_ERR_UNSUPPORTED and not h.value, "no CPU fallback: creation must fail without a GPU"
+        with pytest.raises(binding.QcfError):
+            binding.Context(8, 2, 128, 1e6, 1, 128, 8)
