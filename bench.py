@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py — fused context tokens/s per qcf_layer_step at rho = 0.3 (BASELINE.json metric) on a B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl qcf|reference] [--no-cpu-baseline]
+
+One "step" = one pass of the whole hot path (a1 reposition -> a2 score -> a3 top-k -> a4 scatter -> a5 recompute
+attention) over one batch of seeded synthetic requests.  N = 1 runs BASELINE.json configs[1]
+("c2": Qwen3-8B-shaped layer, 10 x 512-token chunks, Lq 64).  N > 1 (torchrun, one rank per GPU): requests are
+independent, so every rank runs its own replica of the workload with no data-path collective —
+weak scaling; `value` = tokens all ranks processed / max-over-ranks device time.
+
+Timing: W >= 3 warm-up steps, then exactly K steps, each bracketed by CUDA events on the launching stream; an L2
+flush (a write of a 256 MiB buffer, outside the event pair) precedes every step because the c2 working set fits the
+126 MB L2.  Barrier + synchronize on both sides of the timed region; max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fused context tokens/s per layer step at r=0.3"
+UNIT = "tokens/s"
+KERNELS_PER_STEP = 6           # reposition, score_stats, score_colsum, topk, scatter, attn
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one attn_kernel launch on c2, from the ncu --set full capture
+# summarised in profiles/ (None until a capture of the current kernel is committed)
+A5_DRAM_TRAFFIC_BYTES = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--ratio", type=float, default=None)
+    ap.add_argument("--impl", default="qcf", choices=["qcf", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return d, "measured"
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+def n_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+
+def oracle_inputs(wl, b=0):
+    from oracle import qcf_oracle as O
+    r = wl.requests[b]
+    w = O.widen_bf16
+    return (r, [w(wl.pool_k[i]) for i in r.chunk_ids], [w(wl.pool_v[i]) for i in r.chunk_ids],
+            w(r.q_probe), w(r.q_new), w(r.k_new), w(r.v_new))
+
+
+def oracle_full_step_seconds(wl) -> float:
+    """The oracle as it stands, whole layer step of request 0."""
+    from oracle import qcf_oracle as O
+    r, kp, vp, qp, qn, kn, vn = oracle_inputs(wl)
+    t0 = time.perf_counter()
+    O.layer_step(kp, vp, wl.cfg.rope_theta, qp, wl.cfg.ratio, qn, kn, vn)
+    return time.perf_counter() - t0
+
+
+def oracle_sampled_step_seconds(wl, inp, stride: int = 8) -> float:
+    """a1 + a2 + a3 + a4 in full, a5 on every `stride`-th row of R (rows are independent given the fused cache, so
+    the sample is exact per row); the a5 time is scaled by |R| / |sample|."""
+    from oracle import qcf_oracle as O
+    r, kp, vp, qp, qn, kn, vn = inp
+    t0 = time.perf_counter()
+    k_ctx, v_ctx = O.reposition(kp, vp, wl.cfg.rope_theta)
+    sc = O.score(qp, k_ctx)
+    sel = O.select_topk(sc, O.n_select(r.n_ctx, wl.cfg.ratio))
+    k_f, v_f = O.fuse(k_ctx, v_ctx, sel, kn, vn)
+    t1 = time.perf_counter()
+    rows = np.concatenate([sel, np.arange(r.n_ctx, r.n_ctx + r.n_query)])
+    sample = rows[::stride]
+    O.recompute_attn(qn[sample], sample, k_f, v_f)
+    t2 = time.perf_counter()
+    return (t1 - t0) + (t2 - t1) * (len(rows) / max(len(sample), 1))
+
+
+def run_reference(args) -> None:
+    """--impl reference: the fp64 oracle on the host cores, same metric / config.  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2606_05875_b200 import inputs
+    wl = inputs.make_workload(args.workload, ratio=args.ratio, batch=1)
+    inp = oracle_inputs(wl)
+    stride = 8
+    for _ in range(max(args.warmup, 0)):
+        oracle_sampled_step_seconds(wl, inp, stride)
+    times = [oracle_sampled_step_seconds(wl, inp, stride) for _ in range(args.steps)]
+    t = float(np.mean(times))
+    value = wl.requests[0].n_ctx / t
+    sample = ("per step: a1+a2+a3+a4 of one request in full, a5 on every %d-th row of R (exact per row), a5 time "
+              "scaled by |R|/|sample|" % stride)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(wl, args, l2="n/a (host)"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": n_cores(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def config_dict(wl, args, l2: str) -> dict:
+    cfg = wl.cfg
+    return {"workload": "%s: %d request(s)/GPU x %d chunks x %d tokens (N=%d) + %d-token query, Hq/Hkv=%d/%d, d=%d, "
+                        "bf16, theta=%g, rho=%g" % (cfg.name, cfg.batch, cfg.n_chunks, cfg.chunk_len, cfg.n_ctx,
+                                                    cfg.n_query, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim,
+                                                    cfg.rope_theta, cfg.ratio),
+            "baseline_config": "configs[1]" if cfg.name == "c2" else cfg.name,
+            "ratio": cfg.ratio, "global_batch": cfg.batch * args.gpus, "parallelism": "replicas x%d" % args.gpus,
+            "l2": l2}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc = index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out = self.proc.communicate(timeout=5)[0]
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out = self.proc.communicate()[0]
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in out.splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ qcf arm
+
+def run_qcf(args) -> None:
+    import torch
+    import torch.distributed as dist
+    from paper_2606_05875_b200 import binding, device, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the qcf arm has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    if args.gpus != world and rank == 0:
+        print("bench.py: --gpus %d but WORLD_SIZE %d; using WORLD_SIZE" % (args.gpus, world), file=sys.stderr)
+    args.gpus = world
+
+    wl = inputs.make_workload(args.workload, ratio=args.ratio)     # every rank: its own replica (weak scaling)
+    cfg = wl.cfg
+    ctx = binding.Context(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, max(cfg.batch, 1),
+                          max(cfg.n_ctx, 1024), max(cfg.n_query, 1))
+    dw = device.DeviceWorkload(wl, ctx, device=dev)
+    largs = dw.layer_args(lse=None)
+    tokens_per_step = int(dw.batch.total_ctx)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.4)
+
+    # ---- device-resident leg: per-step events, per-stage events (qcf profiling hooks record on the same stream)
+    ctx.qcf_set_profiling(True)
+    for _ in range(max(args.warmup, 3)):
+        flush.fill_(1)
+        ctx.qcf_layer_step(dw.batch, largs)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ctx.qcf_get_stage_ms()                          # forget the warm-up steps
+    stage_acc, stage_n = np.zeros(5), 0
+    for i in range(args.steps):
+        flush.fill_(i & 0xff)
+        ev[i][0].record()
+        ctx.qcf_layer_step(dw.batch, largs)
+        ev[i][1].record()
+        if i % 512 == 511 and i + 1 < args.steps:   # the library keeps 512 profiled steps: drain (rare host sync)
+            stage_acc += 512 * np.array(ctx.qcf_get_stage_ms()); stage_n += 512
+    barrier()
+    rest = args.steps - stage_n
+    stage_acc += rest * np.array(ctx.qcf_get_stage_ms()); stage_n += rest
+    stage_ms = stage_acc / stage_n                  # mean per-stage device time over the K timed steps
+    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    total_ms = float(step_ms.sum())
+    ctx.qcf_set_profiling(False)
+
+    # ---- end-to-end leg: the same step through the C ABI with HOST (pinned) buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hw = device.DeviceWorkload(wl, ctx, device="cpu", pin=True)
+        hargs = hw.layer_args()
+        n_e2e = max(3, min(args.steps, 20))
+        for _ in range(2):
+            ctx.qcf_layer_step_host(hw.batch, hargs, hw.pool_rows)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            ctx.qcf_layer_step_host(hw.batch, hargs, hw.pool_rows)     # synchronises the stream before returning
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        nb = lambda t: t.numel() * t.element_size()
+        h2d = nb(hw.k_pool) + nb(hw.v_pool) + nb(hw.q_probe) + nb(hw.q_new) + nb(hw.k_new) + nb(hw.v_new)
+        d2h = nb(hw.out) + nb(hw.sel) + nb(hw.n_sel) + nb(hw.scores)
+        e2e = (e2e_s, h2d, d2h, n_e2e)
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- max over ranks
+    t = torch.tensor([total_ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_s = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_per_step = total_ms / args.steps
+    value = tokens_per_step * world / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (a5 recompute attention: tensor-bound)
+    peaks, peak_kind = load_peaks()
+    sel = dw.sel.cpu().numpy()
+    n_sel = dw.n_sel.cpu().numpy()
+    flops = 0.0
+    for b, (n, lq) in enumerate(zip(dw.batch.n_ctx, dw.batch.n_query)):
+        pos = np.concatenate([sel[b, : n_sel[b]].astype(np.int64), np.arange(n, n + lq)])
+        flops += device.attn_flops(cfg, n, pos)
+    a5_ms = float(stage_ms[4])
+    achieved = flops / (a5_ms * 1e-3) / 1e12
+    peak = float(peaks["bf16_tflops"])
+    roofline = {"kernel": "attn_kernel (a5 recompute attention)", "bound": "tensor", "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": A5_DRAM_TRAFFIC_BYTES,
+                "peak_source": "%s bf16_tflops (burst: the kernel is timed alone between events in a sub-ms step)" % peak_kind,
+                "algorithmic_flops_per_launch": flops, "ms_per_launch": a5_ms}
+    hbm = float(peaks["hbm_gbs"])
+    work = dw.algorithmic_work()
+    stages = {
+        "a1_reposition": {"ms": float(stage_ms[0]), "GBps": work["a1_bytes"] / (stage_ms[0] * 1e-3) / 1e9,
+                          "frac_hbm": work["a1_bytes"] / (stage_ms[0] * 1e-3) / 1e9 / hbm},
+        "a2_score": {"ms": float(stage_ms[1]), "TFLOPps": work["a2_flops"] / (stage_ms[1] * 1e-3) / 1e12},
+        "a3_topk": {"ms": float(stage_ms[2])},
+        "a4_scatter": {"ms": float(stage_ms[3]), "GBps": work["a4_bytes"] / (stage_ms[3] * 1e-3) / 1e9,
+                       "frac_hbm": work["a4_bytes"] / (stage_ms[3] * 1e-3) / 1e9 / hbm},
+        "a5_attn": {"ms": a5_ms, "TFLOPps": achieved},
+    }
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": config_dict(wl, args, l2="flushed before every timed step (256 MiB write, outside the event pair)"),
+        "clocks": clocks, "gpu_launches": KERNELS_PER_STEP * args.steps, "roofline": roofline, "stages": stages,
+        "step_ms_min_med_max": [float(step_ms.min()), float(np.median(step_ms)), float(step_ms.max())],
+    }
+    if e2e:
+        line["e2e"] = {"value": tokens_per_step * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(e2e[1]),
+                       "d2h_bytes_per_step": int(e2e[2]), "ms_per_step": e2e_s * 1e3, "steps": e2e[3],
+                       "api": "qcf_layer_step_host (pinned host buffers, stream-synchronised per step)"}
+    if not args.no_cpu_baseline:
+        wl1 = inputs.make_workload(args.workload, ratio=args.ratio, batch=1) if cfg.batch != 1 else wl
+        sec = oracle_full_step_seconds(wl1)
+        line["cpu_baseline"] = {"value": wl1.requests[0].n_ctx / sec, "unit": UNIT, "cores": n_cores(), "kind": "oracle",
+                                "sample": "one whole oracle.layer_step (fp64 numpy) of one %s request, %.1f s" % (cfg.name, sec)}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_qcf(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -215,9 +215,10 @@ QCF_API qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_la
 QCF_API qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* host,
                                        int64_t pool_rows, void* stream);
 
-/* Per-stage device time of the most recent qcf_layer_step issued with profiling enabled.
- * qcf_set_profiling(ctx, 1) makes qcf_layer_step record CUDA events between stages (still asynchronous);
- * qcf_get_stage_ms synchronises on the last event and fills ms[5] = {a1, a2, a3, a4, a5}. */
+/* Per-stage device time.  qcf_set_profiling(ctx, 1) makes every qcf_layer_step record CUDA events between its
+ * stages on `stream` (still asynchronous, no host synchronisation; up to 512 steps are kept).
+ * qcf_get_stage_ms synchronises on the last recorded event and fills ms[5] = {a1, a2, a3, a4, a5} with the MEAN
+ * over the profiled steps issued since the previous call (or since profiling was enabled), then forgets them. */
 QCF_API qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable);
 QCF_API qcf_status qcf_get_stage_ms(qcf_ctx* ctx, float* ms5);
 

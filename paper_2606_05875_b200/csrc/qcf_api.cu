@@ -123,7 +123,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->counters = nullptr;
   c->stage = nullptr;
   c->profiling = 0; c->ev_valid = false;
-  for (auto& ev : c->ev) ev = nullptr;
+  c->ev_ring = nullptr; c->ev_count = 0; c->ev = nullptr;
 
   const size_t stats_n = static_cast<size_t>(max_batch) * lay->n_q_heads * (max_query > 0 ? max_query : 1) * kScoreSplits;
   const size_t part_n = static_cast<size_t>(max_batch) * lay->n_kv_heads * max_ctx;
@@ -133,7 +133,6 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
             cudaMalloc(&c->score_part, part_n * sizeof(float)) == cudaSuccess &&
             cudaMalloc(&c->counters, c->n_counters * sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(c->counters, 0, c->n_counters * sizeof(unsigned int)) == cudaSuccess;
-  for (auto& ev : c->ev) ok = ok && cudaEventCreate(&ev) == cudaSuccess;
   if (!ok) {
     const cudaError_t le = cudaGetLastError();
     qcf_destroy(c);
@@ -146,7 +145,11 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
 void qcf_destroy(qcf_ctx* c) {
   if (!c) return;
   cudaFree(c->stats_m); cudaFree(c->stats_l); cudaFree(c->score_part); cudaFree(c->counters);
-  for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
+  if (c->ev_ring) {
+    for (int i = 0; i < qcf_ctx::kEvRing; ++i)
+      for (int j = 0; j < 6; ++j) if (c->ev_ring[i][j]) cudaEventDestroy(c->ev_ring[i][j]);
+    delete[] c->ev_ring;
+  }
   if (c->stage) { c->stage->release_all(); delete c->stage; }
   delete c;
 }
@@ -354,8 +357,9 @@ qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args
   QCF_REQUIRE(ctx, a != nullptr, "qcf_layer_step: args is NULL");
   if (a->select_now) QCF_REQUIRE(ctx, a->ratio >= 0.0 && a->ratio <= 1.0, "qcf_layer_step: ratio must be in [0, 1]");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  const bool prof = ctx->profiling != 0;
+  const bool prof = ctx->profiling != 0 && ctx->ev_ring && ctx->ev_count < qcf_ctx::kEvRing;
   ctx->ev_valid = false;
+  ctx->ev = prof ? ctx->ev_ring[ctx->ev_count] : nullptr;
   if (prof) cudaEventRecord(ctx->ev[0], s);
   if (qcf_status st = qcf_rope_reposition(ctx, b, a->k_pool, a->v_pool, a->k_fused, a->v_fused, stream)) return st;
   if (prof) cudaEventRecord(ctx->ev[1], s);
@@ -372,13 +376,22 @@ qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args
   if (prof) {
     if (b->batch == 0 || b->t_stride == 0) cudaEventRecord(ctx->ev[4], s);
     cudaEventRecord(ctx->ev[5], s);
+    ctx->ev_count++;
   }
+  ctx->ev_valid = false;
   return QCF_OK;
 }
 
 qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable) {
   if (!ctx) return QCF_ERR_INVALID_ARG;
+  if (enable && !ctx->ev_ring) {
+    ctx->ev_ring = new (std::nothrow) cudaEvent_t[qcf_ctx::kEvRing][6]();
+    if (!ctx->ev_ring) return fail(ctx, QCF_ERR_WORKSPACE, "out of host memory");
+    for (int i = 0; i < qcf_ctx::kEvRing; ++i)
+      for (int j = 0; j < 6; ++j) QCF_CUDA(ctx, cudaEventCreate(&ctx->ev_ring[i][j]));
+  }
   ctx->profiling = enable != 0;
+  ctx->ev_count = 0;
   ctx->ev_valid = false;
   return QCF_OK;
 }
@@ -386,9 +399,18 @@ qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable) {
 qcf_status qcf_get_stage_ms(qcf_ctx* ctx, float* ms5) {
   if (!ctx) return QCF_ERR_INVALID_ARG;
   QCF_REQUIRE(ctx, ms5 != nullptr, "ms5 is NULL");
-  QCF_REQUIRE(ctx, ctx->ev_valid, "no profiled qcf_layer_step has been issued");
-  QCF_CUDA(ctx, cudaEventSynchronize(ctx->ev[5]));
-  for (int i = 0; i < 5; ++i) QCF_CUDA(ctx, cudaEventElapsedTime(&ms5[i], ctx->ev[i], ctx->ev[i + 1]));
+  QCF_REQUIRE(ctx, ctx->ev_ring && ctx->ev_count > 0, "no profiled qcf_layer_step has been issued");
+  const int n = ctx->ev_count;
+  QCF_CUDA(ctx, cudaEventSynchronize(ctx->ev_ring[n - 1][5]));
+  double acc[5] = {0, 0, 0, 0, 0};
+  for (int k = 0; k < n; ++k)
+    for (int i = 0; i < 5; ++i) {
+      float ms = 0.f;
+      QCF_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->ev_ring[k][i], ctx->ev_ring[k][i + 1]));
+      acc[i] += ms;
+    }
+  for (int i = 0; i < 5; ++i) ms5[i] = static_cast<float>(acc[i] / n);
+  ctx->ev_count = 0;
   return QCF_OK;
 }
 

@@ -55,7 +55,10 @@ struct qcf_ctx {
   struct HostStage* stage;
   // profiling
   int profiling;
-  cudaEvent_t ev[6];
+  static constexpr int kEvRing = 512;   // profiled steps kept between two qcf_get_stage_ms calls
+  cudaEvent_t (*ev_ring)[6];            // [kEvRing][6], created by qcf_set_profiling(1)
+  int ev_count;                         // sets recorded since the last qcf_get_stage_ms
+  cudaEvent_t* ev;                      // set being recorded by the current qcf_layer_step (or nullptr)
   bool ev_valid;
   mutable std::string err;
 };

@@ -73,7 +73,11 @@ def test_reposition_parity(name):
         k_g, v_g = _f64(dw.k_fused[b, :n]), _f64(dw.v_fused[b, :n])
         assert np.array_equal(v_g, v_o), "V is a byte copy"
         # a correctly rounded fp32 evaluation: within half a bf16 ulp (+ fp32 slack) of the exact value
-        assert np.all(np.abs(k_g - k_exact) <= 0.5 * _ulp_bf16(k_exact) + 1e-5 * np.abs(k_exact) + 1e-30)
+        # (fp32 slack scales with the PAIR's norm, not the element: a cos - b sin may cancel)
+        half = wl.cfg.head_dim // 2
+        pair = np.hypot(k_exact[..., :half], k_exact[..., half:])
+        slack = 1e-6 * np.concatenate([pair, pair], axis=-1) + 1e-30
+        assert np.all(np.abs(k_g - k_exact) <= 0.5 * _ulp_bf16(k_exact) + slack)
         diff = np.abs(k_g - k_o)
         assert np.all(diff <= np.maximum(2e-2, _ulp_bf16(k_o)))
         assert np.mean(diff != 0) < 2e-3, "only values on a rounding boundary may differ"
@@ -201,7 +205,7 @@ def _run_recompute(ctx, dw, sel_list, by_position=True, q_new=None, k_new=None, 
     torch.cuda.synchronize()
 
 
-def _check_recompute(wl, dw, b, sel):
+def _check_recompute(wl, dw, b, sel, sentinel=True):
     r, k_pic, v_pic = _oracle_inputs(wl, b)
     n, lq = r.n_ctx, r.n_query
     ref = O.layer_step(k_pic, v_pic, wl.cfg.rope_theta, None, 0.0, O.widen_bf16(r.q_new), O.widen_bf16(r.k_new),
@@ -216,7 +220,8 @@ def _check_recompute(wl, dw, b, sel):
     kf = _f64(dw.k_fused[b, : n + lq])
     assert np.all(np.abs(kf - ref["k_fused"]) <= np.maximum(2e-2, _ulp_bf16(ref["k_fused"])))
     assert np.array_equal(_f64(dw.v_fused[b, : n + lq]), ref["v_fused"])
-    assert torch.all(dw.out[b, n_r:] == 55.0), "rows past |R_b| are untouched"
+    if sentinel:
+        assert torch.all(dw.out[b, n_r:] == 55.0), "rows past |R_b| are untouched"
     # log-sum-exp of each row's logits
     _, lse = O.recompute_attn(O.widen_bf16(r.q_new)[rows], rows, ref["k_fused"], ref["v_fused"], return_lse=True)
     np.testing.assert_allclose(dw.lse[b, :n_r].cpu().numpy(), lse, rtol=0, atol=2e-2)
@@ -287,7 +292,7 @@ def test_layer_step_chain(name):
         assert k == len(ref["sel"])
         got_sel = dw.sel[b, :k].cpu().numpy().astype(np.int64)
         _check_selection(got_sel, ref["scores"], k)
-        _check_recompute(wl, dw, b, got_sel)        # outputs checked against the oracle run on the GPU's selection
+        _check_recompute(wl, dw, b, got_sel, sentinel=False)        # outputs checked against the oracle run on the GPU's selection
 
 
 def test_layer_step_profiling_and_noncritical():
