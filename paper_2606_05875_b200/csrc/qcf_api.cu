@@ -122,6 +122,10 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->stats_m = c->stats_l = c->score_part = nullptr;
   c->counters = nullptr;
   c->stage = nullptr;
+  {
+    const char* e = std::getenv("QCF_ATTN_IMPL");
+    c->attn_impl = (e && std::strcmp(e, "mma") == 0) ? 0 : 1;
+  }
   c->profiling = 0; c->ev_valid = false;
   c->ev_ring = nullptr; c->ev_count = 0; c->ev = nullptr;
 

@@ -45,6 +45,7 @@ struct qcf_ctx {
   int device;
   int n_sm;
   int max_batch, max_ctx, max_query;
+  int attn_impl;         // 1: tcgen05/TMEM/TMA kernel (default); 0: legacy mma.sync kernel (QCF_ATTN_IMPL=mma, for A/B timing)
   // workspace (device)
   float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]
   float* stats_l;        // score pass-1 partial row sum-exp
@@ -96,6 +97,10 @@ cudaError_t launch_scatter(const qcf_ctx*, const qcf_batch*, const int32_t* sel,
 cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
+
+cudaError_t launch_attn_tc(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
+                           const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
+                           const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
 
 // ------------------------------------------------------------------------------------------- device helpers
 #ifdef __CUDACC__

@@ -1,0 +1,367 @@
+// a5 on the 5th-generation tensor cores — PAPER.md:134: causal GQA attention of the recomputed rows R = P u U over
+// the fused cache, as a warp-specialised tcgen05 / TMEM / TMA kernel.
+//
+//   tile      : 128 MMA rows = 128/G consecutive rows of R (ascending positions) x the G query heads of one kv-head,
+//               against key tiles of 128 positions of that kv-head (K/V fetched once serve all G heads)
+//   warp 0    : TMA producer — K and V tiles (4-D tensor maps over [B][T][Hkv][d], 128-byte swizzle) into 2-stage rings
+//   warp 1    : UMMA issuer  — S[j] = Q K_j^T (SS, fp32 in TMEM, double-buffered), O += P_j V_j (TS: P read from TMEM,
+//               V as an MN-major smem operand); S[j+1] is issued before P_j V_j so the softmax of tile j overlaps it
+//   warps 2-5 : softmax      — one thread per row (= TMEM lane): row max, exp2, bf16 P written back over S[j] in TMEM,
+//               lazy rescale of O (only when the running max grows by more than 2^8), final normalisation + store
+// The causal limit is monotone in the tile (rows ascending), so only key tiles reaching past the tile's first position
+// are masked and the key loop stops at the tile's last position.  sel == nullptr is the dense comparator (Eq. 2).
+#include "qcf_internal.cuh"
+#include "sm100_ptx.cuh"
+
+namespace qcf {
+
+namespace {
+
+using namespace ptx;
+
+constexpr int BM = 128;         // MMA rows per tile
+constexpr int BN = 128;         // keys per tile
+constexpr int kStages = 2;      // K and V ring depth
+constexpr int kThreads = 192;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kRescaleThreshold = 8.0f;     // log2 units: P stays <= 2^8, exactly representable headroom in bf16/fp32
+
+template <int D>
+struct Smem {
+  static constexpr int kTile = BN * D * 2;                 // bytes of one K or V tile (= Q tile)
+  static constexpr int kBlk = BN * 128;                    // bytes of one 64-column block (128 rows x 128 B)
+  static constexpr int oQ = 0;
+  static constexpr int oK = oQ + kTile;
+  static constexpr int oV = oK + kStages * kTile;
+  static constexpr int oBar = oV + kStages * kTile;        // mbarriers (8 B each)
+  static constexpr int kNumBar = 4 * kStages + 2 + 2 + 1;
+  static constexpr int oTmem = oBar + kNumBar * 8;
+  static constexpr int kBytes = oTmem + 16;
+};
+
+__device__ __forceinline__ float ex2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v, BatchDev bd, int hq,
+               int hkv, float scale_log2, const int32_t* __restrict__ sel, const int32_t* __restrict__ n_sel,
+               const __nv_bfloat16* __restrict__ q, int q_by_position, __nv_bfloat16* __restrict__ out,
+               float* __restrict__ lse_out) {
+  extern __shared__ unsigned char smem_raw[];
+  // 128-byte-swizzle atoms need 1024-byte alignment; the launch reserves 1 KB of slack for this round-up
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  using S = Smem<D>;
+  const int G = hq / hkv;
+  const int PT = BM / G;
+  const int b = blockIdx.z, g = blockIdx.y;
+  const int N = bd.n_ctx[b], Lq = bd.n_query[b];
+  const bool dense = sel == nullptr;
+  const int ns = dense ? 0 : n_sel[b];
+  const int n_rows = dense ? N + Lq : ns + Lq;
+  const int n_tiles = (n_rows + PT - 1) / PT;
+  const int tile = static_cast<int>(gridDim.x) - 1 - static_cast<int>(blockIdx.x);        // heaviest first
+  if (tile >= n_tiles) return;
+  const int ridx0 = tile * PT;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int* sel_b = dense ? nullptr : sel + static_cast<size_t>(b) * bd.n_stride;
+  auto pos_of = [&](int r) -> int {          // request position of row r of R (padding rows: 0, never stored)
+    if (r >= n_rows) return 0;
+    return dense ? r : (r < ns ? __ldg(sel_b + r) : N + (r - ns));
+  };
+  const int p_min = pos_of(ridx0);
+  const int p_max = pos_of(min(ridx0 + PT, n_rows) - 1);
+  const int n_kt = p_max / BN + 1;
+  const int t_end = N + Lq;                  // rows >= t_end of the cache are padding
+
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t sQ = sbase + S::oQ, sK = sbase + S::oK, sV = sbase + S::oV;
+  auto bar = [&](int i) -> uint32_t { return sbase + S::oBar + 8 * i; };
+  // barrier indices
+  const int kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages;
+  const int kSFull = 4 * kStages, kPReady = kSFull + 2, kODone = kPReady + 2;
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + S::oTmem);
+
+  if (warp == 0) {
+    if (lane == 0) {
+      prefetch_tensormap(&tm_k);
+      prefetch_tensormap(&tm_v);
+      for (int i = 0; i < 4 * kStages; ++i) mbar_init(bar(i), 1);
+      mbar_init(bar(kSFull), 1); mbar_init(bar(kSFull + 1), 1);
+      mbar_init(bar(kPReady), 128); mbar_init(bar(kPReady + 1), 128);
+      mbar_init(bar(kODone), 1);
+      fence_barrier_init();
+    }
+  } else if (warp == 1) {
+    tmem_alloc<512>(sbase + S::oTmem);
+  } else {
+    // Q tile -> smem in the K-major 128B-swizzle layout: row r at r*128 in each 64-column block, chunk c at c ^ (r & 7)
+    const int r = (warp & 3) * 32 + lane;
+    const int pl = r / G, hl = r % G;
+    const int ridx = ridx0 + pl;
+    const uint4* src = nullptr;
+    if (ridx < n_rows) {
+      const int src_row = (dense || q_by_position) ? pos_of(ridx) : ridx;
+      src = reinterpret_cast<const uint4*>(q + ((static_cast<size_t>(b) * bd.t_stride + src_row) * hq + g * G + hl) * D);
+    }
+#pragma unroll
+    for (int c = 0; c < D / 8; ++c) {
+      const uint4 v = src ? __ldg(src + c) : make_uint4(0u, 0u, 0u, 0u);
+      unsigned char* dst = smem + S::oQ + (c >> 3) * S::kBlk + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+      *reinterpret_cast<uint4*>(dst) = v;
+    }
+    fence_proxy_async_smem();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_o = tmem_base + 256;
+
+  if (warp == 0) {
+    // ===================================================================== TMA producer
+    if (lane == 0) {
+      for (int j = 0; j < n_kt; ++j) {
+        const int st = j % kStages;
+        const uint32_t ph = (j / kStages) & 1;
+        mbar_wait(bar(kEmptyK + st), ph ^ 1);
+        mbar_arrive_expect_tx(bar(kFullK + st), S::kTile);
+#pragma unroll
+        for (int kb = 0; kb < D / 64; ++kb)
+          tma_load_4d(sK + st * S::kTile + kb * S::kBlk, &tm_k, bar(kFullK + st), kb * 64, g, j * BN, b);
+        mbar_wait(bar(kEmptyV + st), ph ^ 1);
+        mbar_arrive_expect_tx(bar(kFullV + st), S::kTile);
+#pragma unroll
+        for (int kb = 0; kb < D / 64; ++kb)
+          tma_load_4d(sV + st * S::kTile + kb * S::kBlk, &tm_v, bar(kFullV + st), kb * 64, g, j * BN, b);
+      }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ===================================================================== UMMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
+      constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
+      auto issue_qk = [&](int j) {
+        const int st = j % kStages;
+        mbar_wait(bar(kFullK + st), (j / kStages) & 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + (j & 1) * 128;
+#pragma unroll
+        for (int ks = 0; ks < D / 16; ++ks) {
+          const uint32_t koff = (ks >> 2) * S::kBlk + (ks & 3) * 32;
+          umma_ss(d_tmem, umma_smem_desc_sw128(sQ + koff, 16, 1024),
+                  umma_smem_desc_sw128(sK + st * S::kTile + koff, 16, 1024), idesc_qk, ks > 0 ? 1u : 0u);
+        }
+        umma_commit(bar(kEmptyK + st));
+        umma_commit(bar(kSFull + (j & 1)));
+      };
+      issue_qk(0);
+      for (int j = 0; j < n_kt; ++j) {
+        if (j + 1 < n_kt) issue_qk(j + 1);
+        const int st = j % kStages;
+        mbar_wait(bar(kPReady + (j & 1)), (j >> 1) & 1);
+        mbar_wait(bar(kFullV + st), (j / kStages) & 1);
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < BN / 16; ++ks) {
+          umma_ts(tmem_o, tmem_base + (j & 1) * 128 + ks * 8,
+                  umma_smem_desc_sw128(sV + st * S::kTile + ks * 2048, S::kBlk, 1024), idesc_pv,
+                  (j > 0 || ks > 0) ? 1u : 0u);
+        }
+        umma_commit(bar(kEmptyV + st));
+        umma_commit(bar(kODone));
+      }
+    }
+    __syncwarp();
+  } else {
+    // ===================================================================== softmax / correction / epilogue
+    const int quarter = warp & 3;
+    const int r = quarter * 32 + lane;
+    const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16);
+    const int pl = r / G, hl = r % G;
+    const int ridx = ridx0 + pl;
+    const bool valid = ridx < n_rows;
+    const int pos = pos_of(ridx);
+    float m_used = -INFINITY, l = 0.f;
+
+    for (int j = 0; j < n_kt; ++j) {
+      mbar_wait(bar(kSFull + (j & 1)), (j >> 1) & 1);
+      tc_fence_after();
+      uint32_t s[4][32];
+      const uint32_t s_addr = lane_addr + (j & 1) * 128;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_ld32(s_addr + c * 32, s[c]);
+      tmem_wait_ld();
+      const int key0 = j * BN;
+      if (key0 + BN - 1 > p_min) {           // tile reaches past the first row's position: causal mask
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            if (key0 + c * 32 + i > pos) s[c][i] = 0xff800000u;      // -inf
+      }
+      float mx = -INFINITY;
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(s[c][i]));
+      const float m_new = mx * scale_log2;
+      if (j == 0) {
+        m_used = m_new;                      // key 0 is visible to every row: finite
+      } else if (__any_sync(0xffffffffu, m_new > m_used + kRescaleThreshold)) {
+        // lazy correction: O and l are kept relative to m_used; rescale only when the max grew by > 2^8
+        mbar_wait(bar(kODone), (j - 1) & 1);           // P_{j-1} V_{j-1} has landed in O
+        tc_fence_after();
+        const float m_t = fmaxf(m_used, m_new);
+        const float f = ex2(m_used - m_t);
+        m_used = m_t;
+        l *= f;
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t o[32];
+          tmem_ld32(lane_addr + 256 + c * 32, o);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+          tmem_st32(lane_addr + 256 + c * 32, o);
+        }
+        tmem_wait_st();
+      }
+      // P = exp2(s * scale - m_used) as bf16 pairs, written over the first 64 columns of S[j]
+      float lsum = 0.f;
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        uint32_t pk[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+          const int e = c * 64 + 2 * i;
+          const float p0 = ex2(fmaf(__uint_as_float(s[e >> 5][e & 31]), scale_log2, -m_used));
+          const float p1 = ex2(fmaf(__uint_as_float(s[(e + 1) >> 5][(e + 1) & 31]), scale_log2, -m_used));
+          lsum += p0 + p1;
+          pk[i] = pack_bf16(p0, p1);
+        }
+        tmem_st32(s_addr + c * 32, pk);
+      }
+      l += lsum;
+      if (key0 + BN > t_end) {
+        // the last tile reaches into padding rows of the cache: their V must not poison O (0 * NaN)
+        const int st = j % kStages;
+        mbar_wait(bar(kFullV + st), (j / kStages) & 1);
+        if (key0 + r >= t_end) {
+#pragma unroll
+          for (int kb = 0; kb < D / 64; ++kb) {
+            uint4* row = reinterpret_cast<uint4*>(smem + S::oV + st * S::kTile + kb * S::kBlk + r * 128);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) row[c] = make_uint4(0u, 0u, 0u, 0u);
+          }
+        }
+        fence_proxy_async_smem();
+      }
+      tmem_wait_st();
+      tc_fence_before();
+      mbar_arrive(bar(kPReady + (j & 1)));
+    }
+
+    // epilogue: O / l -> bf16 -> global (each thread owns one (row, head) vector of D elements)
+    mbar_wait(bar(kODone), (n_kt - 1) & 1);
+    tc_fence_after();
+    const float inv = 1.f / l;
+    __nv_bfloat16* dst = out + ((static_cast<size_t>(b) * bd.t_stride + ridx) * hq + g * G + hl) * D;
+#pragma unroll
+    for (int c = 0; c < D / 32; ++c) {
+      uint32_t o[32];
+      tmem_ld32(lane_addr + 256 + c * 32, o);
+      tmem_wait_ld();
+      if (valid) {
+#pragma unroll
+        for (int v4 = 0; v4 < 4; ++v4) {
+          uint4 w;
+          w.x = pack_bf16(__uint_as_float(o[8 * v4 + 0]) * inv, __uint_as_float(o[8 * v4 + 1]) * inv);
+          w.y = pack_bf16(__uint_as_float(o[8 * v4 + 2]) * inv, __uint_as_float(o[8 * v4 + 3]) * inv);
+          w.z = pack_bf16(__uint_as_float(o[8 * v4 + 4]) * inv, __uint_as_float(o[8 * v4 + 5]) * inv);
+          w.w = pack_bf16(__uint_as_float(o[8 * v4 + 6]) * inv, __uint_as_float(o[8 * v4 + 7]) * inv);
+          *reinterpret_cast<uint4*>(dst + c * 32 + v4 * 8) = w;
+        }
+      }
+    }
+    if (valid && lse_out)
+      lse_out[(static_cast<size_t>(b) * bd.t_stride + ridx) * hq + g * G + hl] = (m_used + log2f(l)) * kLn2;
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc<512>(tmem_base);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- host side
+using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeFn get_encode() {
+  static EncodeFn fn = []() -> EncodeFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<EncodeFn>(p);
+  }();
+  return fn;
+}
+
+// [B][T][Hkv][d] bf16, box = 128 rows x 64 elements of one head, 128-byte swizzle, zero fill out of bounds
+bool make_kv_map(CUtensorMap* m, const void* base, int batch, int t_stride, int hkv, int d) {
+  EncodeFn enc = get_encode();
+  if (!enc) return false;
+  const cuuint64_t dims[4] = {static_cast<cuuint64_t>(d), static_cast<cuuint64_t>(hkv),
+                              static_cast<cuuint64_t>(t_stride), static_cast<cuuint64_t>(batch)};
+  const cuuint64_t strides[3] = {static_cast<cuuint64_t>(d) * 2, static_cast<cuuint64_t>(hkv) * d * 2,
+                                 static_cast<cuuint64_t>(t_stride) * hkv * d * 2};
+  const cuuint32_t box[4] = {64, 1, BN, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+cudaError_t launch_attn_tc(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                           const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
+                           const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t stream) {
+  if (b->batch == 0 || b->t_stride == 0) return cudaSuccess;
+  const Layout& L = ctx->lay;
+  CUtensorMap tm_k, tm_v;
+  if (!make_kv_map(&tm_k, k_f, b->batch, b->t_stride, L.hkv, L.d) ||
+      !make_kv_map(&tm_v, v_f, b->batch, b->t_stride, L.hkv, L.d))
+    return cudaErrorInvalidValue;
+  const int PT = BM / L.g;
+  const int max_tiles = (b->t_stride + PT - 1) / PT;
+  const dim3 grid(max_tiles, L.hkv, b->batch);
+  const float scale_log2 = L.scale * kLog2e;
+  if (L.d == 128) {
+    auto kern = attn_tc_kernel<128>;
+    const int smem = Smem<128>::kBytes + 1024;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, scale_log2, sel, n_sel, q, rows_by_position,
+                                           out, lse);
+  } else {
+    auto kern = attn_tc_kernel<64>;
+    const int smem = Smem<64>::kBytes + 1024;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, scale_log2, sel, n_sel, q, rows_by_position,
+                                           out, lse);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace qcf
