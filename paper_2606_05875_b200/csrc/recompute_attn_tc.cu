@@ -20,25 +20,34 @@ namespace {
 using namespace ptx;
 
 constexpr int BM = 128;         // MMA rows per tile
-constexpr int BN = 128;         // keys per tile
+constexpr int BN = 64;          // keys per tile
 constexpr int kStages = 2;      // K and V ring depth
 constexpr int kThreads = 192;
+constexpr int kTmemCols = 256;  // S_0, S_1 (BN fp32 columns each; bf16 P_j aliases the first BN/2 of S_j) + O (up to 128)
+constexpr int kColO = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
-constexpr float kRescaleThreshold = 8.0f;     // log2 units: P stays <= 2^8, exactly representable headroom in bf16/fp32
+constexpr float kRescaleThreshold = 8.0f;     // log2 units: P stays <= 2^8
 
+// Two CTAs are resident per SM (96 KB of shared memory, 256 TMEM columns and <= 168 registers each).  Inside a CTA
+// S_{j+1} = Q K_{j+1}^T is issued before P_j V_j, so the softmax of tile j overlaps it; across the two CTAs the
+// remaining bubbles (barrier round trips, TMA latency) are filled, and each SM sub-partition holds two softmax warps.
 template <int D>
 struct Smem {
-  static constexpr int kTile = BN * D * 2;                 // bytes of one K or V tile (= Q tile)
-  static constexpr int kBlk = BN * 128;                    // bytes of one 64-column block (128 rows x 128 B)
+  static constexpr int kQBlk = BM * 128;                   // one 64-column block of Q (128 rows x 128 B)
+  static constexpr int kBlk = BN * 128;                    // one 64-column block of a K or V tile
+  static constexpr int kQ = BM * D * 2;
+  static constexpr int kTile = BN * D * 2;                 // bytes of one K or V tile
   static constexpr int oQ = 0;
-  static constexpr int oK = oQ + kTile;
+  static constexpr int oK = oQ + kQ;
   static constexpr int oV = oK + kStages * kTile;
   static constexpr int oBar = oV + kStages * kTile;        // mbarriers (8 B each)
-  static constexpr int kNumBar = 4 * kStages + 2 + 2 + 1;
+  static constexpr int kNumBar = 4 * kStages + 6;
   static constexpr int oTmem = oBar + kNumBar * 8;
   static constexpr int kBytes = oTmem + 16;
 };
+enum { kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages, kSFull = 4 * kStages,
+       kPReady = 4 * kStages + 2, kODone = 4 * kStages + 4 };
 
 __device__ __forceinline__ float ex2(float x) {
   float y;
@@ -46,25 +55,40 @@ __device__ __forceinline__ float ex2(float x) {
   return y;
 }
 
+// 2^x for x <= ~8 on the FMA pipe: n = round(x) via the 1.5*2^23 trick, f = x - n in [-0.5, 0.5], degree-3 minimax
+// polynomial (max relative error 7.5e-5, far below the bf16 rounding of P), exponent added with one integer op.
+__device__ __forceinline__ float ex2_poly(float x) {
+  x = fmaxf(x, -125.f);
+  const float r = x + 12582912.f;
+  const float f = x - (r - 12582912.f);
+  float p = fmaf(0.0551716685f, f, 0.2426111251f);
+  p = fmaf(p, f, 0.6932609677f);
+  p = fmaf(p, f, 0.9999280572f);
+  return __uint_as_float(__float_as_uint(p) + (__float_as_uint(r) << 23));
+}
+
 template <int D>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, 2)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v, BatchDev bd, int hq,
-               int hkv, float scale_log2, const int32_t* __restrict__ sel, const int32_t* __restrict__ n_sel,
-               const __nv_bfloat16* __restrict__ q, int q_by_position, __nv_bfloat16* __restrict__ out,
-               float* __restrict__ lse_out) {
+               int hkv, int max_tiles, float scale_log2, const int32_t* __restrict__ sel,
+               const int32_t* __restrict__ n_sel, const __nv_bfloat16* __restrict__ q, int q_by_position,
+               __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
   extern __shared__ unsigned char smem_raw[];
   // 128-byte-swizzle atoms need 1024-byte alignment; the launch reserves 1 KB of slack for this round-up
   unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   using S = Smem<D>;
   const int G = hq / hkv;
   const int PT = BM / G;
-  const int b = blockIdx.z, g = blockIdx.y;
+  // 1-D grid, heaviest tiles of ALL (request, kv-head) pairs first: block id -> (tile descending, head, request)
+  const int n_gb = hkv * bd.batch;
+  const int tile = max_tiles - 1 - static_cast<int>(blockIdx.x) / n_gb;
+  const int gb = static_cast<int>(blockIdx.x) % n_gb;
+  const int b = gb / hkv, g = gb % hkv;
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
   const bool dense = sel == nullptr;
   const int ns = dense ? 0 : n_sel[b];
   const int n_rows = dense ? N + Lq : ns + Lq;
   const int n_tiles = (n_rows + PT - 1) / PT;
-  const int tile = static_cast<int>(gridDim.x) - 1 - static_cast<int>(blockIdx.x);        // heaviest first
   if (tile >= n_tiles) return;
   const int ridx0 = tile * PT;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -81,23 +105,17 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const uint32_t sbase = smem_u32(smem);
   const uint32_t sQ = sbase + S::oQ, sK = sbase + S::oK, sV = sbase + S::oV;
   auto bar = [&](int i) -> uint32_t { return sbase + S::oBar + 8 * i; };
-  // barrier indices
-  const int kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages;
-  const int kSFull = 4 * kStages, kPReady = kSFull + 2, kODone = kPReady + 2;
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + S::oTmem);
 
   if (warp == 0) {
     if (lane == 0) {
       prefetch_tensormap(&tm_k);
       prefetch_tensormap(&tm_v);
-      for (int i = 0; i < 4 * kStages; ++i) mbar_init(bar(i), 1);
-      mbar_init(bar(kSFull), 1); mbar_init(bar(kSFull + 1), 1);
-      mbar_init(bar(kPReady), 128); mbar_init(bar(kPReady + 1), 128);
-      mbar_init(bar(kODone), 1);
+      for (int i = 0; i < S::kNumBar; ++i) mbar_init(bar(i), (i == kPReady || i == kPReady + 1) ? 128 : 1);
       fence_barrier_init();
     }
   } else if (warp == 1) {
-    tmem_alloc<512>(sbase + S::oTmem);
+    tmem_alloc<kTmemCols>(sbase + S::oTmem);
   } else {
     // Q tile -> smem in the K-major 128B-swizzle layout: row r at r*128 in each 64-column block, chunk c at c ^ (r & 7)
     const int r = (warp & 3) * 32 + lane;
@@ -111,7 +129,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 #pragma unroll
     for (int c = 0; c < D / 8; ++c) {
       const uint4 v = src ? __ldg(src + c) : make_uint4(0u, 0u, 0u, 0u);
-      unsigned char* dst = smem + S::oQ + (c >> 3) * S::kBlk + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+      unsigned char* dst = smem + S::oQ + (c >> 3) * S::kQBlk + r * 128 + (((c & 7) ^ (r & 7)) << 4);
       *reinterpret_cast<uint4*>(dst) = v;
     }
     fence_proxy_async_smem();
@@ -120,7 +138,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  const uint32_t tmem_o = tmem_base + 256;
+  const uint32_t tmem_o = tmem_base + kColO;
 
   if (warp == 0) {
     // ===================================================================== TMA producer
@@ -150,12 +168,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         const int st = j % kStages;
         mbar_wait(bar(kFullK + st), (j / kStages) & 1);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (j & 1) * 128;
+        // S_j overwrites the buffer of S_{j-2} / P_{j-2}: P_{j-2} V_{j-2} was issued earlier and UMMAs of one CTA
+        // execute in issue order; the softmax warps finished reading S_{j-2} before they signalled P_{j-2}.
+        const uint32_t d_tmem = tmem_base + (j & 1) * BN;
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
-          const uint32_t koff = (ks >> 2) * S::kBlk + (ks & 3) * 32;
-          umma_ss(d_tmem, umma_smem_desc_sw128(sQ + koff, 16, 1024),
-                  umma_smem_desc_sw128(sK + st * S::kTile + koff, 16, 1024), idesc_qk, ks > 0 ? 1u : 0u);
+          umma_ss(d_tmem, umma_smem_desc_sw128(sQ + (ks >> 2) * S::kQBlk + (ks & 3) * 32, 16, 1024),
+                  umma_smem_desc_sw128(sK + st * S::kTile + (ks >> 2) * S::kBlk + (ks & 3) * 32, 16, 1024), idesc_qk,
+                  ks > 0 ? 1u : 0u);
         }
         umma_commit(bar(kEmptyK + st));
         umma_commit(bar(kSFull + (j & 1)));
@@ -168,13 +188,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         mbar_wait(bar(kFullV + st), (j / kStages) & 1);
         tc_fence_after();
 #pragma unroll
-        for (int ks = 0; ks < BN / 16; ++ks) {
-          umma_ts(tmem_o, tmem_base + (j & 1) * 128 + ks * 8,
+        for (int ks = 0; ks < BN / 16; ++ks)
+          umma_ts(tmem_o, tmem_base + (j & 1) * BN + ks * 8,
                   umma_smem_desc_sw128(sV + st * S::kTile + ks * 2048, S::kBlk, 1024), idesc_pv,
                   (j > 0 || ks > 0) ? 1u : 0u);
-        }
         umma_commit(bar(kEmptyV + st));
-        umma_commit(bar(kODone));
+        umma_commit(bar(kODone + (j & 1)));
       }
     }
     __syncwarp();
@@ -190,69 +209,104 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     float m_used = -INFINITY, l = 0.f;
 
     for (int j = 0; j < n_kt; ++j) {
+      const int key0 = j * BN;
+      const bool need_mask = key0 + BN - 1 > p_min;     // tile reaches past the tile's first position
+      const uint32_t s_addr = lane_addr + (j & 1) * BN;
       mbar_wait(bar(kSFull + (j & 1)), (j >> 1) & 1);
       tc_fence_after();
-      uint32_t s[4][32];
-      const uint32_t s_addr = lane_addr + (j & 1) * 128;
+
+      uint32_t pk[BN / 2];      // P_j as bf16 pairs, kept in registers until the reference max is known to be valid
+      float tile_max, tile_sum;
+      // One sweep over the S row: p = 2^(s*scale - m_ref) against the REFERENCE max of the previous tiles, while the
+      // true row max of this tile is tracked on the ALU pipe.  3 of 4 exponentials go to MUFU.EX2, the 4th is a
+      // Cody-Waite + degree-3 polynomial on the FMA pipe (MUFU, at 16/clk/SM, is as tight as the tensor pipe here).
+      auto sweep = [&](float m_ref) {
+        float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+        uint32_t sa[32], sb[32];
+        tmem_ld32(s_addr, sa);
+        tmem_ld32(s_addr + 32, sb);
 #pragma unroll
-      for (int c = 0; c < 4; ++c) tmem_ld32(s_addr + c * 32, s[c]);
-      tmem_wait_ld();
-      const int key0 = j * BN;
-      if (key0 + BN - 1 > p_min) {           // tile reaches past the first row's position: causal mask
+        for (int c = 0; c < BN / 32; ++c) {
+          uint32_t(&cur)[32] = (c & 1) ? sb : sa;
+          if (c == 0) tmem_wait_ld();
 #pragma unroll
-        for (int c = 0; c < 4; ++c)
-#pragma unroll
-          for (int i = 0; i < 32; ++i)
-            if (key0 + c * 32 + i > pos) s[c][i] = 0xff800000u;      // -inf
-      }
-      float mx = -INFINITY;
-#pragma unroll
-      for (int c = 0; c < 4; ++c)
-#pragma unroll
-        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(s[c][i]));
-      const float m_new = mx * scale_log2;
+          for (int i = 0; i < 32; i += 4) {
+            float v0 = __uint_as_float(cur[i]), v1 = __uint_as_float(cur[i + 1]);
+            float v2 = __uint_as_float(cur[i + 2]), v3 = __uint_as_float(cur[i + 3]);
+            if (need_mask) {
+              const int k = key0 + c * 32 + i;
+              if (k > pos) v0 = -INFINITY;
+              if (k + 1 > pos) v1 = -INFINITY;
+              if (k + 2 > pos) v2 = -INFINITY;
+              if (k + 3 > pos) v3 = -INFINITY;
+            }
+            mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1); mx2 = fmaxf(mx2, v2); mx3 = fmaxf(mx3, v3);
+            const float p0 = ex2(fmaf(v0, scale_log2, -m_ref));
+            const float p1 = ex2(fmaf(v1, scale_log2, -m_ref));
+            const float p2 = ex2(fmaf(v2, scale_log2, -m_ref));
+            const float p3 = ex2_poly(fmaf(v3, scale_log2, -m_ref));
+            l0 += p0; l1 += p1; l2 += p2; l3 += p3;
+            pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
+            pk[c * 16 + (i >> 1) + 1] = pack_bf16(p2, p3);
+          }
+        }
+        tile_max = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
+        tile_sum = (l0 + l1) + (l2 + l3);
+      };
+
       if (j == 0) {
-        m_used = m_new;                      // key 0 is visible to every row: finite
-      } else if (__any_sync(0xffffffffu, m_new > m_used + kRescaleThreshold)) {
-        // lazy correction: O and l are kept relative to m_used; rescale only when the max grew by > 2^8
-        mbar_wait(bar(kODone), (j - 1) & 1);           // P_{j-1} V_{j-1} has landed in O
-        tc_fence_after();
-        const float m_t = fmaxf(m_used, m_new);
-        const float f = ex2(m_used - m_t);
-        m_used = m_t;
-        l *= f;
+        // first tile: the reference is its own max (key 0 is visible to every row, so it is finite)
+        float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-        for (int c = 0; c < D / 32; ++c) {
-          uint32_t o[32];
-          tmem_ld32(lane_addr + 256 + c * 32, o);
+        for (int c = 0; c < BN / 32; ++c) {
+          uint32_t t[32];
+          tmem_ld32(s_addr + c * 32, t);
           tmem_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-          tmem_st32(lane_addr + 256 + c * 32, o);
+          for (int i = 0; i < 32; i += 2) {
+            float v0 = __uint_as_float(t[i]), v1 = __uint_as_float(t[i + 1]);
+            if (need_mask) {
+              if (c * 32 + i > pos) v0 = -INFINITY;
+              if (c * 32 + i + 1 > pos) v1 = -INFINITY;
+            }
+            mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1);
+          }
         }
-        tmem_wait_st();
-      }
-      // P = exp2(s * scale - m_used) as bf16 pairs, written over the first 64 columns of S[j]
-      float lsum = 0.f;
+        m_used = fmaxf(mx0, mx1) * scale_log2;
+        sweep(m_used);
+      } else {
+        sweep(m_used);
+        if (__any_sync(0xffffffffu, tile_max > m_used + kRescaleThreshold)) {
+          // lazy correction: O and l are relative to m_used; move the reference only when the max grew by > 2^8
+          // P_{j-1} V_{j-1} has landed in O.  (Two alternating barriers: a warp may run one tile ahead of the
+          // slowest warp, and a single barrier's parity would then alias two phases.)
+          mbar_wait(bar(kODone + ((j - 1) & 1)), ((j - 1) >> 1) & 1);
+          tc_fence_after();
+          const float m_t = fmaxf(m_used, tile_max);
+          const float f = ex2(m_used - m_t);
+          m_used = m_t;
+          l *= f;
 #pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        uint32_t pk[32];
+          for (int c = 0; c < D / 32; ++c) {
+            uint32_t o[32];
+            tmem_ld32(lane_addr + kColO + c * 32, o);
+            tmem_wait_ld();
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          const int e = c * 64 + 2 * i;
-          const float p0 = ex2(fmaf(__uint_as_float(s[e >> 5][e & 31]), scale_log2, -m_used));
-          const float p1 = ex2(fmaf(__uint_as_float(s[(e + 1) >> 5][(e + 1) & 31]), scale_log2, -m_used));
-          lsum += p0 + p1;
-          pk[i] = pack_bf16(p0, p1);
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+            tmem_st32(lane_addr + kColO + c * 32, o);
+          }
+          tmem_wait_st();
+          sweep(m_used);                                 // S_j is still intact: P_j has not been stored yet
         }
-        tmem_st32(s_addr + c * 32, pk);
       }
-      l += lsum;
+      l += tile_sum;
+      tmem_st32(s_addr, pk);                             // P_j (BN/2 packed columns) over the first half of S_j
       if (key0 + BN > t_end) {
         // the last tile reaches into padding rows of the cache: their V must not poison O (0 * NaN)
         const int st = j % kStages;
         mbar_wait(bar(kFullV + st), (j / kStages) & 1);
-        if (key0 + r >= t_end) {
+        if (r < BN && key0 + r >= t_end) {
 #pragma unroll
           for (int kb = 0; kb < D / 64; ++kb) {
             uint4* row = reinterpret_cast<uint4*>(smem + S::oV + st * S::kTile + kb * S::kBlk + r * 128);
@@ -268,14 +322,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     }
 
     // epilogue: O / l -> bf16 -> global (each thread owns one (row, head) vector of D elements)
-    mbar_wait(bar(kODone), (n_kt - 1) & 1);
+    mbar_wait(bar(kODone + ((n_kt - 1) & 1)), ((n_kt - 1) >> 1) & 1);
     tc_fence_after();
     const float inv = 1.f / l;
     __nv_bfloat16* dst = out + ((static_cast<size_t>(b) * bd.t_stride + ridx) * hq + g * G + hl) * D;
 #pragma unroll
     for (int c = 0; c < D / 32; ++c) {
       uint32_t o[32];
-      tmem_ld32(lane_addr + 256 + c * 32, o);
+      tmem_ld32(lane_addr + kColO + c * 32, o);
       tmem_wait_ld();
       if (valid) {
 #pragma unroll
@@ -297,7 +351,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
-    tmem_dealloc<512>(tmem_base);
+    tmem_dealloc<kTmemCols>(tmem_base);
   }
 }
 
@@ -326,7 +380,7 @@ bool make_kv_map(CUtensorMap* m, const void* base, int batch, int t_stride, int 
                               static_cast<cuuint64_t>(t_stride), static_cast<cuuint64_t>(batch)};
   const cuuint64_t strides[3] = {static_cast<cuuint64_t>(d) * 2, static_cast<cuuint64_t>(hkv) * d * 2,
                                  static_cast<cuuint64_t>(t_stride) * hkv * d * 2};
-  const cuuint32_t box[4] = {64, 1, BN, 1};
+  const cuuint32_t box[4] = {64, 1, BN, 1};   // BN keys x 64 elements
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -346,19 +400,19 @@ cudaError_t launch_attn_tc(const qcf_ctx* ctx, const qcf_batch* b, const int32_t
     return cudaErrorInvalidValue;
   const int PT = BM / L.g;
   const int max_tiles = (b->t_stride + PT - 1) / PT;
-  const dim3 grid(max_tiles, L.hkv, b->batch);
+  const dim3 grid(static_cast<unsigned>(max_tiles) * L.hkv * b->batch);
   const float scale_log2 = L.scale * kLog2e;
   if (L.d == 128) {
     auto kern = attn_tc_kernel<128>;
     const int smem = Smem<128>::kBytes + 1024;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, scale_log2, sel, n_sel, q, rows_by_position,
+    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position,
                                            out, lse);
   } else {
     auto kern = attn_tc_kernel<64>;
     const int smem = Smem<64>::kBytes + 1024;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, scale_log2, sel, n_sel, q, rows_by_position,
+    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position,
                                            out, lse);
   }
   return cudaGetLastError();
