@@ -119,22 +119,29 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->device = dev;
   c->n_sm = prop.multiProcessorCount;
   c->max_batch = max_batch; c->max_ctx = max_ctx; c->max_query = max_query;
-  c->stats_m = c->stats_l = c->score_part = nullptr;
+  c->stats_m = c->stats_l = c->score_part = c->score_lse = nullptr;
+  c->score_row_ctr = nullptr;
   c->counters = nullptr;
   c->stage = nullptr;
   {
     const char* e = std::getenv("QCF_ATTN_IMPL");
     c->attn_impl = (e && std::strcmp(e, "mma") == 0) ? 0 : 1;
+    const char* e2 = std::getenv("QCF_SCORE_IMPL");
+    c->score_impl = (e2 && std::strcmp(e2, "mma") == 0) ? 0 : 1;
   }
   c->profiling = 0; c->ev_valid = false;
   c->ev_ring = nullptr; c->ev_count = 0; c->ev = nullptr;
 
-  const size_t stats_n = static_cast<size_t>(max_batch) * lay->n_q_heads * (max_query > 0 ? max_query : 1) * kScoreSplits;
+  const size_t stats_n = static_cast<size_t>(max_batch) * lay->n_q_heads * (max_query > 0 ? max_query : 1) * kScoreSplitsMax;
   const size_t part_n = static_cast<size_t>(max_batch) * lay->n_kv_heads * max_ctx;
+  const size_t row_ctr_n = static_cast<size_t>(max_batch) * lay->n_kv_heads * ((static_cast<size_t>(max_query) * g + 127) / 128 + 1);
   c->n_counters = static_cast<size_t>(max_batch) * ((max_ctx + 63) / 64) + 64;
   bool ok = cudaMalloc(&c->stats_m, stats_n * sizeof(float)) == cudaSuccess &&
             cudaMalloc(&c->stats_l, stats_n * sizeof(float)) == cudaSuccess &&
             cudaMalloc(&c->score_part, part_n * sizeof(float)) == cudaSuccess &&
+            cudaMalloc(&c->score_lse, stats_n / kScoreSplitsMax * sizeof(float)) == cudaSuccess &&
+            cudaMalloc(&c->score_row_ctr, row_ctr_n * sizeof(unsigned int)) == cudaSuccess &&
+            cudaMemset(c->score_row_ctr, 0, row_ctr_n * sizeof(unsigned int)) == cudaSuccess &&
             cudaMalloc(&c->counters, c->n_counters * sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(c->counters, 0, c->n_counters * sizeof(unsigned int)) == cudaSuccess;
   if (!ok) {
@@ -149,6 +156,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
 void qcf_destroy(qcf_ctx* c) {
   if (!c) return;
   cudaFree(c->stats_m); cudaFree(c->stats_l); cudaFree(c->score_part); cudaFree(c->counters);
+  cudaFree(c->score_lse); cudaFree(c->score_row_ctr);
   if (c->ev_ring) {
     for (int i = 0; i < qcf_ctx::kEvRing; ++i)
       for (int j = 0; j < 6; ++j) if (c->ev_ring[i][j]) cudaEventDestroy(c->ev_ring[i][j]);

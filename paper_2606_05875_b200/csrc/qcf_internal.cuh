@@ -45,10 +45,13 @@ struct qcf_ctx {
   int device;
   int n_sm;
   int max_batch, max_ctx, max_query;
+  int score_impl;        // 1: tcgen05 kernels (default); 0: legacy mma.sync kernels (QCF_SCORE_IMPL=mma)
   int attn_impl;         // 1: tcgen05/TMEM/TMA kernel (default); 0: legacy mma.sync kernel (QCF_ATTN_IMPL=mma, for A/B timing)
   // workspace (device)
   float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]
   float* stats_l;        // score pass-1 partial row sum-exp
+  float* score_lse;      // log2-sum-exp per probe row [max_batch][Hq*max_query]
+  unsigned int* score_row_ctr;   // pass-1 arrival counters per (request, kv-head, row tile), self-resetting
   float* score_part;     // score pass-2 per-kv-head partial column sums [max_batch][Hkv][max_ctx]
   unsigned int* counters;  // tile counters (zeroed, self-resetting)
   size_t n_counters;
@@ -81,7 +84,8 @@ struct qcf_batch {
 
 namespace qcf {
 
-constexpr int kScoreSplits = 8;     // key-range splits of the score statistics pass
+constexpr int kScoreSplits = 8;     // key-range splits of the legacy (mma.sync) score statistics pass
+constexpr int kScoreSplitsMax = 32; // upper bound of the tcgen05 pass-1 key splits (sizes the statistics workspace)
 
 // Stage launchers (each validates nothing: arguments were checked by the API layer). Return cudaGetLastError().
 cudaError_t launch_reposition(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool,
@@ -98,6 +102,8 @@ cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, co
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
 
+cudaError_t launch_score_tc(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* q_probe, const __nv_bfloat16* k_f,
+                            float* scores, int accumulate, cudaStream_t);
 cudaError_t launch_attn_tc(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                            const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                            const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);

@@ -49,24 +49,6 @@ struct Smem {
 enum { kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages, kSFull = 4 * kStages,
        kPReady = 4 * kStages + 2, kODone = 4 * kStages + 4 };
 
-__device__ __forceinline__ float ex2(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
-// 2^x for x <= ~8 on the FMA pipe: n = round(x) via the 1.5*2^23 trick, f = x - n in [-0.5, 0.5], degree-3 minimax
-// polynomial (max relative error 7.5e-5, far below the bf16 rounding of P), exponent added with one integer op.
-__device__ __forceinline__ float ex2_poly(float x) {
-  x = fmaxf(x, -125.f);
-  const float r = x + 12582912.f;
-  const float f = x - (r - 12582912.f);
-  float p = fmaf(0.0551716685f, f, 0.2426111251f);
-  p = fmaf(p, f, 0.6932609677f);
-  p = fmaf(p, f, 0.9999280572f);
-  return __uint_as_float(__float_as_uint(p) + (__float_as_uint(r) << 23));
-}
-
 template <int D>
 __global__ void __launch_bounds__(kThreads, 2)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v, BatchDev bd, int hq,

@@ -277,6 +277,7 @@ __global__ void __launch_bounds__(128) score_colsum_kernel(BatchDev bd, int hq, 
 cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* q_probe,
                          const __nv_bfloat16* k_f, float* scores, int accumulate, cudaStream_t stream) {
   if (b->batch == 0 || b->max_ctx == 0) return cudaSuccess;
+  if (ctx->score_impl == 1) return launch_score_tc(ctx, b, q_probe, k_f, scores, accumulate, stream);
   const Layout& L = ctx->lay;
   const float scale_log2 = L.scale * kLog2e;
   const int stats_rows = L.hq * ctx->max_query;

@@ -1,0 +1,399 @@
+// a2 on the 5th-generation tensor cores — Eq. 18 / 20:
+//
+//   I(t) = 1/(Hq Lq) sum_{i,h} exp(s_{i,h,t} - lse_{i,h}),   s = q_probe[i][h] . K'[t][h/G] * scale
+//
+// The row normaliser lse spans ALL context keys, so two sweeps are needed, and each wants its reduction to be local to a
+// thread (= one TMEM lane):
+//   pass 1 (stats)  : S   = Q_tile K_j^T   query rows on the lanes, key tiles streamed -> per-row (max, sum-exp)
+//   pass 2 (colsum) : S^T = K_tile Q_j^T   KEYS on the lanes, query-row chunks streamed -> per-key sum_r 2^(s - lse_r)
+// Both are the same warp-specialised skeleton: a fixed 128-row operand A and a 2-stage TMA ring of 128-row operands B
+// (128-byte swizzle), S double-buffered in TMEM (2 x 128 fp32 columns), one UMMA-issuing thread, and 128 consumer
+// threads that sweep their own TMEM lane.  GQA packing: a "query row" is (token i, head hl) of one kv-head,
+// r = i * G + hl, loaded by TMA boxes {64 elements, G heads, 128/G tokens}.  The Hkv per-head partial column sums are
+// combined in fixed order by the last CTA of each key tile (bit-reproducible scores, deterministic top-k).
+#include "qcf_internal.cuh"
+#include "sm100_ptx.cuh"
+
+namespace qcf {
+
+namespace {
+
+using namespace ptx;
+
+constexpr int BT = 128;            // rows of A, rows of one B tile, fp32 columns of one S buffer
+constexpr int kThreads = 192;
+constexpr int kTmemCols = 256;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kRescaleThreshold = 8.0f;
+
+template <int D>
+struct Smem {
+  static constexpr int kBlk = BT * 128;                 // one 64-column block (128 rows x 128 B)
+  static constexpr int kTile = BT * D * 2;
+  static constexpr int oA = 0;
+  static constexpr int oB = kTile;
+  static constexpr int oLse = oB + 2 * kTile;           // pass 2: lse of the 128 streamed query rows, double-buffered
+  static constexpr int oBar = oLse + 2 * BT * 4;
+  static constexpr int kNumBar = 9;
+  static constexpr int oTmem = oBar + kNumBar * 8;
+  static constexpr int oFlag = oTmem + 8;
+  static constexpr int kBytes = oFlag + 8;
+};
+enum { kAFull = 0, kBFull = 1, kBEmpty = 3, kSFull = 5, kSEmpty = 7 };
+
+struct ScoreArgs {
+  float scale_log2;
+  int hq, hkv, n_splits;
+  float* stats_m; float* stats_l; int stats_rows;        // [B][n_splits][stats_rows]
+  float* part; int part_stride;                          // [B][Hkv][part_stride]
+  unsigned int* counters;
+  float* scores; int accumulate;
+};
+
+template <int D, int PASS>
+__global__ void __launch_bounds__(kThreads, 2)
+score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k, BatchDev bd,
+                ScoreArgs a) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  using S = Smem<D>;
+  const int G = a.hq / a.hkv;
+  const int TPT = BT / G;                         // query tokens per 128-row tile
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  // ---- work decode
+  int b, g, row_tile = 0, key_tile = 0, split = 0;
+  if (PASS == 1) {
+    split = blockIdx.x; row_tile = blockIdx.y; g = blockIdx.z % a.hkv; b = blockIdx.z / a.hkv;
+  } else {
+    key_tile = blockIdx.x; g = blockIdx.y; b = blockIdx.z;
+  }
+  const int N = bd.n_ctx[b], Lq = bd.n_query[b];
+  const int rows = Lq * G;
+  int k_begin = 0, k_end = 0, n_j = 0;
+  if (PASS == 1) {
+    if (row_tile * BT >= rows) return;
+    const int span = (((N + a.n_splits - 1) / a.n_splits + BT - 1) / BT) * BT;
+    k_begin = split * span;
+    k_end = min(N, k_begin + span);
+    n_j = k_end > k_begin ? (k_end - k_begin + BT - 1) / BT : 0;
+  } else {
+    if (key_tile * BT >= N) return;
+    n_j = (rows + BT - 1) / BT;
+  }
+
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t sA = sbase + S::oA, sB = sbase + S::oB;
+  auto bar = [&](int i) -> uint32_t { return sbase + S::oBar + 8 * i; };
+  volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + S::oTmem);
+  float* s_lse = reinterpret_cast<float*>(smem + S::oLse);
+
+  if (warp == 0) {
+    if (lane == 0) {
+      prefetch_tensormap(&tm_q);
+      prefetch_tensormap(&tm_k);
+      mbar_init(bar(kAFull), 1);
+      for (int i = 0; i < 2; ++i) {
+        mbar_init(bar(kBFull + i), 1);
+        mbar_init(bar(kBEmpty + i), 1);
+        mbar_init(bar(kSFull + i), 1);
+        mbar_init(bar(kSEmpty + i), 128);
+      }
+      fence_barrier_init();
+    }
+  } else if (warp == 1) {
+    tmem_alloc<kTmemCols>(sbase + S::oTmem);
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  // TMA coordinates of a 128-row tile of query rows / of keys
+  auto load_q_tile = [&](uint32_t dst, uint32_t mbar, int tile) {
+#pragma unroll
+    for (int kb = 0; kb < D / 64; ++kb) tma_load_4d(dst + kb * S::kBlk, &tm_q, mbar, kb * 64, g * G, tile * TPT, b);
+  };
+  auto load_k_tile = [&](uint32_t dst, uint32_t mbar, int key0) {
+#pragma unroll
+    for (int kb = 0; kb < D / 64; ++kb) tma_load_4d(dst + kb * S::kBlk, &tm_k, mbar, kb * 64, g, key0, b);
+  };
+
+  if (warp == 0) {
+    // ===================================================================== producer
+    if (n_j > 0 && lane == 0) {
+      mbar_arrive_expect_tx(bar(kAFull), S::kTile);
+      if (PASS == 1) load_q_tile(sA, bar(kAFull), row_tile); else load_k_tile(sA, bar(kAFull), key_tile * BT);
+    }
+    for (int j = 0; j < n_j; ++j) {
+      const int st = j & 1;
+      const uint32_t ph = (j >> 1) & 1;
+      if (lane == 0) {
+        mbar_wait(bar(kBEmpty + st), ph ^ 1);
+        mbar_arrive_expect_tx(bar(kBFull + st), S::kTile);
+        if (PASS == 1) load_k_tile(sB + st * S::kTile, bar(kBFull + st), k_begin + j * BT);
+        else load_q_tile(sB + st * S::kTile, bar(kBFull + st), j);
+      }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ===================================================================== UMMA issuer
+    if (lane == 0 && n_j > 0) {
+      constexpr uint32_t idesc = umma_idesc_bf16(BT, BT, false, false);
+      mbar_wait(bar(kAFull), 0);
+      for (int j = 0; j < n_j; ++j) {
+        const int st = j & 1;
+        const uint32_t ph = (j >> 1) & 1;
+        mbar_wait(bar(kSEmpty + st), ph ^ 1);               // consumers have released S_{j-2}
+        mbar_wait(bar(kBFull + st), ph);
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < D / 16; ++ks) {
+          const uint32_t koff = (ks >> 2) * S::kBlk + (ks & 3) * 32;
+          umma_ss(tmem_base + st * BT, umma_smem_desc_sw128(sA + koff, 16, 1024),
+                  umma_smem_desc_sw128(sB + st * S::kTile + koff, 16, 1024), idesc, ks > 0 ? 1u : 0u);
+        }
+        umma_commit(bar(kBEmpty + st));
+        umma_commit(bar(kSFull + st));
+      }
+    }
+    __syncwarp();
+  } else {
+    // ===================================================================== consumers: one TMEM lane each
+    const int quarter = warp & 3;
+    const int r = quarter * 32 + lane;
+    const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16);
+    if (PASS == 1) {
+      // lane = query row: online (max, sum-exp) over the streamed keys, reference max moved lazily
+      float m_ref = -INFINITY, l = 0.f;
+      for (int j = 0; j < n_j; ++j) {
+        const int st = j & 1;
+        const int key0 = k_begin + j * BT;
+        const bool tail = key0 + BT > k_end;
+        mbar_wait(bar(kSFull + st), (j >> 1) & 1);
+        tc_fence_after();
+        float tile_max, tile_sum;
+        auto sweep = [&](float ref, bool with_sum) {
+          float mx0 = -INFINITY, mx1 = -INFINITY, l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+#pragma unroll
+          for (int c = 0; c < BT / 32; ++c) {
+            uint32_t s[32];
+            tmem_ld32(lane_addr + st * BT + c * 32, s);
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; i += 4) {
+              float v0 = __uint_as_float(s[i]), v1 = __uint_as_float(s[i + 1]);
+              float v2 = __uint_as_float(s[i + 2]), v3 = __uint_as_float(s[i + 3]);
+              if (tail) {
+                const int k = key0 + c * 32 + i;
+                if (k >= k_end) v0 = -INFINITY;
+                if (k + 1 >= k_end) v1 = -INFINITY;
+                if (k + 2 >= k_end) v2 = -INFINITY;
+                if (k + 3 >= k_end) v3 = -INFINITY;
+              }
+              mx0 = fmaxf(mx0, fmaxf(v0, v1)); mx1 = fmaxf(mx1, fmaxf(v2, v3));
+              if (with_sum) {
+                l0 += ex2(fmaf(v0, a.scale_log2, -ref)); l1 += ex2(fmaf(v1, a.scale_log2, -ref));
+                l2 += ex2(fmaf(v2, a.scale_log2, -ref)); l3 += ex2_poly(fmaf(v3, a.scale_log2, -ref));
+              }
+            }
+          }
+          tile_max = fmaxf(mx0, mx1) * a.scale_log2;
+          tile_sum = (l0 + l1) + (l2 + l3);
+        };
+        if (j == 0) {
+          sweep(0.f, false);
+          m_ref = tile_max;                       // the first tile of a non-empty range has >= 1 valid key: finite
+          sweep(m_ref, true);
+        } else {
+          sweep(m_ref, true);
+          if (__any_sync(0xffffffffu, tile_max > m_ref + kRescaleThreshold)) {
+            const float m_t = fmaxf(m_ref, tile_max);
+            l *= ex2(m_ref - m_t);
+            m_ref = m_t;
+            sweep(m_ref, true);
+          }
+        }
+        l += tile_sum;
+        tc_fence_before();
+        mbar_arrive(bar(kSEmpty + st));
+      }
+      const int row = row_tile * BT + r;
+      if (row < rows) {
+        const size_t o = (static_cast<size_t>(b) * a.n_splits + split) * a.stats_rows + static_cast<size_t>(g) * rows + row;
+        a.stats_m[o] = m_ref;                      // empty key range: (-inf, 0), neutral in the combine
+        a.stats_l[o] = l;
+      }
+    } else {
+      // lane = key: sum over the streamed query rows of 2^(s * scale - lse_row)
+      float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
+      for (int j = 0; j < n_j; ++j) {
+        const int st = j & 1;
+        {
+          // lse2 of this thread's row of the chunk: combine the pass-1 partials (log2 domain); overlaps the TMA / UMMA
+          // latency of the chunk.  The slot was last read two chunks ago; the barrier of the chunk in between orders it.
+          const int row = j * BT + r;
+          float lse = INFINITY;                              // rows past the end contribute 2^(-inf) = 0
+          if (row < rows) {
+            // partials are laid out [split][row]: for a fixed split the 128 threads read consecutive words
+            const size_t o = static_cast<size_t>(b) * a.n_splits * a.stats_rows + static_cast<size_t>(g) * rows + row;
+            float M = -INFINITY, L = 0.f;
+#pragma unroll 8
+            for (int sidx = 0; sidx < a.n_splits; ++sidx) {
+              const float m_s = __ldcg(a.stats_m + o + static_cast<size_t>(sidx) * a.stats_rows);
+              const float l_s = __ldcg(a.stats_l + o + static_cast<size_t>(sidx) * a.stats_rows);
+              const float Mn = fmaxf(M, m_s);
+              if (Mn > -INFINITY) L = L * ex2(M - Mn) + l_s * ex2(m_s - Mn);
+              M = Mn;
+            }
+            lse = M + log2f(L);
+          }
+          s_lse[st * BT + r] = lse;
+          asm volatile("bar.sync 1, 128;" ::: "memory");
+        }
+        mbar_wait(bar(kSFull + st), (j >> 1) & 1);
+        tc_fence_after();
+        const float4* lse4 = reinterpret_cast<const float4*>(s_lse + st * BT);
+        const int n_valid = rows - j * BT;                   // < BT only in the last chunk
+#pragma unroll
+        for (int c = 0; c < BT / 32; ++c) {
+          uint32_t s[32];
+          tmem_ld32(lane_addr + st * BT + c * 32, s);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; i += 4) {
+            const float4 z = lse4[c * 8 + (i >> 2)];         // same address in every lane: broadcast
+            float p0 = ex2(fmaf(__uint_as_float(s[i]), a.scale_log2, -z.x));
+            float p1 = ex2(fmaf(__uint_as_float(s[i + 1]), a.scale_log2, -z.y));
+            float p2 = ex2(fmaf(__uint_as_float(s[i + 2]), a.scale_log2, -z.z));
+            float p3 = ex2_poly(fmaf(__uint_as_float(s[i + 3]), a.scale_log2, -z.w));
+            if (n_valid < BT) {                              // rows past the end hold whatever the buffer holds
+              const int col = c * 32 + i;
+              if (col >= n_valid) p0 = 0.f;
+              if (col + 1 >= n_valid) p1 = 0.f;
+              if (col + 2 >= n_valid) p2 = 0.f;
+              if (col + 3 >= n_valid) p3 = 0.f;
+            }
+            acc0 += p0; acc1 += p1; acc2 += p2; acc3 += p3;
+          }
+        }
+        tc_fence_before();
+        mbar_arrive(bar(kSEmpty + st));
+      }
+      const int key = key_tile * BT + r;
+      if (key < N) a.part[(static_cast<size_t>(b) * a.hkv + g) * a.part_stride + key] = (acc0 + acc1) + (acc2 + acc3);
+    }
+  }
+
+  if (PASS == 2) {
+    // last CTA of this key tile sums the Hkv partials in fixed order (deterministic)
+    volatile int* s_last = reinterpret_cast<volatile int*>(smem + S::oFlag);
+    __threadfence();
+    __syncthreads();
+    const int n_tiles_b = (bd.n_stride + BT - 1) / BT;
+    unsigned int* ctr = a.counters + static_cast<size_t>(b) * n_tiles_b + key_tile;
+    if (threadIdx.x == 0) *s_last = (atomicAdd(ctr, 1u) == static_cast<unsigned int>(a.hkv - 1));
+    __syncthreads();
+    if (*s_last) {
+      __threadfence();
+      const int key = key_tile * BT + static_cast<int>(threadIdx.x);
+      if (threadIdx.x < BT && key < N) {
+        float sum = 0.f;
+        for (int gg = 0; gg < a.hkv; ++gg) sum += __ldcg(a.part + (static_cast<size_t>(b) * a.hkv + gg) * a.part_stride + key);
+        const float v = rows > 0 ? sum / static_cast<float>(a.hq * Lq) : 0.f;
+        float* dst = a.scores + static_cast<size_t>(b) * bd.n_stride + key;
+        *dst = a.accumulate ? *dst + v : v;
+      }
+      if (threadIdx.x == 0) *ctr = 0u;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc<kTmemCols>(tmem_base);
+  }
+}
+
+using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                              const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeFn get_encode() {
+  static EncodeFn fn = []() -> EncodeFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<EncodeFn>(p);
+  }();
+  return fn;
+}
+// [B][T][H][d] bf16; box = {64 elements, box_heads heads, box_rows rows}; 128-byte swizzle; zero fill out of bounds
+bool make_map(CUtensorMap* m, const void* base, int batch, int t_stride, int heads, int d, int box_heads, int box_rows) {
+  EncodeFn enc = get_encode();
+  if (!enc) return false;
+  const cuuint64_t dims[4] = {static_cast<cuuint64_t>(d), static_cast<cuuint64_t>(heads),
+                              static_cast<cuuint64_t>(t_stride), static_cast<cuuint64_t>(batch)};
+  const cuuint64_t strides[3] = {static_cast<cuuint64_t>(d) * 2, static_cast<cuuint64_t>(heads) * d * 2,
+                                 static_cast<cuuint64_t>(t_stride) * heads * d * 2};
+  const cuuint32_t box[4] = {64, static_cast<cuuint32_t>(box_heads), static_cast<cuuint32_t>(box_rows), 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int D>
+cudaError_t launch(const qcf_ctx* ctx, const qcf_batch* b, const CUtensorMap& tm_q, const CUtensorMap& tm_k,
+                   ScoreArgs a, int row_tiles, int key_tiles, cudaStream_t stream) {
+  const int smem = Smem<D>::kBytes + 1024;
+  if (row_tiles > 0) {
+    auto k1 = score_tc_kernel<D, 1>;
+    cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    k1<<<dim3(a.n_splits, row_tiles, b->batch * a.hkv), kThreads, smem, stream>>>(tm_q, tm_k, b->dev, a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  auto k2 = score_tc_kernel<D, 2>;
+  cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  k2<<<dim3(key_tiles, a.hkv, b->batch), kThreads, smem, stream>>>(tm_q, tm_k, b->dev, a);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_score_tc(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* q_probe,
+                            const __nv_bfloat16* k_f, float* scores, int accumulate, cudaStream_t stream) {
+  if (b->batch == 0 || b->max_ctx == 0) return cudaSuccess;
+  const Layout& L = ctx->lay;
+  const int max_rows = b->max_query * L.g;
+  const int row_tiles = (max_rows + BT - 1) / BT;
+  const int key_tiles = (b->max_ctx + BT - 1) / BT;
+  // enough key splits in pass 1 to fill the machine twice, at least one 128-key tile each
+  int n_splits = 1;
+  if (row_tiles > 0) {
+    const int ctas = row_tiles * L.hkv * b->batch;
+    n_splits = (2 * ctx->n_sm) / ctas;            // one resident wave (2 CTAs per SM)
+    if (n_splits > key_tiles) n_splits = key_tiles;
+    if (n_splits > kScoreSplitsMax) n_splits = kScoreSplitsMax;
+    if (n_splits < 1) n_splits = 1;
+  }
+  CUtensorMap tm_q, tm_k;
+  // q_probe may be NULL when no request has query tokens: map a valid dummy address (never dereferenced: n_j == 0)
+  const void* qbase = q_probe ? static_cast<const void*>(q_probe) : static_cast<const void*>(k_f);
+  if (!make_map(&tm_q, qbase, b->batch, b->q_stride > 0 ? b->q_stride : 1, L.hq, L.d, L.g, BT / L.g) ||
+      !make_map(&tm_k, k_f, b->batch, b->t_stride, L.hkv, L.d, 1, BT))
+    return cudaErrorInvalidValue;
+  ScoreArgs a;
+  a.scale_log2 = L.scale * kLog2e;
+  a.hq = L.hq; a.hkv = L.hkv; a.n_splits = n_splits;
+  a.stats_m = ctx->stats_m; a.stats_l = ctx->stats_l; a.stats_rows = L.hq * ctx->max_query;
+  a.part = ctx->score_part; a.part_stride = ctx->max_ctx;
+  a.counters = ctx->counters;
+  a.scores = scores; a.accumulate = accumulate;
+  return L.d == 128 ? launch<128>(ctx, b, tm_q, tm_k, a, row_tiles, key_tiles, stream)
+                    : launch<64>(ctx, b, tm_q, tm_k, a, row_tiles, key_tiles, stream);
+}
+
+}  // namespace qcf
