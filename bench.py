@@ -10,8 +10,9 @@ independent, so every rank runs its own replica of the worklo
 weak scaling; `value` = tokens all ranks processed / max-over-ranks device time.
 
 Timing: W >= 3 warm-up steps, then exactly K steps, each bracketed by CUDA events on the launching stream; an L2
-flush (a write of a 256 MiB buffer, outside the event pair) precedes every step because the c2 working set fits the
-126 MB L2.  Barrier + synchronize on both sides of the timed region; max over ranks.
+flush (a write of a 256 MiB buffer followed by a read of a second 256 MiB buffer, so that the cache is left full of
+CLEAN foreign lines; outside the event pair) precedes every step because the c2 working set fits the 126 MB L2.
+Barrier + synchronize on both sides of the timed region; max over ranks.
 """
 from __future__ import annotations
 
@@ -211,7 +212,12 @@ def run_qcf(args) -> None:
     dw = device.DeviceWorkload(wl, ctx, device=dev)
     largs = dw.layer_args(lse=None)
     tokens_per_step = int(dw.batch.total_ctx)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    flush_w = torch.empty(256 << 20, dtype=torch.uint8, device=dev)    # > 126 MB L2
+    flush_r = torch.zeros(64 << 20, dtype=torch.int32, device=dev)     # 256 MiB, read after the write
+
+    def flush_l2(i):
+        flush_w.fill_(i & 0xff)        # evicts everything ...
+        flush_r.max()                  # ... and the read pass replaces the dirty lines by clean ones
 
     def barrier():
         torch.cuda.synchronize()
@@ -227,14 +233,14 @@ def run_qcf(args) -> None:
     # ---- device-resident leg: per-step events, per-stage events (qcf profiling hooks record on the same stream)
     ctx.qcf_set_profiling(True)
     for _ in range(max(args.warmup, 3)):
-        flush.fill_(1)
+        flush_l2(1)
         ctx.qcf_layer_step(dw.batch, largs)
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     ctx.qcf_get_stage_ms()                          # forget the warm-up steps
     stage_acc, stage_n = np.zeros(5), 0
     for i in range(args.steps):
-        flush.fill_(i & 0xff)
+        flush_l2(i)
         ev[i][0].record()
         ctx.qcf_layer_step(dw.batch, largs)
         ev[i][1].record()
@@ -247,6 +253,21 @@ def run_qcf(args) -> None:
     step_ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = float(step_ms.sum())
     ctx.qcf_set_profiling(False)
+
+    # ---- comparator: the library's own dense causal attention over all N + Lq rows (Eq. 2), same flush protocol
+    out_full = torch.empty_like(dw.out)
+    n_full = max(3, min(args.steps, 30))
+    evf = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_full)]
+    for i in range(3 + n_full):
+        flush_l2(i)
+        if i >= 3:
+            evf[i - 3][0].record()
+        ctx.qcf_full_prefill_attn(dw.batch, dw.q_new, dw.k_new, dw.v_new, out_full)
+        if i >= 3:
+            evf[i - 3][1].record()
+    barrier()
+    full_ms = float(np.mean([a.elapsed_time(b) for a, b in evf]))
+    del out_full
 
     # ---- end-to-end leg: the same step through the C ABI with HOST (pinned) buffers, copies inside the timed region
     e2e = None
@@ -269,10 +290,10 @@ def run_qcf(args) -> None:
     clocks = sampler.stop() if rank == 0 else None
 
     # ---- max over ranks
-    t = torch.tensor([total_ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
+    t = torch.tensor([total_ms, e2e[0] if e2e else 0.0, full_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_s = float(t[0]), float(t[1])
+    total_ms, e2e_s, full_ms = float(t[0]), float(t[1]), float(t[2])
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -308,12 +329,17 @@ def run_qcf(args) -> None:
         "a5_attn": {"ms": a5_ms, "TFLOPps": achieved},
     }
 
+    full_flops = sum(device.attn_flops(cfg, n, np.arange(n + lq)) for n, lq in zip(dw.batch.n_ctx, dw.batch.n_query))
+    comparator = {"kernel": "qcf_full_prefill_attn (dense causal GQA over all N+Lq rows, Eq. 2)", "ms": full_ms,
+                  "TFLOPps": full_flops / (full_ms * 1e-3) / 1e12, "frac_tensor_peak": full_flops / (full_ms * 1e-3) / 1e12 / peak,
+                  "selective_step_over_full_prefill_attn": ms_per_step / full_ms}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
-        "config": config_dict(wl, args, l2="flushed before every timed step (256 MiB write, outside the event pair)"),
+        "config": config_dict(wl, args, l2="flushed before every timed step (256 MiB write then 256 MiB read, outside the event pair)"),
         "clocks": clocks, "gpu_launches": KERNELS_PER_STEP * args.steps, "roofline": roofline, "stages": stages,
+        "full_prefill_attn": comparator,
         "step_ms_min_med_max": [float(step_ms.min()), float(np.median(step_ms)), float(step_ms.max())],
     }
     if e2e:

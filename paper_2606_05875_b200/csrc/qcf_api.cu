@@ -128,6 +128,10 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
     c->attn_impl = (e && std::strcmp(e, "mma") == 0) ? 0 : 1;
     const char* e2 = std::getenv("QCF_SCORE_IMPL");
     c->score_impl = (e2 && std::strcmp(e2, "mma") == 0) ? 0 : 1;
+    const char* e3 = std::getenv("QCF_ATTN_CLUSTER");
+    const int cl = e3 ? std::atoi(e3) : 0;
+    c->attn_cluster = (cl == 1 || cl == 2 || cl == 4) ? cl : 0;
+    c->ratio_hint = 0.3;
   }
   c->profiling = 0; c->ev_valid = false;
   c->ev_ring = nullptr; c->ev_count = 0; c->ev = nullptr;
@@ -323,6 +327,7 @@ qcf_status qcf_select_topk(qcf_ctx* ctx, const qcf_batch* b, const float* scores
   if (b->batch == 0) return QCF_OK;
   QCF_REQUIRE(ctx, n_sel != nullptr, "qcf_select_topk: n_sel is NULL");
   QCF_REQUIRE(ctx, (scores && sel) || b->n_stride == 0, "qcf_select_topk: NULL tensor pointer");
+  ctx->ratio_hint = ratio;
   QCF_CUDA(ctx, launch_topk(ctx, b, scores, ratio, sel, n_sel, static_cast<cudaStream_t>(stream)));
   return QCF_OK;
 }

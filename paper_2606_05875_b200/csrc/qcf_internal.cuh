@@ -47,6 +47,8 @@ struct qcf_ctx {
   int max_batch, max_ctx, max_query;
   int score_impl;        // 1: tcgen05 kernels (default); 0: legacy mma.sync kernels (QCF_SCORE_IMPL=mma)
   int attn_impl;         // 1: tcgen05/TMEM/TMA kernel (default); 0: legacy mma.sync kernel (QCF_ATTN_IMPL=mma, for A/B timing)
+  int attn_cluster;      // split-KV cluster size of the tcgen05 attention kernel: 0 = heuristic, else 1/2/4 (QCF_ATTN_CLUSTER)
+  double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
   // workspace (device)
   float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]
   float* stats_l;        // score pass-1 partial row sum-exp

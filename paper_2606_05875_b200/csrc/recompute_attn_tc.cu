@@ -10,6 +10,13 @@
 //               lazy rescale of O (only when the running max grows by more than 2^8), final normalisation + store
 // The causal limit is monotone in the tile (rows ascending), so only key tiles reaching past the tile's first position
 // are masked and the key loop stops at the tile's last position.  sel == nullptr is the dense comparator (Eq. 2).
+//
+// Split-KV over a thread-block cluster: when the problem is too small to balance (the heaviest tile is a large share
+// of an SM's load) the key tiles of one work item are divided among the 1, 2 or 4 CTAs of a cluster.  Ranks > 0 park
+// their unnormalised O (fp32) and (m, l) in their own shared memory (the drained K/V rings), rank 0 pulls them over
+// distributed shared memory, merges in rank order (deterministic) and stores.  No global workspace, no atomics.
+#include <cmath>
+
 #include "qcf_internal.cuh"
 #include "sm100_ptx.cuh"
 
@@ -44,10 +51,41 @@ struct Smem {
   static constexpr int oBar = oV + kStages * kTile;        // mbarriers (8 B each)
   static constexpr int kNumBar = 4 * kStages + 6;
   static constexpr int oTmem = oBar + kNumBar * 8;
-  static constexpr int kBytes = oTmem + 16;
+  static constexpr int oStat = oTmem + 16;                 // split-KV: (m, l) of this CTA's 128 rows
+  static constexpr int kBytes = oStat + 2 * BM * 4;
+  static_assert(2 * kStages * kTile >= BM * D * 4, "the K/V rings must hold one fp32 O tile for the split-KV merge");
 };
 enum { kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages, kSFull = 4 * kStages,
        kPReady = 4 * kStages + 2, kODone = 4 * kStages + 4 };
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {        // every thread of every CTA of the cluster
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local_smem_addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_smem_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ float ld_dsmem_f32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ float4 ld_dsmem_f32x4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+  return v;
+}
 
 template <int D>
 __global__ void __launch_bounds__(kThreads, 2)
@@ -62,9 +100,13 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int G = hq / hkv;
   const int PT = BM / G;
   // 1-D grid, heaviest tiles of ALL (request, kv-head) pairs first: block id -> (tile descending, head, request)
+  // The CTAs of a cluster (consecutive block ids) share one work item and split its key tiles.
+  const int ncl = static_cast<int>(cluster_nctarank());
+  const int crank = static_cast<int>(cluster_ctarank());
+  const int item = static_cast<int>(blockIdx.x) / ncl;
   const int n_gb = hkv * bd.batch;
-  const int tile = max_tiles - 1 - static_cast<int>(blockIdx.x) / n_gb;
-  const int gb = static_cast<int>(blockIdx.x) % n_gb;
+  const int tile = max_tiles - 1 - item / n_gb;
+  const int gb = item % n_gb;
   const int b = gb / hkv, g = gb % hkv;
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
   const bool dense = sel == nullptr;
@@ -81,7 +123,11 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   };
   const int p_min = pos_of(ridx0);
   const int p_max = pos_of(min(ridx0 + PT, n_rows) - 1);
-  const int n_kt = p_max / BN + 1;
+  const int n_kt_all = p_max / BN + 1;
+  // this CTA's key tiles: [jt0, jt0 + n_kt); rank 0 always has at least one, ranks > 0 none when n_kt_all < ncl
+  const int kt_base = n_kt_all / ncl, kt_rem = n_kt_all % ncl;
+  const int jt0 = crank * kt_base + min(crank, kt_rem);
+  const int n_kt = kt_base + (crank < kt_rem ? 1 : 0);
   const int t_end = N + Lq;                  // rows >= t_end of the cache are padding
 
   const uint32_t sbase = smem_u32(smem);
@@ -132,12 +178,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         mbar_arrive_expect_tx(bar(kFullK + st), S::kTile);
 #pragma unroll
         for (int kb = 0; kb < D / 64; ++kb)
-          tma_load_4d(sK + st * S::kTile + kb * S::kBlk, &tm_k, bar(kFullK + st), kb * 64, g, j * BN, b);
+          tma_load_4d(sK + st * S::kTile + kb * S::kBlk, &tm_k, bar(kFullK + st), kb * 64, g, (jt0 + j) * BN, b);
         mbar_wait(bar(kEmptyV + st), ph ^ 1);
         mbar_arrive_expect_tx(bar(kFullV + st), S::kTile);
 #pragma unroll
         for (int kb = 0; kb < D / 64; ++kb)
-          tma_load_4d(sV + st * S::kTile + kb * S::kBlk, &tm_v, bar(kFullV + st), kb * 64, g, j * BN, b);
+          tma_load_4d(sV + st * S::kTile + kb * S::kBlk, &tm_v, bar(kFullV + st), kb * 64, g, (jt0 + j) * BN, b);
       }
     }
     __syncwarp();
@@ -162,7 +208,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         umma_commit(bar(kEmptyK + st));
         umma_commit(bar(kSFull + (j & 1)));
       };
-      issue_qk(0);
+      if (n_kt > 0) issue_qk(0);
       for (int j = 0; j < n_kt; ++j) {
         if (j + 1 < n_kt) issue_qk(j + 1);
         const int st = j % kStages;
@@ -191,7 +237,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     float m_used = -INFINITY, l = 0.f;
 
     for (int j = 0; j < n_kt; ++j) {
-      const int key0 = j * BN;
+      const int key0 = (jt0 + j) * BN;
       const bool need_mask = key0 + BN - 1 > p_min;     // tile reaches past the tile's first position
       const uint32_t s_addr = lane_addr + (j & 1) * BN;
       mbar_wait(bar(kSFull + (j & 1)), (j >> 1) & 1);
@@ -238,7 +284,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
       };
 
       if (j == 0) {
-        // first tile: the reference is its own max (key 0 is visible to every row, so it is finite)
+        // first tile: the reference is its own max.  Key 0 is visible to every row, so it is finite on rank 0; on a
+        // split-KV rank > 0 a row may see none of this CTA's keys: the clamp keeps the reference finite (p = 0, l = 0).
         float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
         for (int c = 0; c < BN / 32; ++c) {
@@ -249,13 +296,13 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
           for (int i = 0; i < 32; i += 2) {
             float v0 = __uint_as_float(t[i]), v1 = __uint_as_float(t[i + 1]);
             if (need_mask) {
-              if (c * 32 + i > pos) v0 = -INFINITY;
-              if (c * 32 + i + 1 > pos) v1 = -INFINITY;
+              if (key0 + c * 32 + i > pos) v0 = -INFINITY;
+              if (key0 + c * 32 + i + 1 > pos) v1 = -INFINITY;
             }
             mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1);
           }
         }
-        m_used = fmaxf(mx0, mx1) * scale_log2;
+        m_used = fmaxf(fmaxf(mx0, mx1) * scale_log2, -1e30f);
         sweep(m_used);
       } else {
         sweep(m_used);
@@ -304,29 +351,109 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     }
 
     // epilogue: O / l -> bf16 -> global (each thread owns one (row, head) vector of D elements)
-    mbar_wait(bar(kODone + ((n_kt - 1) & 1)), ((n_kt - 1) >> 1) & 1);
-    tc_fence_after();
-    const float inv = 1.f / l;
+    if (n_kt > 0) {
+      mbar_wait(bar(kODone + ((n_kt - 1) & 1)), ((n_kt - 1) >> 1) & 1);
+      tc_fence_after();
+    } else {
+      m_used = -1e30f;                                       // no keys on this rank: neutral element of the merge
+    }
     __nv_bfloat16* dst = out + ((static_cast<size_t>(b) * bd.t_stride + ridx) * hq + g * G + hl) * D;
+    float w_own = 1.f, m_all = m_used;
+    float w_rem[3] = {0.f, 0.f, 0.f};
+    if (ncl > 1) {
+      // ---- split-KV merge.  Ranks > 0 park (O, m, l) in their own shared memory: all of this CTA's TMA loads and
+      // UMMAs have completed (o_done of the last tile), so the K/V rings are free.  O is laid out [D/4][128 rows] float4
+      // so that both the local stores and rank 0's remote loads are conflict-free.
+      float* s_stat = reinterpret_cast<float*>(smem + S::oStat);
+      if (crank > 0) {
+        float4* park = reinterpret_cast<float4*>(smem + S::oK);
 #pragma unroll
-    for (int c = 0; c < D / 32; ++c) {
-      uint32_t o[32];
-      tmem_ld32(lane_addr + kColO + c * 32, o);
-      tmem_wait_ld();
-      if (valid) {
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t o[32];
+          if (n_kt > 0) {
+            tmem_ld32(lane_addr + kColO + c * 32, o);
+            tmem_wait_ld();
+          } else {
 #pragma unroll
-        for (int v4 = 0; v4 < 4; ++v4) {
-          uint4 w;
-          w.x = pack_bf16(__uint_as_float(o[8 * v4 + 0]) * inv, __uint_as_float(o[8 * v4 + 1]) * inv);
-          w.y = pack_bf16(__uint_as_float(o[8 * v4 + 2]) * inv, __uint_as_float(o[8 * v4 + 3]) * inv);
-          w.z = pack_bf16(__uint_as_float(o[8 * v4 + 4]) * inv, __uint_as_float(o[8 * v4 + 5]) * inv);
-          w.w = pack_bf16(__uint_as_float(o[8 * v4 + 6]) * inv, __uint_as_float(o[8 * v4 + 7]) * inv);
-          *reinterpret_cast<uint4*>(dst + c * 32 + v4 * 8) = w;
+            for (int i = 0; i < 32; ++i) o[i] = 0u;
+          }
+#pragma unroll
+          for (int v4 = 0; v4 < 8; ++v4)
+            park[(c * 8 + v4) * BM + r] = make_float4(__uint_as_float(o[4 * v4]), __uint_as_float(o[4 * v4 + 1]),
+                                                      __uint_as_float(o[4 * v4 + 2]), __uint_as_float(o[4 * v4 + 3]));
+        }
+        s_stat[r] = m_used;
+        s_stat[BM + r] = l;
+      }
+    }
+    if (ncl > 1) {
+      cluster_sync_all();                                    // parked partials are visible cluster-wide
+      if (crank == 0) {
+        float m_r[3] = {-1e30f, -1e30f, -1e30f}, l_r[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+        for (int q = 1; q < 4; ++q) {
+          if (q < ncl) {
+            const uint32_t st_addr = dsmem_addr(sbase + S::oStat + r * 4, q);
+            m_r[q - 1] = ld_dsmem_f32(st_addr);
+            l_r[q - 1] = ld_dsmem_f32(st_addr + BM * 4);
+            m_all = fmaxf(m_all, m_r[q - 1]);
+          }
+        }
+        w_own = ex2(m_used - m_all);
+        l *= w_own;
+#pragma unroll
+        for (int q = 1; q < 4; ++q) {                        // fixed rank order: bit-reproducible
+          if (q < ncl) {
+            w_rem[q - 1] = ex2(m_r[q - 1] - m_all);
+            l += l_r[q - 1] * w_rem[q - 1];
+          }
         }
       }
     }
-    if (valid && lse_out)
-      lse_out[(static_cast<size_t>(b) * bd.t_stride + ridx) * hq + g * G + hl] = (m_used + log2f(l)) * kLn2;
+    if (crank == 0) {
+      const float inv = 1.f / l;
+#pragma unroll
+      for (int c = 0; c < D / 32; ++c) {
+        uint32_t o[32];
+        tmem_ld32(lane_addr + kColO + c * 32, o);
+        tmem_wait_ld();
+        if (ncl > 1) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * w_own);
+#pragma unroll
+          for (int q = 1; q < 4; ++q) {
+            if (q >= ncl) break;
+            const uint32_t base = dsmem_addr(sK + (c * 8 * BM + r) * 16, q);
+            const float w = w_rem[q - 1];
+#pragma unroll
+            for (int v4 = 0; v4 < 8; ++v4) {
+              const float4 t = ld_dsmem_f32x4(base + v4 * BM * 16);
+              o[4 * v4] = __float_as_uint(fmaf(t.x, w, __uint_as_float(o[4 * v4])));
+              o[4 * v4 + 1] = __float_as_uint(fmaf(t.y, w, __uint_as_float(o[4 * v4 + 1])));
+              o[4 * v4 + 2] = __float_as_uint(fmaf(t.z, w, __uint_as_float(o[4 * v4 + 2])));
+              o[4 * v4 + 3] = __float_as_uint(fmaf(t.w, w, __uint_as_float(o[4 * v4 + 3])));
+            }
+          }
+        }
+        if (valid) {
+#pragma unroll
+          for (int v4 = 0; v4 < 4; ++v4) {
+            uint4 w;
+            w.x = pack_bf16(__uint_as_float(o[8 * v4 + 0]) * inv, __uint_as_float(o[8 * v4 + 1]) * inv);
+            w.y = pack_bf16(__uint_as_float(o[8 * v4 + 2]) * inv, __uint_as_float(o[8 * v4 + 3]) * inv);
+            w.z = pack_bf16(__uint_as_float(o[8 * v4 + 4]) * inv, __uint_as_float(o[8 * v4 + 5]) * inv);
+            w.w = pack_bf16(__uint_as_float(o[8 * v4 + 6]) * inv, __uint_as_float(o[8 * v4 + 7]) * inv);
+            *reinterpret_cast<uint4*>(dst + c * 32 + v4 * 8) = w;
+          }
+        }
+      }
+      if (valid && lse_out)
+        lse_out[(static_cast<size_t>(b) * bd.t_stride + ridx) * hq + g * G + hl] = (m_all + log2f(l)) * kLn2;
+    }
+  }
+  if (ncl > 1) {
+    if (warp < 2) cluster_sync_all();                        // producer / issuer warps: pair the softmax warps' first sync
+    cluster_sync_all();                                      // parked partials stay alive until rank 0 has merged them
   }
 
   tc_fence_before();
@@ -382,22 +509,50 @@ cudaError_t launch_attn_tc(const qcf_ctx* ctx, const qcf_batch* b, const int32_t
     return cudaErrorInvalidValue;
   const int PT = BM / L.g;
   const int max_tiles = (b->t_stride + PT - 1) / PT;
-  const dim3 grid(static_cast<unsigned>(max_tiles) * L.hkv * b->batch);
+  // Split-KV width (cluster size).  Splitting costs a second prologue/epilogue per item and a cluster rendezvous, and
+  // measured on c2 (400 items for 296 resident CTAs) it loses to the unsplit launch (112 -> 131 us at 2, 201 us at 4),
+  // so it is used only where the unsplit grid leaves most of the machine empty: few rows against a long cache
+  // (rho ~ 0: the Lq query rows alone give Lq*G/128 items per kv-head).  A scheduling hint only — the selected rows
+  // are device-side: rows ~ ratio_hint * N + Lq in selective mode.
+  int ncl = ctx->attn_cluster;
+  if (ncl == 0) {
+    double items = 0.0;
+    for (int i = 0; i < b->batch; ++i) {
+      const int n = b->h_n_ctx[i], lq = b->h_n_query[i];
+      const double rows = sel ? ctx->ratio_hint * n + lq : static_cast<double>(n + lq);
+      items += std::ceil(rows / PT) * L.hkv;
+    }
+    const double slots = 2.0 * ctx->n_sm;
+    const int kt_max = (b->t_stride + BN - 1) / BN;
+    ncl = (kt_max >= 16 && items * 4 <= slots) ? 4 : ((kt_max >= 8 && items * 2 <= slots) ? 2 : 1);
+  }
+  const dim3 grid(static_cast<unsigned>(max_tiles) * L.hkv * b->batch * ncl);
   const float scale_log2 = L.scale * kLog2e;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(kThreads);
+  cfg.stream = stream;
+  cudaLaunchAttribute attrs[1];
+  attrs[0].id = cudaLaunchAttributeClusterDimension;
+  attrs[0].val.clusterDim.x = static_cast<unsigned>(ncl);
+  attrs[0].val.clusterDim.y = 1;
+  attrs[0].val.clusterDim.z = 1;
+  cfg.attrs = attrs;
+  cfg.numAttrs = 1;
+  const BatchDev bd = b->dev;
+  const int hq = L.hq, hkv = L.hkv;
   if (L.d == 128) {
     auto kern = attn_tc_kernel<128>;
-    const int smem = Smem<128>::kBytes + 1024;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position,
-                                           out, lse);
-  } else {
-    auto kern = attn_tc_kernel<64>;
-    const int smem = Smem<64>::kBytes + 1024;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    kern<<<grid, kThreads, smem, stream>>>(tm_k, tm_v, b->dev, L.hq, L.hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position,
-                                           out, lse);
+    cfg.dynamicSmemBytes = Smem<128>::kBytes + 1024;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(cfg.dynamicSmemBytes));
+    return cudaLaunchKernelEx(&cfg, kern, tm_k, tm_v, bd, hq, hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position,
+                              out, lse);
   }
-  return cudaGetLastError();
+  auto kern = attn_tc_kernel<64>;
+  cfg.dynamicSmemBytes = Smem<64>::kBytes + 1024;
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(cfg.dynamicSmemBytes));
+  return cudaLaunchKernelEx(&cfg, kern, tm_k, tm_v, bd, hq, hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position, out,
+                            lse);
 }
 
 }  // namespace qcf

@@ -276,6 +276,30 @@ def test_recompute_attn_compact_rows():
     _check_recompute(wl, dw, 0, sel)
 
 
+@pytest.mark.parametrize("ncl", [1, 2, 4])
+@pytest.mark.parametrize("name", ["c1", "t_ragged", "t_batch", "t_mid"])
+def test_recompute_attn_split_kv_cluster(name, ncl, monkeypatch):
+    """Split-KV over a 1/2/4-CTA cluster (forced; the default is a host heuristic): same rows, same tolerance, and
+    ranks with no key tiles / rows that see none of a rank's keys merge as neutral elements."""
+    monkeypatch.setenv("QCF_ATTN_CLUSTER", str(ncl))
+    wl, ctx, dw = _setup(name)
+    rng = np.random.default_rng(11 + ncl)
+    sels = []
+    for r in wl.requests:
+        k = O.n_select(r.n_ctx, wl.cfg.ratio)
+        sels.append(np.sort(rng.choice(r.n_ctx, size=k, replace=False)))
+    _run_recompute(ctx, dw, sels)
+    for b in range(dw.B):
+        _check_recompute(wl, dw, b, sels[b])
+    # dense comparator through the same split
+    out2 = torch.zeros_like(dw.out)
+    ctx.qcf_full_prefill_attn(dw.batch, dw.q_new, dw.k_new, dw.v_new, out2)
+    torch.cuda.synchronize()
+    r = wl.requests[0]
+    want = O.full_prefill_attn(O.widen_bf16(r.q_new), O.widen_bf16(r.k_new), O.widen_bf16(r.v_new))
+    assert np.max(np.abs(_f64(out2[0, : r.n_ctx + r.n_query]) - want)) <= 2e-2
+
+
 # --------------------------------------------------------------------------------------------- a6
 
 @pytest.mark.parametrize("name", SMALL)
@@ -381,3 +405,65 @@ def test_error_reporting():
     assert e.value.status == binding.QCF_ERR_INVALID_ARG and "ratio" in str(e.value)
     with pytest.raises(binding.QcfError):
         ctx.qcf_rope_reposition(b, 8, 16, 16, 16)        # misaligned pointer
+
+
+# --------------------------------------------------------------------------------------------- full sizes
+# BASELINE.json's own sizes, in the launch configuration bench.py times (default ctx, chained qcf_layer_step).
+# Scores and the selection are checked in full; attention outputs on a declared row sample (rows are independent
+# given the fused cache, so the oracle computes each sampled row exactly): all query rows, the first 64 and last 64
+# selected rows and 256 seeded random rows.
+
+def _sample_rows(k, lq, seed):
+    rng = np.random.default_rng(seed)
+    first, last = np.arange(min(64, k)), np.arange(max(k - 64, 0), k)
+    rnd = rng.choice(k, size=min(256, k), replace=False) if k > 0 else np.empty(0, np.int64)
+    return np.unique(np.concatenate([first, last, rnd, np.arange(k, k + lq)])).astype(np.int64)
+
+
+def _check_full_size(wl, dw, b, seed):
+    r, k_pic, v_pic = _oracle_inputs(wl, b)
+    n, lq = r.n_ctx, r.n_query
+    k_ctx, v_ctx = O.reposition(k_pic, v_pic, wl.cfg.rope_theta)
+    kf_g = _f64(dw.k_fused[b, : n + lq])
+    want_sc = O.score(O.widen_bf16(r.q_probe), k_ctx)
+    got_sc = dw.scores[b, :n].cpu().numpy().astype(np.float64)
+    np.testing.assert_allclose(got_sc, want_sc, rtol=1e-2, atol=0)            # north_star: scores 1e-2 relative
+    k = int(dw.n_sel[b])
+    assert k == O.n_select(n, wl.cfg.ratio)
+    sel = dw.sel[b, :k].cpu().numpy().astype(np.int64)
+    _check_selection(sel, want_sc, k)
+    assert np.array_equal(sel, O.select_topk(dw.scores[b, :n].cpu().numpy(), k))   # integer work: bit-exact
+    k_f, v_f = O.fuse(k_ctx, v_ctx, sel, O.widen_bf16(r.k_new), O.widen_bf16(r.v_new))
+    assert np.all(np.abs(kf_g - k_f) <= np.maximum(2e-2, _ulp_bf16(k_f)))     # DESIGN.md §5 bound for re-positioned K
+    assert np.array_equal(_f64(dw.v_fused[b, : n + lq]), v_f)
+    rows = np.concatenate([sel, np.arange(n, n + lq)])
+    samp = _sample_rows(k, lq, seed)
+    want = O.recompute_attn(O.widen_bf16(r.q_new[rows[samp]]), rows[samp], k_f, v_f)
+    got = _f64(dw.out[b])[samp]
+    assert np.max(np.abs(got - want)) <= 2e-2                                 # north_star: max-abs 2e-2
+    return len(samp)
+
+
+def test_full_size_c2():
+    wl, ctx, dw = _setup("c2")
+    ctx.qcf_layer_step(dw.batch, dw.layer_args())
+    torch.cuda.synchronize()
+    assert _check_full_size(wl, dw, 0, 21) >= 64 + 128
+
+
+def test_full_size_c5_long_context_heavy_hitters():
+    wl, ctx, dw = _setup("c5")
+    ctx.qcf_layer_step(dw.batch, dw.layer_args())
+    torch.cuda.synchronize()
+    _check_full_size(wl, dw, 0, 22)
+
+
+@pytest.mark.parametrize("ratio", [0.1, 0.5])
+def test_full_size_c4_batched_pool(ratio):
+    """Config 4's request shape and its 256-chunk pool; 3 of the 16 requests (the generator draws chunk sets
+    independently per request, so a smaller batch is a prefix of the full one)."""
+    wl, ctx, dw = _setup("c4", ratio=ratio, batch=3)
+    ctx.qcf_layer_step(dw.batch, dw.layer_args())
+    torch.cuda.synchronize()
+    for b in (0, 2):
+        _check_full_size(wl, dw, b, 23 + b)
