@@ -16,7 +16,7 @@ rho in 0.1..0.5): the datasets and weights are not in the cont
 from __future__ import annotations
 
 from dataclasses import dataclass, field
-from typing import Dict, List, Optional
+from typing import Dict, List, Optional, Tuple
 
 import numpy as np
 
@@ -222,3 +222,91 @@ def make_workload(name: str, *, ratio: Optional[float] = None, batch: Optional[i
             anchor_idx=np.concatenate(a_list).astype(np.int32) if a_list else np.empty(0, np.int32),
             anchor_ptr=a_ptr))
     return wl
+
+
+# --------------------------------------------------------------------------- config 3: full-stack workload
+
+
+@dataclass(frozen=True)
+class StackSpec:
+    """BASELINE.json configs[2] ("c3") and its reduced test shapes: a Qwen3-shaped decoder stack with random-init
+    weights plus one multi-chunk request.  No arithmetic of the method lives here: only seeded tensors."""
+
+    name: str
+    seed: int
+    n_layers: int
+    hidden: int
+    ffn: int
+    vocab: int
+    n_q_heads: int
+    n_kv_heads: int
+    head_dim: int
+    rope_theta: float
+    n_chunks: int
+    chunk_len: int
+    n_query: int
+    ratio: float
+    crit_layers: Tuple[int, ...]      # 0-based layer indices of L* (reading (p): the three middle layers)
+    r_a: float = 0.1                  # anchor retained ratio (PAPER.md:297)
+    rms_eps: float = 1e-6
+
+    @property
+    def n_ctx(self) -> int:
+        return self.n_chunks * self.chunk_len
+
+
+STACKS: Dict[str, StackSpec] = {
+    # configs[2]: 36 layers, hidden 4096, FFN 12288, GQA 32/8, d 128; 20 x 512 context + 64-token query; L* = {17,18,19} (1-based)
+    "c3": StackSpec("c3", 1003, 36, 4096, 12288, 32768, 32, 8, 128, 1e6, 20, 512, 64, 0.3, (16, 17, 18)),
+    # free-running parity stack (SURVEY.md §8(c)): 4 layers, hidden 512, FFN 1536, 8/2 heads, d 64, 4 x 128 tokens
+    "s_small": StackSpec("s_small", 3001, 4, 512, 1536, 1024, 8, 2, 64, 1e6, 4, 128, 16, 0.3, (1, 2)),
+    # d = 128 variant with ragged GEMM tails (hidden 384 = 1.5 K-blocks of 256, n_R not a multiple of 128)
+    "s_d128": StackSpec("s_d128", 3002, 3, 384, 1152, 512, 8, 2, 128, 1e6, 3, 160, 24, 0.35, (0, 2)),
+    # one c3-shaped layer slice for teacher-forced full-width checks: real widths, 2 layers, short context
+    "s_wide": StackSpec("s_wide", 3003, 2, 4096, 12288, 2048, 32, 8, 128, 1e6, 3, 256, 32, 0.3, (0, 1)),
+}
+
+_W_NAMES = ("wq", "wk", "wv", "wo", "wg", "wu", "wd")
+
+
+@dataclass
+class StackWorkload:
+    spec: StackSpec
+    embed: np.ndarray                            # uint16 [vocab, hidden]  bf16 bits, N(0, 1)
+    layers: List[Dict[str, np.ndarray]]          # per layer: wq.. wd uint16 [out, in] (N(0, 0.02^2)); g_* uint16 gains
+    chunk_tokens: List[np.ndarray]               # int32 [chunk_len] each
+    query_tokens: np.ndarray                     # int32 [Lq]
+    anchor_idx: np.ndarray                       # int32 CSR values (chunk-local anchor positions, ascending)
+    anchor_ptr: np.ndarray                       # int32 [m+1]
+
+
+def make_stack_workload(name: str, *, ratio: Optional[float] = None, with_weights: bool = True) -> StackWorkload:
+    """Seeded stack + request.  Weights ~ N(0, 0.02^2), embeddings ~ N(0, 1), norm gains 1 + 0.1 N(0, 1) (so that a
+    dropped gain is visible to the parity tests), all rounded to bf16 (both the oracle and the library read these
+    bit patterns); token ids uniform over the synthetic vocabulary; anchors as in make_workload (reading (o))."""
+    sp = STACKS[name]
+    if ratio is not None:
+        sp = StackSpec(**{**sp.__dict__, "ratio": ratio})
+    ss = np.random.SeedSequence(sp.seed)
+    s_emb, s_w, s_tok, s_anchor = ss.spawn(4)
+    rng_e, rng_w = np.random.default_rng(s_emb), np.random.default_rng(s_w)
+    rng_t, rng_a = np.random.default_rng(s_tok), np.random.default_rng(s_anchor)
+    hq, hkv, d, hid, ffn = sp.n_q_heads, sp.n_kv_heads, sp.head_dim, sp.hidden, sp.ffn
+    shapes = {"wq": (hq * d, hid), "wk": (hkv * d, hid), "wv": (hkv * d, hid), "wo": (hid, hq * d),
+              "wg": (ffn, hid), "wu": (ffn, hid), "wd": (hid, ffn)}
+    # with_weights=False: tokens and anchors only (c3's 13.9 GB of weights are drawn on the device by the bench)
+    embed = f32_to_bf16_bits(rng_e.standard_normal((sp.vocab, hid), dtype=np.float32)) if with_weights else None
+    layers = []
+    for _ in range(sp.n_layers if with_weights else 0):
+        lw = {n: f32_to_bf16_bits(rng_w.standard_normal(shapes[n], dtype=np.float32) * np.float32(0.02))
+              for n in _W_NAMES}
+        for n, sz in (("g_attn", hid), ("g_ffn", hid), ("g_q", d), ("g_k", d)):
+            lw[n] = f32_to_bf16_bits(np.float32(1.0) + np.float32(0.1) * rng_w.standard_normal(sz, dtype=np.float32))
+        layers.append(lw)
+    chunk_tokens = [rng_t.integers(0, sp.vocab, size=sp.chunk_len, dtype=np.int32) for _ in range(sp.n_chunks)]
+    query_tokens = rng_t.integers(0, sp.vocab, size=sp.n_query, dtype=np.int32)
+    a_list = [_anchors_for_chunk(rng_a, sp.chunk_len, sp.r_a) for _ in range(sp.n_chunks)]
+    a_ptr = np.zeros(sp.n_chunks + 1, dtype=np.int32)
+    a_ptr[1:] = np.cumsum([len(a) for a in a_list])
+    return StackWorkload(sp, embed, layers, chunk_tokens, query_tokens,
+                         np.concatenate(a_list).astype(np.int32), a_ptr)
