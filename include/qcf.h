@@ -74,6 +74,13 @@ typedef struct {
   int32_t n_query;             /* Lq = |U| >= 0                                                        */
   const int32_t* chunk_len;    /* host [m], each >= 0                                                  */
   const int64_t* chunk_row;    /* host [m], first pool row of chunk i's PIC cache, >= 0                */
+  const int32_t* chunk_pos;    /* host [m] or NULL.  NULL: chunk i is rotated by off_i, the exclusive prefix sum of
+                                  chunk_len (Eq. 4: contiguous stitching).  Non-NULL: chunk i is rotated by
+                                  chunk_pos[i] >= 0 while its rows are still WRITTEN contiguously in chunk order —
+                                  the anchor stitch of Eq. 15-16: "chunk" i = the |A_i| anchor rows
+                                  of c_i kept compactly in an anchor pool, chunk_pos[i] = off_i of c_i in the full
+                                  request, so every anchor keeps its original request position off_i + a
+                                   while the anchor cache stays a compact subsequence.             */
 } qcf_request;
 
 typedef struct {
@@ -179,6 +186,13 @@ QCF_API qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const in
 QCF_API qcf_status qcf_full_prefill_attn(qcf_ctx* ctx, const qcf_batch* b, const void* q, const void* k,
                                          const void* v, void* out, float* lse, void* stream);
 
+/* ------------------------------------------------------------------------------------------------ a1' */
+
+/* Anchor stitch (Eq. 15-16) is qcf_rope_reposition on a batch whose requests were created
+ * with chunk_pos (see qcf_request): k_pool / v_pool are then the layer's compact ANCHOR pool, k_fused / v_fused
+ * the probe cache KV^A(C_A) [B][t_stride][Hkv][d] (t_stride of that batch = max_b (|C_A|_b + Lq_b)).  With
+ * v_pool == NULL and v_fused == NULL only K is re-positioned (scoring prefetch of the critical layers reads no V). */
+
 /* ------------------------------------------------------------------------------------------------ a6 */
 
 /* Everything one layer needs, by name.  Pointers as documented at the stage entry points. */
@@ -221,6 +235,100 @@ QCF_API qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const q
  * over the profiled steps issued since the previous call (or since profiling was enabled), then forgets them. */
 QCF_API qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable);
 QCF_API qcf_status qcf_get_stage_ms(qcf_ctx* ctx, float* ms5);
+
+/* ---------------------------------------------------------------------------------------- a7 / a8 (config 3) */
+
+/* Row-wise dense projection of the recomputed rows (BASELINE config 3):
+ *     c[M][N] = a[M][K] . w[N][K]^T          bf16 operands (nn.Linear layout [out][in]), fp32 accumulation
+ *   epilogue QCF_EPI_STORE        : c = acc                                  (bf16, RNE)
+ *            QCF_EPI_ADD_RESIDUAL : c = residual + acc   (residual [M][N] bf16; residual == c allowed)
+ *            QCF_EPI_SWIGLU       : w holds (gate_j, up_j) rows INTERLEAVED (row 2j = W_g[j], 2j+1 = W_u[j]);
+ *                                   c[M][N/2] = silu(acc[2j]) * acc[2j+1]
+ * All dev pointers 16-byte aligned; K % 8 == 0, N % 8 == 0 (N % 16 == 0 for SWIGLU).  M, N, K tails are handled. */
+typedef enum { QCF_EPI_STORE = 0, QCF_EPI_ADD_RESIDUAL = 1, QCF_EPI_SWIGLU = 2 } qcf_epilogue;
+QCF_API qcf_status qcf_linear(qcf_ctx* ctx, const void* a, const void* w, const void* residual, void* c, int32_t M,
+                              int32_t N, int32_t K, int32_t epilogue, void* stream);
+
+typedef struct qcf_stack qcf_stack;   /* opaque: weights table, activation workspace, loader stream, events */
+
+typedef struct {
+  int32_t n_layers;   /* L                                                   */
+  int32_t hidden;     /* model width, % 8 == 0                               */
+  int32_t ffn;        /* SwiGLU inner width, % 8 == 0                        */
+  int32_t vocab;      /* rows of the embedding table                         */
+  float rms_eps;      /* RMSNorm epsilon (1e-6)                              */
+} qcf_stack_dims;
+
+/* One decoder layer (readings (l), (q)): pre-norm block, QK-norm before RoPE, no biases, SwiGLU.
+ * Device pointers to bf16 tensors owned by the caller; they must outlive the stack. */
+typedef struct {
+  const void* w_qkv;       /* [(Hq + 2 Hkv) d][hidden]: q heads, then k heads, then v heads            */
+  const void* w_o;         /* [hidden][Hq d]                                                           */
+  const void* w_gate_up;   /* [2 ffn][hidden], gate/up rows interleaved (see QCF_EPI_SWIGLU)           */
+  const void* w_down;      /* [hidden][ffn]                                                            */
+  const void* g_attn;      /* [hidden] RMSNorm gain before attention                                   */
+  const void* g_ffn;       /* [hidden] RMSNorm gain before the MLP                                     */
+  const void* g_q;         /* [d] per-head RMSNorm gain of q                                           */
+  const void* g_k;         /* [d] per-head RMSNorm gain of k                                           */
+} qcf_layer_weights;
+
+/* layers: host array [n_layers]; embed: dev [vocab][hidden] bf16.  max_rows bounds the rows any call pushes through
+ * the block (N + Lq for full prefill), max_pos the largest request position + 1 (RoPE table, evaluated in double),
+ * max_pool_rows the PIC / anchor pool rows staged per layer by qcf_stack_fuse (0: fuse not used).  The head layout
+ * is the ctx's.  Only single-request batches (B = 1) are supported by the stack calls. */
+QCF_API qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_layer_weights* layers,
+                                    const void* embed, int32_t max_rows, int32_t max_pos, int64_t max_pool_rows,
+                                    qcf_stack** out);
+QCF_API void qcf_stack_destroy(qcf_stack* s);
+
+/* Eq. 2 / Eq. 3: all T = N + Lq rows of the batch's request, token ids tokens[T] (dev int32) at
+ * positions 0..T-1, through every layer with dense causal attention.  k_cache / v_cache: host arrays [n_layers] of
+ * dev pointers [T][Hkv][d] that receive each layer's K (post QK-norm, post RoPE) and V.  hidden_out: dev
+ * [T][hidden] final hidden states, or NULL.  Used for the full-prefill comparator (Eq. 2) and, on a one-chunk batch
+ * with Lq = 0, for building that chunk's PIC cache at chunk-local positions (Eq. 3). */
+QCF_API qcf_status qcf_stack_prefill(qcf_stack* s, const qcf_batch* b, const int32_t* tokens, void* const* k_cache,
+                                     void* const* v_cache, void* hidden_out, void* stream);
+
+/* One layer of Fig. 9 stage 2 for the rows R = sel[0..n_sel) u U of the batch's request:
+ *   RMSNorm -> QKV projection -> QK-norm + RoPE at the rows' request positions -> a4 scatter + a5 attention over
+ *   k_fused / v_fused (which must already hold this layer's stitched PIC entries) -> O projection + residual ->
+ *   RMSNorm -> SwiGLU MLP + residual.
+ *   x: dev [n_rows][hidden] bf16, in/out (compact, P ascending then U); n_rows = n_sel + Lq must be given by the
+ *   caller (host; qcf_n_select).  sel == NULL: dense mode — rows are positions 0..n_rows-1 and k_fused / v_fused
+ *   receive their K/V (one layer of qcf_stack_prefill).  query_pos0 >= 0 overrides the request position of the
+ *   first query row (default N_b): the probe stage runs U over the compact anchor cache at positions N..N+Lq-1
+ *   (PAPER.md:293).  q_tap: dev [n_rows][Hq][d] or NULL, receives the post-RoPE query states (Eq. 17). */
+QCF_API qcf_status qcf_stack_layer(qcf_stack* s, int32_t layer, const qcf_batch* b, const int32_t* sel,
+                                   const int32_t* n_sel, int32_t n_rows, int32_t query_pos0, void* x, void* k_fused,
+                                   void* v_fused, void* q_tap, void* stream);
+
+/* The whole online pipeline of Fig. 9 for one request.
+ *   stage 1  for l = 0..max(L*): load anchor pool l, stitch (a1'), run U through layer l over the anchor cache
+ *            (Eq. 17); for l in L*: load PIC pool l, stitch (a1), score (a2, Eq. 18/20); then top-k (a3, Eq. 11)
+ *   stage 2  for every layer: load PIC pool l+1.. and stitch them on a second stream WHILE layer l recomputes the
+ *            rows R on `stream` (a8: PAPER.md:23, 341-342), a4 + a5 + a7 per layer
+ * Pools may live in pinned host memory (the paper's setting) or on the device (cudaMemcpyDefault). */
+typedef struct {
+  const void* const* k_pic;      /* host array [L] of pointers to [pool_rows][Hkv][d] bf16 PIC pools              */
+  const void* const* v_pic;
+  int64_t pool_rows;
+  const void* const* k_anchor;   /* host array [L] (entries l <= max(L*) are read) of compact anchor pools         */
+  const void* const* v_anchor;
+  int64_t anchor_rows;
+  const int32_t* crit_layers;    /* host [n_crit], ascending 0-based layer indices of L*                           */
+  int32_t n_crit;
+  double ratio;                  /* rho                                                                             */
+  const int32_t* tokens;         /* dev int32 [N + Lq] token ids by request position                                */
+  void* const* k_fused;          /* host array [L] of dev [t_stride][Hkv][d]: receives KV^Fuse of every layer       */
+  void* const* v_fused;
+  float* scores;                 /* dev [n_stride]   out: Eq. 20 scores                                             */
+  int32_t* sel;                  /* dev [n_stride]   out: P ascending                                               */
+  int32_t* n_sel;                /* dev [1]                                                                         */
+  void* hidden_out;              /* dev [n_R][hidden] out: final hidden states of the rows R (P ascending, then U)  */
+  int32_t overlap;               /* != 0: layer-ahead loading on a second stream (a8); 0: serial, for the ablation  */
+} qcf_fuse_args;
+QCF_API qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* main_batch, const qcf_batch* probe_batch,
+                                  const qcf_fuse_args* args, void* stream);
 
 #ifdef __cplusplus
 }

@@ -22,7 +22,10 @@ EXPORTS = (
     "qcf_create", "qcf_destroy", "qcf_last_error", "qcf_version", "qcf_batch_create", "qcf_batch_destroy",
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms",
+    "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse",
 )
+
+QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
 
 
 class QcfError(RuntimeError):
@@ -38,7 +41,8 @@ class qcf_layout(C.Structure):
 
 class qcf_request(C.Structure):
     _fields_ = [("n_chunks", C.c_int32), ("n_query", C.c_int32),
-                ("chunk_len", C.POINTER(C.c_int32)), ("chunk_row", C.POINTER(C.c_int64))]
+                ("chunk_len", C.POINTER(C.c_int32)), ("chunk_row", C.POINTER(C.c_int64)),
+                ("chunk_pos", C.POINTER(C.c_int32))]
 
 
 class qcf_batch_info(C.Structure):
@@ -52,6 +56,25 @@ class qcf_layer_args(C.Structure):
                 ("q_new", C.c_void_p), ("k_new", C.c_void_p), ("v_new", C.c_void_p), ("out", C.c_void_p),
                 ("lse", C.c_void_p), ("ratio", C.c_double), ("rows_by_position", C.c_int32),
                 ("is_critical_layer", C.c_int32), ("accumulate", C.c_int32), ("select_now", C.c_int32)]
+
+
+class qcf_stack_dims(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("hidden", C.c_int32), ("ffn", C.c_int32), ("vocab", C.c_int32),
+                ("rms_eps", C.c_float)]
+
+
+class qcf_layer_weights(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("w_qkv", "w_o", "w_gate_up", "w_down", "g_attn", "g_ffn", "g_q", "g_k")]
+
+
+class qcf_fuse_args(C.Structure):
+    _fields_ = [
+        ("k_pic", C.POINTER(C.c_void_p)), ("v_pic", C.POINTER(C.c_void_p)), ("pool_rows", C.c_int64),
+        ("k_anchor", C.POINTER(C.c_void_p)), ("v_anchor", C.POINTER(C.c_void_p)), ("anchor_rows", C.c_int64),
+        ("crit_layers", C.POINTER(C.c_int32)), ("n_crit", C.c_int32), ("ratio", C.c_double), ("tokens", C.c_void_p),
+        ("k_fused", C.POINTER(C.c_void_p)), ("v_fused", C.POINTER(C.c_void_p)), ("scores", C.c_void_p),
+        ("sel", C.c_void_p), ("n_sel", C.c_void_p), ("hidden_out", C.c_void_p), ("overlap", C.c_int32),
+    ]
 
 
 _lib = None
@@ -87,6 +110,13 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_layer_step_host": (i32, [vp, vp, C.POINTER(qcf_layer_args), i64, vp]),
         "qcf_set_profiling": (i32, [vp, i32]),
         "qcf_get_stage_ms": (i32, [vp, C.POINTER(C.c_float)]),
+        "qcf_linear": (i32, [vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]),
+        "qcf_stack_create": (i32, [vp, C.POINTER(qcf_stack_dims), C.POINTER(qcf_layer_weights), vp, i32, i32, i64,
+                                   C.POINTER(vp)]),
+        "qcf_stack_destroy": (None, [vp]),
+        "qcf_stack_prefill": (i32, [vp, vp, vp, C.POINTER(vp), C.POINTER(vp), vp, vp]),
+        "qcf_stack_layer": (i32, [vp, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp]),
+        "qcf_stack_fuse": (i32, [vp, vp, vp, C.POINTER(qcf_fuse_args), vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(lib, name)
@@ -123,7 +153,7 @@ class Batch:
     """qcf_batch: device-resident description of a batch of requests (chunk lengths + PIC pool rows)."""
 
     def __init__(self, ctx: "Context", chunk_lens: Sequence[Sequence[int]], chunk_rows: Sequence[Sequence[int]],
-                 n_query: Sequence[int]):
+                 n_query: Sequence[int], chunk_pos: Optional[Sequence[Sequence[int]]] = None):
         self.ctx = ctx
         n = len(chunk_lens)
         reqs = (qcf_request * max(n, 1))()
@@ -137,6 +167,11 @@ class Batch:
             reqs[b].n_query = int(n_query[b])
             reqs[b].chunk_len = cl.ctypes.data_as(C.POINTER(C.c_int32))
             reqs[b].chunk_row = cr.ctypes.data_as(C.POINTER(C.c_int64))
+            if chunk_pos is not None:              # anchor stitch (Eq. 15-16): rotate by the chunk's ORIGINAL offset
+                cp = np.ascontiguousarray(chunk_pos[b], dtype=np.int32)
+                assert cp.shape == cl.shape
+                self._keep.append(cp)
+                reqs[b].chunk_pos = cp.ctypes.data_as(C.POINTER(C.c_int32))
         h = C.c_void_p()
         ctx._check(ctx.lib.qcf_batch_create(ctx.handle, reqs, n, C.byref(h)))
         self.handle = h
@@ -187,8 +222,12 @@ class Context:
         except Exception:
             pass
 
-    def batch(self, chunk_lens, chunk_rows, n_query) -> Batch:
-        return Batch(self, chunk_lens, chunk_rows, n_query)
+    def batch(self, chunk_lens, chunk_rows, n_query, chunk_pos=None) -> Batch:
+        return Batch(self, chunk_lens, chunk_rows, n_query, chunk_pos)
+
+    def qcf_linear(self, a, w, residual, c, M: int, N: int, K: int, epilogue: int = QCF_EPI_STORE, stream=None):
+        self._check(self.lib.qcf_linear(self.handle, _ptr(a), _ptr(w), _ptr(residual), _ptr(c), M, N, K, epilogue,
+                                        _stream(stream)))
 
     # ---- stage entry points (names and argument order of include/qcf.h)
     def qcf_rope_reposition(self, b: Batch, k_pool, v_pool, k_fused, v_fused, stream=None):
@@ -235,3 +274,61 @@ class Context:
         ms = (C.c_float * 5)()
         self._check(self.lib.qcf_get_stage_ms(self.handle, ms))
         return [float(x) for x in ms]
+
+
+def _ptr_array(ptrs):
+    arr = (C.c_void_p * len(ptrs))()
+    for i, p in enumerate(ptrs):
+        arr[i] = _ptr(p)
+    return arr
+
+
+class Stack:
+    """qcf_stack (config 3).  `layers`: list of dicts of device tensors keyed by the field names of qcf_layer_weights;
+    the tensors are kept alive by this object."""
+
+    def __init__(self, ctx: Context, n_layers: int, hidden: int, ffn: int, vocab: int, rms_eps: float, layers, embed,
+                 max_rows: int, max_pos: int, max_pool_rows: int = 0):
+        self.ctx, self.lib, self.handle = ctx, ctx.lib, None
+        self._keep = (layers, embed)
+        self.n_layers, self.hidden, self.ffn = n_layers, hidden, ffn
+        dims = qcf_stack_dims(n_layers, hidden, ffn, vocab, rms_eps)
+        lw = (qcf_layer_weights * n_layers)()
+        for i, d in enumerate(layers):
+            for name, _ in qcf_layer_weights._fields_:
+                setattr(lw[i], name, _ptr(d[name]))
+        h = C.c_void_p()
+        ctx._check(self.lib.qcf_stack_create(ctx.handle, C.byref(dims), lw, _ptr(embed), max_rows, max_pos,
+                                             max_pool_rows, C.byref(h)))
+        self.handle = h
+
+    def close(self):
+        if self.handle:
+            self.lib.qcf_stack_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def qcf_stack_prefill(self, b: Batch, tokens, k_cache, v_cache, hidden_out=None, stream=None):
+        self.ctx._check(self.lib.qcf_stack_prefill(self.handle, b.handle, _ptr(tokens), _ptr_array(k_cache),
+                                                   _ptr_array(v_cache), _ptr(hidden_out), _stream(stream)))
+
+    def qcf_stack_layer(self, layer: int, b: Batch, sel, n_sel, n_rows: int, x, k_fused, v_fused, query_pos0: int = -1,
+                        q_tap=None, stream=None):
+        self.ctx._check(self.lib.qcf_stack_layer(self.handle, layer, b.handle, _ptr(sel), _ptr(n_sel), n_rows,
+                                                 query_pos0, _ptr(x), _ptr(k_fused), _ptr(v_fused), _ptr(q_tap),
+                                                 _stream(stream)))
+
+    def qcf_stack_fuse(self, main: Batch, probe: Batch, *, k_pic, v_pic, pool_rows: int, k_anchor, v_anchor,
+                       anchor_rows: int, crit_layers, ratio: float, tokens, k_fused, v_fused, scores, sel, n_sel,
+                       hidden_out=None, overlap: bool = True, stream=None):
+        crit = (C.c_int32 * len(crit_layers))(*[int(c) for c in crit_layers])
+        keep = [_ptr_array(x) for x in (k_pic, v_pic, k_anchor, v_anchor, k_fused, v_fused)]
+        a = qcf_fuse_args(keep[0], keep[1], pool_rows, keep[2], keep[3], anchor_rows, crit, len(crit_layers), ratio,
+                          _ptr(tokens), keep[4], keep[5], _ptr(scores), _ptr(sel), _ptr(n_sel), _ptr(hidden_out),
+                          1 if overlap else 0)
+        self.ctx._check(self.lib.qcf_stack_fuse(self.handle, main.handle, probe.handle, C.byref(a), _stream(stream)))

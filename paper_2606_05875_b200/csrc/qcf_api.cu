@@ -32,6 +32,13 @@ struct DevBuf {
 
 }  // namespace
 
+namespace qcf {
+qcf_status set_error(const qcf_ctx* ctx, qcf_status st, const std::string& msg) {
+  if (ctx) ctx->err = msg; else g_create_err = msg;
+  return st;
+}
+}  // namespace qcf
+
 // Device staging buffers of qcf_layer_step_host (allocated on first use, kept by the ctx).
 struct HostStage {
   DevBuf k_pool, v_pool, k_f, v_f, q_probe, scores, sel, n_sel, q_new, k_new, v_new, out, lse;
@@ -43,10 +50,7 @@ struct HostStage {
 
 namespace {
 
-qcf_status fail(const qcf_ctx* ctx, qcf_status st, const std::string& msg) {
-  if (ctx) ctx->err = msg; else g_create_err = msg;
-  return st;
-}
+qcf_status fail(const qcf_ctx* ctx, qcf_status st, const std::string& msg) { return qcf::set_error(ctx, st, msg); }
 qcf_status cuda_fail(const qcf_ctx* ctx, cudaError_t e, const char* what) {
   return fail(ctx, QCF_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
@@ -129,6 +133,9 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
     const char* e2 = std::getenv("QCF_SCORE_IMPL");
     c->score_impl = (e2 && std::strcmp(e2, "mma") == 0) ? 0 : 1;
     const char* e3 = std::getenv("QCF_ATTN_CLUSTER");
+    const char* e4 = std::getenv("QCF_GEMM_MT");
+    const int mt = e4 ? std::atoi(e4) : 0;
+    c->gemm_mt = (mt == 1 || mt == 2) ? mt : 0;
     const int cl = e3 ? std::atoi(e3) : 0;
     c->attn_cluster = (cl == 1 || cl == 2 || cl == 4) ? cl : 0;
     c->ratio_hint = 0.3;
@@ -179,7 +186,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
   if (batch > ctx->max_batch) return fail(ctx, QCF_ERR_WORKSPACE, "batch exceeds max_batch of qcf_create");
 
   const int half = ctx->lay.d / 2;
-  std::vector<int32_t> n_ctx(batch), n_query(batch), c_req, c_off, c_len, c_blk;
+  std::vector<int32_t> n_ctx(batch), n_query(batch), c_req, c_off, c_rot, c_len, c_blk;
   std::vector<int64_t> c_row;
   std::vector<float> rot;      // (cos, sin) interleaved
   int64_t total_ctx = 0;
@@ -197,15 +204,18 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
     for (int i = 0; i < r.n_chunks; ++i) {
       QCF_REQUIRE(ctx, r.chunk_len[i] >= 0, "chunk_len must be >= 0");
       QCF_REQUIRE(ctx, r.chunk_row[i] >= 0, "chunk_row must be >= 0");
+      QCF_REQUIRE(ctx, !r.chunk_pos || r.chunk_pos[i] >= 0, "chunk_pos must be >= 0");
       if (off + r.chunk_len[i] > ctx->max_ctx) return fail(ctx, QCF_ERR_WORKSPACE, "context length exceeds max_ctx of qcf_create");
       if (r.chunk_len[i] == 0) continue;
       c_req.push_back(b);
       c_off.push_back(static_cast<int32_t>(off));
+      const int64_t rot_pos = r.chunk_pos ? r.chunk_pos[i] : off;     // Eq. 4 (off_i) or Eq. 15-16 (anchors keep off_i of c_i)
+      c_rot.push_back(static_cast<int32_t>(rot_pos));
       c_len.push_back(r.chunk_len[i]);
       c_row.push_back(r.chunk_row[i]);
       c_blk.push_back(c_blk.back() + (r.chunk_len[i] + kRepoRows - 1) / kRepoRows);
       for (int j = 0; j < half; ++j) {
-        const double phi = static_cast<double>(off) * inv_freq[j];
+        const double phi = static_cast<double>(rot_pos) * inv_freq[j];
         rot.push_back(static_cast<float>(std::cos(phi)));
         rot.push_back(static_cast<float>(std::sin(phi)));
       }
@@ -235,13 +245,14 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
     std::memcpy(qb->h_n_query, n_query.data(), sizeof(int32_t) * batch);
   }
 
-  // one device blob: [n_ctx | n_query | chunk_req | chunk_off | chunk_len | chunk_blk | pad | chunk_row | rot]
+  // one device blob: [n_ctx | n_query | chunk_req | chunk_off | chunk_len | chunk_blk | pad | chunk_row | rot | chunk_rot]
   auto up = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
   size_t o_nctx = 0, o_nq = up(o_nctx + sizeof(int32_t) * batch, 16);
   size_t o_req = up(o_nq + sizeof(int32_t) * batch, 16), o_off = up(o_req + sizeof(int32_t) * n_chunks, 16);
   size_t o_len = up(o_off + sizeof(int32_t) * n_chunks, 16), o_blk = up(o_len + sizeof(int32_t) * n_chunks, 16);
   size_t o_row = up(o_blk + sizeof(int32_t) * (n_chunks + 1), 16), o_rot = up(o_row + sizeof(int64_t) * n_chunks, 16);
-  size_t total = up(o_rot + sizeof(float) * rot.size(), 16) + 16;
+  size_t o_crot = up(o_rot + sizeof(float) * rot.size(), 16);
+  size_t total = up(o_crot + sizeof(int32_t) * n_chunks, 16) + 16;
   std::vector<unsigned char> host(total, 0);
   if (batch > 0) {
     std::memcpy(host.data() + o_nctx, n_ctx.data(), sizeof(int32_t) * batch);
@@ -253,6 +264,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
     std::memcpy(host.data() + o_len, c_len.data(), sizeof(int32_t) * n_chunks);
     std::memcpy(host.data() + o_row, c_row.data(), sizeof(int64_t) * n_chunks);
     std::memcpy(host.data() + o_rot, rot.data(), sizeof(float) * rot.size());
+    std::memcpy(host.data() + o_crot, c_rot.data(), sizeof(int32_t) * n_chunks);
   }
   std::memcpy(host.data() + o_blk, c_blk.data(), sizeof(int32_t) * (n_chunks + 1));
   cudaError_t e = cudaMalloc(&qb->blob, total);
@@ -273,6 +285,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
   bd.chunk_blk = reinterpret_cast<const int32_t*>(d + o_blk);
   bd.chunk_row = reinterpret_cast<const int64_t*>(d + o_row);
   bd.rot = reinterpret_cast<const float2*>(d + o_rot);
+  bd.chunk_rot = reinterpret_cast<const int32_t*>(d + o_crot);
   *out = qb;
   return QCF_OK;
 }
@@ -298,7 +311,8 @@ qcf_status qcf_rope_reposition(qcf_ctx* ctx, const qcf_batch* b, const void* k_p
                                void* v_fused, void* stream) {
   if (qcf_status st = check_ctx_batch(ctx, b)) return st;
   if (b->total_ctx == 0) return QCF_OK;
-  QCF_REQUIRE(ctx, k_pool && v_pool && k_fused && v_fused, "qcf_rope_reposition: NULL tensor pointer");
+  QCF_REQUIRE(ctx, k_pool && k_fused, "qcf_rope_reposition: NULL tensor pointer");
+  QCF_REQUIRE(ctx, (v_pool == nullptr) == (v_fused == nullptr), "qcf_rope_reposition: v_pool and v_fused must both be given or both be NULL");
   QCF_REQUIRE(ctx, aligned16(k_pool) && aligned16(v_pool) && aligned16(k_fused) && aligned16(v_fused),
               "qcf_rope_reposition: pointers must be 16-byte aligned");
   QCF_CUDA(ctx, launch_reposition(ctx, b, static_cast<const __nv_bfloat16*>(k_pool),

@@ -23,7 +23,8 @@ struct BatchDev {
   const int32_t* n_query;  // Lq_b
   // per chunk [n_chunks]
   const int32_t* chunk_req;    // owning request
-  const int32_t* chunk_off;    // off_i: first request position
+  const int32_t* chunk_off;    // off_i: first row of the chunk in the request's fused cache
+  const int32_t* chunk_rot;    // position the chunk is rotated by (= chunk_off unless qcf_request.chunk_pos is given)
   const int32_t* chunk_len;
   const int64_t* chunk_row;    // first row in the PIC pool
   const int32_t* chunk_blk;    // [n_chunks+1] exclusive prefix of ceil(len / kRepoRows): reposition work list
@@ -47,6 +48,7 @@ struct qcf_ctx {
   int max_batch, max_ctx, max_query;
   int score_impl;        // 1: tcgen05 kernels (default); 0: legacy mma.sync kernels (QCF_SCORE_IMPL=mma)
   int attn_impl;         // 1: tcgen05/TMEM/TMA kernel (default); 0: legacy mma.sync kernel (QCF_ATTN_IMPL=mma, for A/B timing)
+  int gemm_mt;           // GEMM tile height in units of 128 rows: 0 = heuristic, else 1 / 2 (QCF_GEMM_MT)
   int attn_cluster;      // split-KV cluster size of the tcgen05 attention kernel: 0 = heuristic, else 1/2/4 (QCF_ATTN_CLUSTER)
   double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
   // workspace (device)
@@ -89,6 +91,9 @@ namespace qcf {
 constexpr int kScoreSplits = 8;     // key-range splits of the legacy (mma.sync) score statistics pass
 constexpr int kScoreSplitsMax = 32; // upper bound of the tcgen05 pass-1 key splits (sizes the statistics workspace)
 
+// Records `msg` as the last error of ctx (or of this thread's failed qcf_create when ctx == nullptr); returns st.
+qcf_status set_error(const qcf_ctx* ctx, qcf_status st, const std::string& msg);
+
 // Stage launchers (each validates nothing: arguments were checked by the API layer). Return cudaGetLastError().
 cudaError_t launch_reposition(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool,
                               const __nv_bfloat16* v_pool, __nv_bfloat16* k_f, __nv_bfloat16* v_f, cudaStream_t);
@@ -103,6 +108,19 @@ cudaError_t launch_scatter(const qcf_ctx*, const qcf_batch*, const int32_t* sel,
 cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
+
+cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
+                        __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
+cudaError_t launch_rope_table(float2* table, int n_pos, int d, double theta, cudaStream_t);
+cudaError_t launch_embed_gather(const __nv_bfloat16* embed, const int32_t* tokens, const int32_t* sel, const int32_t* n_sel,
+                                int n_ctx, int pos_off, int n_rows, int hidden, __nv_bfloat16* x, cudaStream_t);
+cudaError_t launch_rmsnorm(const __nv_bfloat16* x, const __nv_bfloat16* gain, float eps, int n_rows, int hidden,
+                           __nv_bfloat16* y, cudaStream_t);
+// rows r < n_rows of one request; sel == nullptr: position pos_off + r; else sel[r] / query rows at n_ctx + (r - n_sel)
+cudaError_t launch_qknorm_rope(const qcf_ctx*, const __nv_bfloat16* qkv, const __nv_bfloat16* g_q, const __nv_bfloat16* g_k,
+                               const float2* table, const int32_t* sel, const int32_t* n_sel, int n_ctx, int pos_off,
+                               float eps, int n_rows, __nv_bfloat16* q_out, __nv_bfloat16* k_out, __nv_bfloat16* v_out,
+                               cudaStream_t);
 
 cudaError_t launch_score_tc(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* q_probe, const __nv_bfloat16* k_f,
                             float* scores, int accumulate, cudaStream_t);

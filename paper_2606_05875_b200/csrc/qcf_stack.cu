@@ -1,0 +1,331 @@
+// Config 3 (BASELINE.json configs[2]): the decoder stack around the layer step — a7 (row-wise dense ops of the rows
+// R = P u U), a8 (layer-ahead KV loading on a second stream) and the two-stage online pipeline of Fig. 9
+// (PAPER.md:329-344).  Host-side orchestration only: every tensor operation is a kernel of the sibling files.
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "qcf_internal.cuh"
+
+using namespace qcf;
+
+struct qcf_stack {
+  qcf_ctx* ctx;
+  qcf_stack_dims dims;
+  std::vector<qcf_layer_weights> layers;
+  const __nv_bfloat16* embed;
+  int max_rows, max_pos;
+  int64_t max_pool_rows;
+  // activation workspace (device, bf16)
+  __nv_bfloat16 *x, *h, *qkv, *q_new, *k_new, *v_new, *attn, *act;
+  float2* rope_table;
+  // qcf_stack_fuse: staging ring for the loaded pools, probe caches, loader stream, events
+  static constexpr int kRing = 2;
+  __nv_bfloat16* stage_k[kRing];
+  __nv_bfloat16* stage_v[kRing];
+  __nv_bfloat16* probe_k[2];
+  __nv_bfloat16* probe_v[2];
+  size_t probe_rows;
+  cudaStream_t loader;
+  std::vector<cudaEvent_t> ev_ready, ev_done;      // per pipeline slot
+  cudaEvent_t ev_fork, ev_join;
+  int32_t* zero_i32;                               // device zeros: the probe stage's empty selection
+};
+
+namespace {
+
+#define STK_CUDA(ctx, call)                                                                             \
+  do {                                                                                                  \
+    cudaError_t e__ = (call);                                                                           \
+    if (e__ != cudaSuccess) return set_error(ctx, QCF_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e__)); \
+  } while (0)
+#define STK_REQUIRE(ctx, cond, msg)                                          \
+  do {                                                                       \
+    if (!(cond)) return set_error(ctx, QCF_ERR_INVALID_ARG, std::string(msg)); \
+  } while (0)
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <class T>
+cudaError_t dalloc(T** p, size_t n) { return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T) + 16); }
+
+// The block of DESIGN.md §7 for rows 0..n_rows-1 of `x` (in place).  sel == nullptr: dense (K/V go straight into
+// k_fused / v_fused, rows are positions pos0..); else a4 + a5 through qcf_recompute_attn on compact fresh rows.
+qcf_status run_layer(qcf_stack* s, int l, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel, int n_rows,
+                     int query_pos0, __nv_bfloat16* x, void* k_fused, void* v_fused, void* q_tap, cudaStream_t st) {
+  qcf_ctx* ctx = s->ctx;
+  const Layout& L = ctx->lay;
+  const qcf_layer_weights& w = s->layers[l];
+  const int hid = s->dims.hidden, ffn = s->dims.ffn;
+  const int qkv_n = (L.hq + 2 * L.hkv) * L.d;
+  const bool dense = sel == nullptr;
+  auto bf = [](const void* p) { return static_cast<const __nv_bfloat16*>(p); };
+  STK_CUDA(ctx, launch_rmsnorm(x, bf(w.g_attn), s->dims.rms_eps, n_rows, hid, s->h, st));
+  STK_CUDA(ctx, launch_gemm(ctx, s->h, bf(w.w_qkv), nullptr, s->qkv, n_rows, qkv_n, hid, QCF_EPI_STORE, st));
+  __nv_bfloat16* q_dst = q_tap ? static_cast<__nv_bfloat16*>(q_tap) : s->q_new;
+  const int n_ctx = b->h_n_ctx[0];
+  if (dense) {
+    STK_CUDA(ctx, launch_qknorm_rope(ctx, s->qkv, bf(w.g_q), bf(w.g_k), s->rope_table, nullptr, nullptr, n_ctx, 0,
+                                     s->dims.rms_eps, n_rows, q_dst, static_cast<__nv_bfloat16*>(k_fused),
+                                     static_cast<__nv_bfloat16*>(v_fused), st));
+    if (qcf_status e = qcf_full_prefill_attn(ctx, b, q_dst, k_fused, v_fused, s->attn, nullptr, st)) return e;
+  } else {
+    const int qp0 = query_pos0 >= 0 ? query_pos0 : n_ctx;
+    STK_CUDA(ctx, launch_qknorm_rope(ctx, s->qkv, bf(w.g_q), bf(w.g_k), s->rope_table, sel, n_sel, qp0, 0,
+                                     s->dims.rms_eps, n_rows, q_dst, s->k_new, s->v_new, st));
+    if (qcf_status e = qcf_recompute_attn(ctx, b, sel, n_sel, q_dst, s->k_new, s->v_new, 0, k_fused, v_fused, s->attn,
+                                          nullptr, st))
+      return e;
+  }
+  STK_CUDA(ctx, launch_gemm(ctx, s->attn, bf(w.w_o), x, x, n_rows, hid, L.hq * L.d, QCF_EPI_ADD_RESIDUAL, st));
+  STK_CUDA(ctx, launch_rmsnorm(x, bf(w.g_ffn), s->dims.rms_eps, n_rows, hid, s->h, st));
+  STK_CUDA(ctx, launch_gemm(ctx, s->h, bf(w.w_gate_up), nullptr, s->act, n_rows, 2 * ffn, hid, QCF_EPI_SWIGLU, st));
+  STK_CUDA(ctx, launch_gemm(ctx, s->act, bf(w.w_down), x, x, n_rows, hid, ffn, QCF_EPI_ADD_RESIDUAL, st));
+  return QCF_OK;
+}
+
+qcf_status check_stack_batch(qcf_stack* s, const qcf_batch* b, const char* who) {
+  if (!s) return set_error(nullptr, QCF_ERR_INVALID_ARG, std::string(who) + ": stack is NULL");
+  qcf_ctx* ctx = s->ctx;
+  STK_REQUIRE(ctx, b != nullptr && b->ctx == ctx, std::string(who) + ": batch is NULL or from another ctx");
+  STK_REQUIRE(ctx, b->batch == 1, std::string(who) + ": the stack calls take single-request batches (B = 1)");
+  return QCF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+qcf_status qcf_linear(qcf_ctx* ctx, const void* a, const void* w, const void* residual, void* c, int32_t M, int32_t N,
+                      int32_t K, int32_t epilogue, void* stream) {
+  if (!ctx) return set_error(nullptr, QCF_ERR_INVALID_ARG, "ctx is NULL");
+  STK_REQUIRE(ctx, M >= 0 && N >= 0 && K > 0, "qcf_linear: M, N must be >= 0 and K > 0");
+  if (M == 0 || N == 0) return QCF_OK;
+  STK_REQUIRE(ctx, epilogue >= 0 && epilogue <= 2, "qcf_linear: unknown epilogue");
+  STK_REQUIRE(ctx, a && w && c, "qcf_linear: NULL tensor pointer");
+  STK_REQUIRE(ctx, epilogue != QCF_EPI_ADD_RESIDUAL || residual, "qcf_linear: residual is NULL");
+  STK_REQUIRE(ctx, aligned16(a) && aligned16(w) && aligned16(c) && aligned16(residual), "qcf_linear: pointers must be 16-byte aligned");
+  STK_REQUIRE(ctx, K % 8 == 0 && N % 8 == 0 && (epilogue != QCF_EPI_SWIGLU || N % 16 == 0),
+              "qcf_linear: K and N must be multiples of 8 (N of 16 for SWIGLU)");
+  STK_CUDA(ctx, launch_gemm(ctx, static_cast<const __nv_bfloat16*>(a), static_cast<const __nv_bfloat16*>(w),
+                            static_cast<const __nv_bfloat16*>(residual), static_cast<__nv_bfloat16*>(c), M, N, K, epilogue,
+                            static_cast<cudaStream_t>(stream)));
+  return QCF_OK;
+}
+
+qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_layer_weights* layers, const void* embed,
+                            int32_t max_rows, int32_t max_pos, int64_t max_pool_rows, qcf_stack** out) {
+  if (!ctx) return set_error(nullptr, QCF_ERR_INVALID_ARG, "ctx is NULL");
+  STK_REQUIRE(ctx, out != nullptr, "qcf_stack_create: out is NULL");
+  *out = nullptr;
+  STK_REQUIRE(ctx, dims && layers && embed, "qcf_stack_create: NULL argument");
+  STK_REQUIRE(ctx, dims->n_layers >= 1 && dims->hidden >= 8 && dims->ffn >= 8 && dims->vocab >= 1,
+              "qcf_stack_create: n_layers, hidden, ffn, vocab must be positive");
+  STK_REQUIRE(ctx, dims->hidden % 8 == 0 && dims->ffn % 8 == 0, "qcf_stack_create: hidden and ffn must be multiples of 8");
+  STK_REQUIRE(ctx, max_rows >= 1 && max_pos >= 1 && max_pool_rows >= 0, "qcf_stack_create: bad limits");
+  for (int l = 0; l < dims->n_layers; ++l) {
+    const qcf_layer_weights& w = layers[l];
+    STK_REQUIRE(ctx, w.w_qkv && w.w_o && w.w_gate_up && w.w_down && w.g_attn && w.g_ffn && w.g_q && w.g_k,
+                "qcf_stack_create: NULL weight pointer");
+    STK_REQUIRE(ctx, aligned16(w.w_qkv) && aligned16(w.w_o) && aligned16(w.w_gate_up) && aligned16(w.w_down) &&
+                         aligned16(w.g_attn) && aligned16(w.g_ffn),
+                "qcf_stack_create: weight pointers must be 16-byte aligned");
+  }
+  qcf_stack* s = new (std::nothrow) qcf_stack();
+  if (!s) return set_error(ctx, QCF_ERR_WORKSPACE, "out of host memory");
+  s->ctx = ctx; s->dims = *dims;
+  s->layers.assign(layers, layers + dims->n_layers);
+  s->embed = static_cast<const __nv_bfloat16*>(embed);
+  s->max_rows = max_rows; s->max_pos = max_pos; s->max_pool_rows = max_pool_rows;
+  const Layout& L = ctx->lay;
+  const size_t R = max_rows, kv = static_cast<size_t>(L.hkv) * L.d, qd = static_cast<size_t>(L.hq) * L.d;
+  s->x = s->h = s->qkv = s->q_new = s->k_new = s->v_new = s->attn = s->act = nullptr;
+  s->rope_table = nullptr;
+  for (int i = 0; i < qcf_stack::kRing; ++i) s->stage_k[i] = s->stage_v[i] = nullptr;
+  s->probe_k[0] = s->probe_k[1] = s->probe_v[0] = s->probe_v[1] = nullptr;
+  s->loader = nullptr; s->ev_fork = s->ev_join = nullptr; s->zero_i32 = nullptr;
+  s->probe_rows = static_cast<size_t>(max_pool_rows) + ctx->max_query;
+  bool ok = dalloc(&s->x, R * dims->hidden) == cudaSuccess && dalloc(&s->h, R * dims->hidden) == cudaSuccess &&
+            dalloc(&s->qkv, R * (qd + 2 * kv)) == cudaSuccess && dalloc(&s->q_new, R * qd) == cudaSuccess &&
+            dalloc(&s->k_new, R * kv) == cudaSuccess && dalloc(&s->v_new, R * kv) == cudaSuccess &&
+            dalloc(&s->attn, R * qd) == cudaSuccess && dalloc(&s->act, R * dims->ffn) == cudaSuccess &&
+            dalloc(&s->rope_table, static_cast<size_t>(max_pos) * (L.d / 2)) == cudaSuccess;
+  if (ok && max_pool_rows > 0) {
+    for (int i = 0; i < qcf_stack::kRing && ok; ++i)
+      ok = dalloc(&s->stage_k[i], static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess &&
+           dalloc(&s->stage_v[i], static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i)
+      ok = dalloc(&s->probe_k[i], s->probe_rows * kv) == cudaSuccess && dalloc(&s->probe_v[i], s->probe_rows * kv) == cudaSuccess;
+  }
+  ok = ok && dalloc(&s->zero_i32, 4) == cudaSuccess && cudaMemset(s->zero_i32, 0, 16) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&s->loader, cudaStreamNonBlocking) == cudaSuccess &&
+       cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+       cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming) == cudaSuccess;
+  const int n_slots = 2 * dims->n_layers + 4;
+  s->ev_ready.assign(n_slots, nullptr);
+  s->ev_done.assign(n_slots, nullptr);
+  for (int i = 0; i < n_slots && ok; ++i)
+    ok = cudaEventCreateWithFlags(&s->ev_ready[i], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&s->ev_done[i], cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && launch_rope_table(s->rope_table, max_pos, L.d, static_cast<double>(L.theta), nullptr) == cudaSuccess &&
+       cudaDeviceSynchronize() == cudaSuccess;
+  if (!ok) {
+    const cudaError_t le = cudaGetLastError();
+    qcf_stack_destroy(s);
+    return set_error(ctx, QCF_ERR_WORKSPACE, std::string("qcf_stack_create: allocation failed: ") + cudaGetErrorString(le));
+  }
+  *out = s;
+  return QCF_OK;
+}
+
+void qcf_stack_destroy(qcf_stack* s) {
+  if (!s) return;
+  for (void* p : {static_cast<void*>(s->x), static_cast<void*>(s->h), static_cast<void*>(s->qkv), static_cast<void*>(s->q_new),
+                  static_cast<void*>(s->k_new), static_cast<void*>(s->v_new), static_cast<void*>(s->attn),
+                  static_cast<void*>(s->act), static_cast<void*>(s->rope_table)})
+    if (p) cudaFree(p);
+  for (int i = 0; i < qcf_stack::kRing; ++i) { if (s->stage_k[i]) cudaFree(s->stage_k[i]); if (s->stage_v[i]) cudaFree(s->stage_v[i]); }
+  for (int i = 0; i < 2; ++i) { if (s->probe_k[i]) cudaFree(s->probe_k[i]); if (s->probe_v[i]) cudaFree(s->probe_v[i]); }
+  for (cudaEvent_t e : s->ev_ready) if (e) cudaEventDestroy(e);
+  for (cudaEvent_t e : s->ev_done) if (e) cudaEventDestroy(e);
+  if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+  if (s->ev_join) cudaEventDestroy(s->ev_join);
+  if (s->zero_i32) cudaFree(s->zero_i32);
+  if (s->loader) cudaStreamDestroy(s->loader);
+  delete s;
+}
+
+qcf_status qcf_stack_layer(qcf_stack* s, int32_t layer, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                           int32_t n_rows, int32_t query_pos0, void* x, void* k_fused, void* v_fused, void* q_tap,
+                           void* stream) {
+  if (qcf_status e = check_stack_batch(s, b, "qcf_stack_layer")) return e;
+  qcf_ctx* ctx = s->ctx;
+  STK_REQUIRE(ctx, layer >= 0 && layer < s->dims.n_layers, "qcf_stack_layer: layer out of range");
+  STK_REQUIRE(ctx, n_rows >= 0 && n_rows <= s->max_rows, "qcf_stack_layer: n_rows exceeds max_rows of qcf_stack_create");
+  STK_REQUIRE(ctx, x && k_fused && v_fused, "qcf_stack_layer: NULL tensor pointer");
+  STK_REQUIRE(ctx, (sel == nullptr) || n_sel, "qcf_stack_layer: n_sel is NULL");
+  STK_REQUIRE(ctx, sel != nullptr || n_rows == b->h_n_ctx[0] + b->h_n_query[0], "qcf_stack_layer: dense mode takes all N + Lq rows");
+  const int top = sel ? (query_pos0 >= 0 ? query_pos0 : b->h_n_ctx[0]) + b->h_n_query[0] : n_rows;
+  STK_REQUIRE(ctx, top <= s->max_pos, "qcf_stack_layer: positions exceed max_pos of qcf_stack_create");
+  if (n_rows == 0) return QCF_OK;
+  return run_layer(s, layer, b, sel, n_sel, n_rows, query_pos0, static_cast<__nv_bfloat16*>(x), k_fused, v_fused, q_tap,
+                   static_cast<cudaStream_t>(stream));
+}
+
+qcf_status qcf_stack_prefill(qcf_stack* s, const qcf_batch* b, const int32_t* tokens, void* const* k_cache,
+                             void* const* v_cache, void* hidden_out, void* stream) {
+  if (qcf_status e = check_stack_batch(s, b, "qcf_stack_prefill")) return e;
+  qcf_ctx* ctx = s->ctx;
+  const int T = b->h_n_ctx[0] + b->h_n_query[0];
+  STK_REQUIRE(ctx, tokens && k_cache && v_cache, "qcf_stack_prefill: NULL argument");
+  STK_REQUIRE(ctx, T <= s->max_rows && T <= s->max_pos, "qcf_stack_prefill: request exceeds max_rows / max_pos");
+  if (T == 0) return QCF_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  STK_CUDA(ctx, launch_embed_gather(s->embed, tokens, nullptr, nullptr, 0, 0, T, s->dims.hidden, s->x, st));
+  for (int l = 0; l < s->dims.n_layers; ++l) {
+    STK_REQUIRE(ctx, k_cache[l] && v_cache[l], "qcf_stack_prefill: NULL cache pointer");
+    if (qcf_status e = run_layer(s, l, b, nullptr, nullptr, T, -1, s->x, k_cache[l], v_cache[l], nullptr, st)) return e;
+  }
+  if (hidden_out)
+    STK_CUDA(ctx, cudaMemcpyAsync(hidden_out, s->x, static_cast<size_t>(T) * s->dims.hidden * 2, cudaMemcpyDeviceToDevice, st));
+  return QCF_OK;
+}
+
+qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb, const qcf_fuse_args* a, void* stream) {
+  if (qcf_status e = check_stack_batch(s, mb, "qcf_stack_fuse")) return e;
+  if (qcf_status e = check_stack_batch(s, pb, "qcf_stack_fuse")) return e;
+  qcf_ctx* ctx = s->ctx;
+  const Layout& L = ctx->lay;
+  const int n_l = s->dims.n_layers;
+  STK_REQUIRE(ctx, a != nullptr, "qcf_stack_fuse: args is NULL");
+  STK_REQUIRE(ctx, a->k_pic && a->v_pic && a->k_anchor && a->v_anchor && a->k_fused && a->v_fused && a->tokens &&
+                       a->scores && a->sel && a->n_sel,
+              "qcf_stack_fuse: NULL argument");
+  STK_REQUIRE(ctx, a->ratio >= 0.0 && a->ratio <= 1.0, "qcf_stack_fuse: ratio must be in [0, 1]");
+  STK_REQUIRE(ctx, a->n_crit >= 1 && a->crit_layers, "qcf_stack_fuse: at least one critical layer is needed");
+  for (int i = 0; i < a->n_crit; ++i)
+    STK_REQUIRE(ctx, a->crit_layers[i] >= 0 && a->crit_layers[i] < n_l && (i == 0 || a->crit_layers[i] > a->crit_layers[i - 1]),
+                "qcf_stack_fuse: crit_layers must be ascending layer indices");
+  const int N = mb->h_n_ctx[0], Lq = mb->h_n_query[0];
+  STK_REQUIRE(ctx, pb->h_n_query[0] == Lq, "qcf_stack_fuse: probe batch must carry the same query length");
+  STK_REQUIRE(ctx, a->pool_rows >= 0 && a->anchor_rows >= 0 && a->pool_rows <= s->max_pool_rows &&
+                       a->anchor_rows <= s->max_pool_rows && static_cast<size_t>(pb->t_stride) <= s->probe_rows,
+              "qcf_stack_fuse: pools exceed max_pool_rows of qcf_stack_create");
+  const int k_sel = qcf_n_select(N, a->ratio);
+  const int n_rows = k_sel + Lq;
+  STK_REQUIRE(ctx, n_rows <= s->max_rows && Lq <= s->max_rows && N + Lq <= s->max_pos,
+              "qcf_stack_fuse: request exceeds max_rows / max_pos of qcf_stack_create");
+  const int l_max = a->crit_layers[a->n_crit - 1];
+  cudaStream_t cs = static_cast<cudaStream_t>(stream);
+  cudaStream_t ls = a->overlap ? s->loader : cs;
+  const size_t kv_row = static_cast<size_t>(L.hkv) * L.d * 2;
+  auto is_crit = [&](int l) { return std::find(a->crit_layers, a->crit_layers + a->n_crit, l) != a->crit_layers + a->n_crit; };
+  const int slot_pic0 = l_max + 1;                       // event slot of PIC layer l = slot_pic0 + l; anchor layer l = l
+  int ring = 0;
+
+  STK_CUDA(ctx, cudaEventRecord(s->ev_fork, cs));
+  if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(ls, s->ev_fork, 0));
+
+  // Loader jobs, in the order the pipeline consumes them.  The staging buffer of a job is read by the stitch kernel
+  // issued right behind it on the same stream, so ring reuse needs no cross-stream wait; destinations are per layer.
+  auto load_pic = [&](int l) -> qcf_status {
+    STK_REQUIRE(ctx, a->k_pic[l] && a->v_pic[l] && a->k_fused[l] && a->v_fused[l], "qcf_stack_fuse: NULL pool / cache pointer");
+    __nv_bfloat16 *sk = s->stage_k[ring], *sv = s->stage_v[ring];
+    ring = (ring + 1) % qcf_stack::kRing;
+    STK_CUDA(ctx, cudaMemcpyAsync(sk, a->k_pic[l], a->pool_rows * kv_row, cudaMemcpyDefault, ls));
+    STK_CUDA(ctx, cudaMemcpyAsync(sv, a->v_pic[l], a->pool_rows * kv_row, cudaMemcpyDefault, ls));
+    if (qcf_status e = qcf_rope_reposition(ctx, mb, sk, sv, a->k_fused[l], a->v_fused[l], ls)) return e;      // a1
+    STK_CUDA(ctx, cudaEventRecord(s->ev_ready[slot_pic0 + l], ls));
+    return QCF_OK;
+  };
+  auto load_anchor = [&](int l) -> qcf_status {
+    STK_REQUIRE(ctx, a->k_anchor[l] && a->v_anchor[l], "qcf_stack_fuse: NULL anchor pool pointer");
+    __nv_bfloat16 *sk = s->stage_k[ring], *sv = s->stage_v[ring];
+    ring = (ring + 1) % qcf_stack::kRing;
+    STK_CUDA(ctx, cudaMemcpyAsync(sk, a->k_anchor[l], a->anchor_rows * kv_row, cudaMemcpyDefault, ls));
+    STK_CUDA(ctx, cudaMemcpyAsync(sv, a->v_anchor[l], a->anchor_rows * kv_row, cudaMemcpyDefault, ls));
+    if (l >= 2 && ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(ls, s->ev_done[l - 2], 0));   // probe cache l&1 is free again
+    if (qcf_status e = qcf_rope_reposition(ctx, pb, sk, sv, s->probe_k[l & 1], s->probe_v[l & 1], ls)) return e;   // a1'
+    STK_CUDA(ctx, cudaEventRecord(s->ev_ready[l], ls));
+    return QCF_OK;
+  };
+
+  // ---- stage 1: selective token localization.  Loads are issued one layer ahead of their consumer.
+  auto issue_stage1_loads = [&](int l) -> qcf_status {
+    if (qcf_status e = load_anchor(l)) return e;
+    if (is_crit(l)) if (qcf_status e = load_pic(l)) return e;
+    return QCF_OK;
+  };
+  if (qcf_status e = issue_stage1_loads(0)) return e;
+  STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, nullptr, nullptr, 0, N, Lq, s->dims.hidden, s->x, cs));
+  bool first = true;
+  for (int l = 0; l <= l_max; ++l) {
+    if (l + 1 <= l_max) if (qcf_status e = issue_stage1_loads(l + 1)) return e;
+    if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(cs, s->ev_ready[l], 0));
+    if (qcf_status e = run_layer(s, l, pb, s->zero_i32, s->zero_i32, Lq, N, s->x, s->probe_k[l & 1], s->probe_v[l & 1], nullptr, cs))
+      return e;
+    if (is_crit(l)) {
+      if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(cs, s->ev_ready[slot_pic0 + l], 0));
+      if (qcf_status e = qcf_score(ctx, mb, s->q_new, a->k_fused[l], a->scores, first ? 0 : 1, cs)) return e;   // Eq. 18 / 20
+      first = false;
+    }
+    STK_CUDA(ctx, cudaEventRecord(s->ev_done[l], cs));
+  }
+  if (qcf_status e = qcf_select_topk(ctx, mb, a->scores, a->ratio, a->sel, a->n_sel, cs)) return e;               // Eq. 11
+
+  // ---- stage 2: pipeline cache fusion.  The loader runs ahead through all remaining layers
+  // (every layer has its own destination cache); the compute stream consumes them in order.
+  for (int l = 0; l < n_l; ++l)
+    if (!is_crit(l) || l > l_max) { if (qcf_status e = load_pic(l)) return e; }
+  STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, a->sel, a->n_sel, N, 0, n_rows, s->dims.hidden, s->x, cs));
+  for (int l = 0; l < n_l; ++l) {
+    if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(cs, s->ev_ready[slot_pic0 + l], 0));
+    if (qcf_status e = run_layer(s, l, mb, a->sel, a->n_sel, n_rows, -1, s->x, a->k_fused[l], a->v_fused[l], nullptr, cs)) return e;
+  }
+  if (a->hidden_out)
+    STK_CUDA(ctx, cudaMemcpyAsync(a->hidden_out, s->x, static_cast<size_t>(n_rows) * s->dims.hidden * 2, cudaMemcpyDeviceToDevice, cs));
+  return QCF_OK;
+}
+
+}  // extern "C"

@@ -64,10 +64,10 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   const int jc = slot % kSlotsPerHead;           // which group of 8 pairs
   const int e0 = head * D + jc * 8;              // first-half vector (elements), second half at + D/2
 
-  // ---- K: rotate by the chunk's offset angle.  off == 0 is the identity and is copied bit-exactly.
+  // ---- K: rotate by the chunk's offset angle.  A rotation position of 0 is the identity and is copied bit-exactly.
   const __nv_bfloat16* ks = k_pool + src_row * row_elems;
   __nv_bfloat16* kd = k_f + dst_row * row_elems;
-  if (off == 0) {
+  if (bd.chunk_rot[c] == 0) {
     for (int r = rsub; r < rows; r += rows_per_pass) {
       const uint4 a = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0);
       const uint4 b = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0 + D / 2);
@@ -106,7 +106,8 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
     }
   }
 
-  // ---- V: stitched in the same token order (byte copy)
+  // ---- V: stitched in the same token order (byte copy); skipped for the K-only scoring prefetch
+  if (v_pool == nullptr) return;
   const uint4* vs = reinterpret_cast<const uint4*>(v_pool + src_row * row_elems);
   uint4* vd = reinterpret_cast<uint4*>(v_f + dst_row * row_elems);
   const int n_vec = rows * (row_elems / 8);

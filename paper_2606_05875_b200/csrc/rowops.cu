@@ -1,0 +1,168 @@
+// a7 — the row-wise (non-GEMM) ops of the decoder block for the recomputed rows R = P u U (BASELINE config 3;
+// DESIGN.md readings (l), (q)): embedding gather of the layer-1 input, RMSNorm, and the fused per-head RMSNorm
+// ("QK-norm") + RoPE at the row's REQUEST position (anchors and query rows keep their original
+// position ids) that turns the packed QKV projection into q_new / k_new / v_new rows.  All memory-bound streams:
+// 128-bit loads where the layout allows, fp32 arithmetic, one bf16 rounding (RNE) per stored value.
+#include "qcf_internal.cuh"
+
+namespace qcf {
+
+namespace {
+
+// position of row r of a request: dense -> pos_off + r; selective -> sel[r] for r < n_sel, then N + (r - n_sel)
+struct RowPos {
+  const int32_t* sel;       // nullptr: dense
+  const int32_t* n_sel;     // device scalar of the request
+  int n_ctx;
+  int pos_off;
+  __device__ __forceinline__ int operator()(int r) const {
+    if (!sel) return pos_off + r;
+    const int ns = *n_sel;
+    return r < ns ? __ldg(sel + r) : n_ctx + (r - ns);
+  }
+};
+
+// (cos, sin)(p * theta^(-2j/d)) for p < n_pos, j < d/2, evaluated in double (angles reach 3e4 rad at theta^0 = 1)
+__global__ void rope_table_kernel(float2* __restrict__ table, int n_pos, int half, double theta) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_pos * half) return;
+  const int p = i / half, j = i % half;
+  const double inv_freq = pow(theta, -static_cast<double>(j) / static_cast<double>(half));     // -2j/d
+  double s, c;
+  sincos(static_cast<double>(p) * inv_freq, &s, &c);
+  table[i] = make_float2(static_cast<float>(c), static_cast<float>(s));
+}
+
+// x[r][:] = embed[tokens[pos(r)]][:]     one warp per row, 16-byte vectors
+__global__ void __launch_bounds__(256) embed_gather_kernel(const uint4* __restrict__ embed, const int32_t* __restrict__ tokens,
+                                                           RowPos rp, int n_rows, int row_vec, uint4* __restrict__ x) {
+  const int r = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (r >= n_rows) return;
+  const int tok = __ldg(tokens + rp(r));
+  const uint4* src = embed + static_cast<size_t>(tok) * row_vec;
+  uint4* dst = x + static_cast<size_t>(r) * row_vec;
+  for (int i = lane; i < row_vec; i += 32) dst[i] = ld_nc_v4(src + i);
+}
+
+// y = x / sqrt(mean(x^2) + eps) * g      one warp per row; the row (<= 16 KB) is re-read from L1/L2 for the second sweep
+__global__ void __launch_bounds__(256) rmsnorm_kernel(const uint4* __restrict__ x, const uint4* __restrict__ gain, float eps,
+                                                      int n_rows, int row_vec, uint4* __restrict__ y) {
+  const int r = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (r >= n_rows) return;
+  const uint4* src = x + static_cast<size_t>(r) * row_vec;
+  float ss = 0.f;
+  for (int i = lane; i < row_vec; i += 32) {
+    const uint4 v = src[i];
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { const float a = bf16lo(w[k]), b = bf16hi(w[k]); ss = fmaf(a, a, ss); ss = fmaf(b, b, ss); }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+  const float inv = rsqrtf(ss / static_cast<float>(row_vec * 8) + eps);
+  uint4* dst = y + static_cast<size_t>(r) * row_vec;
+  for (int i = lane; i < row_vec; i += 32) {
+    const uint4 v = src[i], gg = __ldg(gain + i);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w}, gw[4] = {gg.x, gg.y, gg.z, gg.w};
+    uint32_t o[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      o[k] = pack_bf16(bf16lo(w[k]) * inv * bf16lo(gw[k]), bf16hi(w[k]) * inv * bf16hi(gw[k]));
+    dst[i] = make_uint4(o[0], o[1], o[2], o[3]);
+  }
+}
+
+// qkv[r] = [q heads | k heads | v heads] (each d wide).  One warp per (row, head):
+//   q, k heads: RMSNorm over d with gain g_q / g_k, then RoPE (half-split pairs) at the row's request position
+//   v heads   : copied
+// Lane l owns pairs j in [l*P, l*P + P), P = d/64, i.e. elements j and j + d/2.
+template <int D>
+__global__ void __launch_bounds__(256) qknorm_rope_kernel(const __nv_bfloat16* __restrict__ qkv, const __nv_bfloat16* __restrict__ g_q,
+                                                          const __nv_bfloat16* __restrict__ g_k, const float2* __restrict__ table,
+                                                          RowPos rp, float eps, int n_rows, int hq, int hkv,
+                                                          __nv_bfloat16* __restrict__ q_out, __nv_bfloat16* __restrict__ k_out,
+                                                          __nv_bfloat16* __restrict__ v_out) {
+  constexpr int P = D / 64;
+  const int heads = hq + 2 * hkv;
+  const long long wid = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (wid >= static_cast<long long>(n_rows) * heads) return;
+  const int r = static_cast<int>(wid / heads), h = static_cast<int>(wid % heads);
+  const __nv_bfloat16* src = qkv + (static_cast<size_t>(r) * heads + h) * D;
+  float a[P], b[P];
+#pragma unroll
+  for (int i = 0; i < P; ++i) {
+    a[i] = __bfloat162float(src[lane * P + i]);
+    b[i] = __bfloat162float(src[D / 2 + lane * P + i]);
+  }
+  __nv_bfloat16* dst;
+  if (h >= hq + hkv) {                                   // v: copy
+    dst = v_out + (static_cast<size_t>(r) * hkv + (h - hq - hkv)) * D;
+#pragma unroll
+    for (int i = 0; i < P; ++i) { dst[lane * P + i] = src[lane * P + i]; dst[D / 2 + lane * P + i] = src[D / 2 + lane * P + i]; }
+    return;
+  }
+  const bool is_q = h < hq;
+  const __nv_bfloat16* gain = is_q ? g_q : g_k;
+  dst = is_q ? q_out + (static_cast<size_t>(r) * hq + h) * D : k_out + (static_cast<size_t>(r) * hkv + (h - hq)) * D;
+  float ss = 0.f;
+#pragma unroll
+  for (int i = 0; i < P; ++i) { ss = fmaf(a[i], a[i], ss); ss = fmaf(b[i], b[i], ss); }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+  const float inv = rsqrtf(ss / static_cast<float>(D) + eps);
+  const int pos = rp(r);
+  const float2* t = table + static_cast<size_t>(pos) * (D / 2) + lane * P;
+#pragma unroll
+  for (int i = 0; i < P; ++i) {
+    const float x0 = a[i] * inv * __bfloat162float(gain[lane * P + i]);
+    const float x1 = b[i] * inv * __bfloat162float(gain[D / 2 + lane * P + i]);
+    const float2 cs = __ldg(t + i);
+    dst[lane * P + i] = __float2bfloat16_rn(fmaf(x0, cs.x, -x1 * cs.y));
+    dst[D / 2 + lane * P + i] = __float2bfloat16_rn(fmaf(x1, cs.x, x0 * cs.y));
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_rope_table(float2* table, int n_pos, int d, double theta, cudaStream_t stream) {
+  const int n = n_pos * (d / 2);
+  if (n <= 0) return cudaSuccess;
+  rope_table_kernel<<<(n + 255) / 256, 256, 0, stream>>>(table, n_pos, d / 2, theta);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_embed_gather(const __nv_bfloat16* embed, const int32_t* tokens, const int32_t* sel, const int32_t* n_sel,
+                                int n_ctx, int pos_off, int n_rows, int hidden, __nv_bfloat16* x, cudaStream_t stream) {
+  if (n_rows <= 0) return cudaSuccess;
+  RowPos rp{sel, n_sel, n_ctx, pos_off};
+  embed_gather_kernel<<<(n_rows + 7) / 8, 256, 0, stream>>>(reinterpret_cast<const uint4*>(embed), tokens, rp, n_rows,
+                                                            hidden / 8, reinterpret_cast<uint4*>(x));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_rmsnorm(const __nv_bfloat16* x, const __nv_bfloat16* gain, float eps, int n_rows, int hidden,
+                           __nv_bfloat16* y, cudaStream_t stream) {
+  if (n_rows <= 0) return cudaSuccess;
+  rmsnorm_kernel<<<(n_rows + 7) / 8, 256, 0, stream>>>(reinterpret_cast<const uint4*>(x), reinterpret_cast<const uint4*>(gain),
+                                                       eps, n_rows, hidden / 8, reinterpret_cast<uint4*>(y));
+  return cudaGetLastError();
+}
+
+cudaError_t launch_qknorm_rope(const qcf_ctx* ctx, const __nv_bfloat16* qkv, const __nv_bfloat16* g_q, const __nv_bfloat16* g_k,
+                               const float2* table, const int32_t* sel, const int32_t* n_sel, int n_ctx, int pos_off,
+                               float eps, int n_rows, __nv_bfloat16* q_out, __nv_bfloat16* k_out, __nv_bfloat16* v_out,
+                               cudaStream_t stream) {
+  if (n_rows <= 0) return cudaSuccess;
+  const Layout& L = ctx->lay;
+  RowPos rp{sel, n_sel, n_ctx, pos_off};
+  const long long warps = static_cast<long long>(n_rows) * (L.hq + 2 * L.hkv);
+  const unsigned blocks = static_cast<unsigned>((warps + 7) / 8);
+  if (L.d == 128)
+    qknorm_rope_kernel<128><<<blocks, 256, 0, stream>>>(qkv, g_q, g_k, table, rp, eps, n_rows, L.hq, L.hkv, q_out, k_out, v_out);
+  else
+    qknorm_rope_kernel<64><<<blocks, 256, 0, stream>>>(qkv, g_q, g_k, table, rp, eps, n_rows, L.hq, L.hkv, q_out, k_out, v_out);
+  return cudaGetLastError();
+}
+
+}  // namespace qcf
