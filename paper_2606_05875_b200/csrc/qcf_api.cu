@@ -127,9 +127,10 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->score_row_ctr = nullptr;
   c->counters = nullptr;
   c->stage = nullptr;
+  c->ptc_units = nullptr; c->ptc_n_units = nullptr; c->ptc_part_o = c->ptc_part_ml = nullptr; c->ptc_item_ctr = nullptr;
   {
     const char* e = std::getenv("QCF_ATTN_IMPL");
-    c->attn_impl = (e && std::strcmp(e, "mma") == 0) ? 0 : 1;
+    c->attn_impl = (e && std::strcmp(e, "mma") == 0) ? 0 : ((e && std::strcmp(e, "ptc") == 0) ? 2 : 1);
     const char* e2 = std::getenv("QCF_SCORE_IMPL");
     c->score_impl = (e2 && std::strcmp(e2, "mma") == 0) ? 0 : 1;
     const char* e3 = std::getenv("QCF_ATTN_CLUSTER");
@@ -155,6 +156,16 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
             cudaMemset(c->score_row_ctr, 0, row_ctr_n * sizeof(unsigned int)) == cudaSuccess &&
             cudaMalloc(&c->counters, c->n_counters * sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(c->counters, 0, c->n_counters * sizeof(unsigned int)) == cudaSuccess;
+  if (c->attn_impl == 2) {     // experimental persistent attention kernel (opt-in): work list, split-KV partials, counters
+    const size_t slots = static_cast<size_t>(attn_ptc_slots(c));
+    const size_t o_bytes = slots * static_cast<size_t>(128) * lay->head_dim * 4, ml_bytes = slots * 2 * 128 * 4;
+    const size_t items = attn_ptc_items(c);
+    ok = ok && cudaMalloc(&c->ptc_units, attn_ptc_units_bytes(c)) == cudaSuccess &&
+         cudaMalloc(&c->ptc_n_units, 16) == cudaSuccess && cudaMemset(c->ptc_n_units, 0, 16) == cudaSuccess &&
+         cudaMalloc(&c->ptc_part_o, o_bytes + 16) == cudaSuccess && cudaMalloc(&c->ptc_part_ml, ml_bytes + 16) == cudaSuccess &&
+         cudaMalloc(&c->ptc_item_ctr, items * sizeof(unsigned int) + 16) == cudaSuccess &&
+         cudaMemset(c->ptc_item_ctr, 0, items * sizeof(unsigned int) + 16) == cudaSuccess;
+  }
   if (!ok) {
     const cudaError_t le = cudaGetLastError();
     qcf_destroy(c);
@@ -168,6 +179,7 @@ void qcf_destroy(qcf_ctx* c) {
   if (!c) return;
   cudaFree(c->stats_m); cudaFree(c->stats_l); cudaFree(c->score_part); cudaFree(c->counters);
   cudaFree(c->score_lse); cudaFree(c->score_row_ctr);
+  cudaFree(c->ptc_units); cudaFree(c->ptc_n_units); cudaFree(c->ptc_part_o); cudaFree(c->ptc_part_ml); cudaFree(c->ptc_item_ctr);
   if (c->ev_ring) {
     for (int i = 0; i < qcf_ctx::kEvRing; ++i)
       for (int j = 0; j < 6; ++j) if (c->ev_ring[i][j]) cudaEventDestroy(c->ev_ring[i][j]);

@@ -47,7 +47,8 @@ struct qcf_ctx {
   int n_sm;
   int max_batch, max_ctx, max_query;
   int score_impl;        // 1: tcgen05 kernels (default); 0: legacy mma.sync kernels (QCF_SCORE_IMPL=mma)
-  int attn_impl;         // 1: tcgen05/TMEM/TMA kernel (default); 0: legacy mma.sync kernel (QCF_ATTN_IMPL=mma, for A/B timing)
+  int attn_impl;         // 2: persistent tcgen05 kernel with a device work list (QCF_ATTN_IMPL=ptc); 1: one CTA per tile (tc);
+                         // 0: legacy mma.sync kernel (mma, for A/B timing)
   int gemm_mt;           // GEMM tile height in units of 128 rows: 0 = heuristic, else 1 / 2 (QCF_GEMM_MT)
   int attn_cluster;      // split-KV cluster size of the tcgen05 attention kernel: 0 = heuristic, else 1/2/4 (QCF_ATTN_CLUSTER)
   double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
@@ -58,6 +59,12 @@ struct qcf_ctx {
   unsigned int* score_row_ctr;   // pass-1 arrival counters per (request, kv-head, row tile), self-resetting
   float* score_part;     // score pass-2 per-kv-head partial column sums [max_batch][Hkv][max_ctx]
   unsigned int* counters;  // tile counters (zeroed, self-resetting)
+  // persistent attention kernel: work list, split-KV partials, per-item arrival counters (zeroed, self-resetting)
+  void* ptc_units;
+  int32_t* ptc_n_units;
+  float* ptc_part_o;
+  float* ptc_part_ml;
+  unsigned int* ptc_item_ctr;
   size_t n_counters;
   // host staging for qcf_layer_step_host
   struct HostStage* stage;
@@ -109,6 +116,13 @@ cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, co
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
 
+cudaError_t launch_attn_ptc(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
+                            const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
+                            const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
+size_t attn_ptc_units_bytes(const qcf_ctx*);
+size_t attn_ptc_items(const qcf_ctx*);
+int attn_ptc_slots(const qcf_ctx*);
+size_t attn_ptc_slot_bytes(const qcf_ctx*);
 cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
                         __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
 cudaError_t launch_rope_table(float2* table, int n_pos, int d, double theta, cudaStream_t);

@@ -205,6 +205,7 @@ cudaError_t launch_attn(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t stream) {
   if (b->batch == 0 || b->t_stride == 0) return cudaSuccess;
+  if (ctx->attn_impl == 2) return launch_attn_ptc(ctx, b, sel, n_sel, q, rows_by_position, k_f, v_f, out, lse, stream);
   if (ctx->attn_impl == 1) return launch_attn_tc(ctx, b, sel, n_sel, q, rows_by_position, k_f, v_f, out, lse, stream);
   const Layout& L = ctx->lay;
   const int PT = BM / L.g;

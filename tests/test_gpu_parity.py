@@ -300,6 +300,40 @@ def test_recompute_attn_split_kv_cluster(name, ncl, monkeypatch):
     assert np.max(np.abs(_f64(out2[0, : r.n_ctx + r.n_query]) - want)) <= 2e-2
 
 
+@pytest.mark.parametrize("impl", ["ptc", "tc"])
+@pytest.mark.parametrize("name", SMALL)
+def test_recompute_attn_impls(name, impl, monkeypatch):
+    """Both tcgen05 attention kernels (the default one-CTA-per-tile kernel and the opt-in persistent work-list kernel
+    with split-KV partials merged by the last arriver) against the oracle on random selections, plus the dense comparator."""
+    monkeypatch.setenv("QCF_ATTN_IMPL", impl)
+    wl, ctx, dw = _setup(name)
+    rng = np.random.default_rng(5)
+    sels = [np.sort(rng.choice(r.n_ctx, size=O.n_select(r.n_ctx, wl.cfg.ratio), replace=False)) for r in wl.requests]
+    _run_recompute(ctx, dw, sels)
+    for b in range(dw.B):
+        _check_recompute(wl, dw, b, sels[b])
+    out2 = torch.zeros_like(dw.out)
+    ctx.qcf_full_prefill_attn(dw.batch, dw.q_new, dw.k_new, dw.v_new, out2)
+    torch.cuda.synchronize()
+    for b, r in enumerate(wl.requests):
+        want = O.full_prefill_attn(O.widen_bf16(r.q_new), O.widen_bf16(r.k_new), O.widen_bf16(r.v_new))
+        assert np.max(np.abs(_f64(out2[b, : r.n_ctx + r.n_query]) - want)) <= 2e-2
+    # repeated launches are bit-identical (split partials are merged in chunk order)
+    out3 = torch.zeros_like(dw.out)
+    ctx.qcf_full_prefill_attn(dw.batch, dw.q_new, dw.k_new, dw.v_new, out3)
+    torch.cuda.synchronize()
+    assert torch.equal(out2, out3)
+
+
+@pytest.mark.parametrize("impl", ["ptc", "tc"])
+def test_full_size_c2_attention_impls(impl, monkeypatch):
+    monkeypatch.setenv("QCF_ATTN_IMPL", impl)
+    wl, ctx, dw = _setup("c2")
+    ctx.qcf_layer_step(dw.batch, dw.layer_args())
+    torch.cuda.synchronize()
+    _check_full_size(wl, dw, 0, 31)
+
+
 # --------------------------------------------------------------------------------------------- a6
 
 @pytest.mark.parametrize("name", SMALL)
