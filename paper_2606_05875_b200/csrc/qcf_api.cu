@@ -134,6 +134,8 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
     const char* e2 = std::getenv("QCF_SCORE_IMPL");
     c->score_impl = (e2 && std::strcmp(e2, "mma") == 0) ? 0 : 1;
     const char* e3 = std::getenv("QCF_ATTN_CLUSTER");
+    const char* e5 = std::getenv("QCF_PDL");
+    c->pdl = (e5 && std::strcmp(e5, "0") == 0) ? 0 : 1;
     const char* e4 = std::getenv("QCF_GEMM_MT");
     const int mt = e4 ? std::atoi(e4) : 0;
     c->gemm_mt = (mt == 1 || mt == 2) ? mt : 0;

@@ -49,6 +49,7 @@ struct qcf_ctx {
   int score_impl;        // 1: tcgen05 kernels (default); 0: legacy mma.sync kernels (QCF_SCORE_IMPL=mma)
   int attn_impl;         // 2: persistent tcgen05 kernel with a device work list (QCF_ATTN_IMPL=ptc); 1: one CTA per tile (tc);
                          // 0: legacy mma.sync kernel (mma, for A/B timing)
+  int pdl;               // 1: chain the step's kernels with programmatic dependent launch (default); 0: QCF_PDL=0
   int gemm_mt;           // GEMM tile height in units of 128 rows: 0 = heuristic, else 1 / 2 (QCF_GEMM_MT)
   int attn_cluster;      // split-KV cluster size of the tcgen05 attention kernel: 0 = heuristic, else 1/2/4 (QCF_ATTN_CLUSTER)
   double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
@@ -145,9 +146,38 @@ cudaError_t launch_attn_tc(const qcf_ctx*, const qcf_batch*, const int32_t* sel,
 // ------------------------------------------------------------------------------------------- device helpers
 #ifdef __CUDACC__
 
+// Host: launch `kern` with the programmatic-stream-serialization attribute when `pdl` is set (plain launch otherwise).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(int pdl, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                              Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
+// Programmatic dependent launch (PDL): a kernel launched with launch_pdl may start while its predecessor in the stream
+// is still draining.  pdl_trigger() lets the NEXT kernel's CTAs be scheduled as soon as every CTA of this grid has
+// called it; pdl_wait() blocks until every predecessor grid has completed and its writes are visible — it must precede
+// the first access to anything a predecessor wrote OR still reads (the step reuses its buffers every layer).
+// A PDL kernel's lifetime overlaps its predecessor's, so data the predecessor writes is NOT read-only for it: such data
+// must be read with coherent loads (plain / __ldcg / TMA), never ld.global.nc / __ldg / const __restrict__ promotion.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// coherent, L1-cached 32-bit load (never promoted to the non-coherent path, see the PDL note above)
+__device__ __forceinline__ int ld_ca_s32(const int32_t* p) {
+  int v;
+  asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
 __device__ __forceinline__ uint4 ld_nc_v4(const void* p) {
   uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+  asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
                : "l"(p));
   return r;

@@ -101,6 +101,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int PT = BM / G;
   // 1-D grid, heaviest tiles of ALL (request, kv-head) pairs first: block id -> (tile descending, head, request)
   // The CTAs of a cluster (consecutive block ids) share one work item and split its key tiles.
+  pdl_trigger();
+  pdl_wait();          // n_sel / sel below are written by the predecessors
   const int ncl = static_cast<int>(cluster_nctarank());
   const int crank = static_cast<int>(cluster_ctarank());
   const int item = static_cast<int>(blockIdx.x) / ncl;
@@ -110,7 +112,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int b = gb / hkv, g = gb % hkv;
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
   const bool dense = sel == nullptr;
-  const int ns = dense ? 0 : n_sel[b];
+  const int ns = dense ? 0 : ld_ca_s32(n_sel + b);     // coherent loads for everything a predecessor wrote (PDL)
   const int n_rows = dense ? N + Lq : ns + Lq;
   const int n_tiles = (n_rows + PT - 1) / PT;
   if (tile >= n_tiles) return;
@@ -119,7 +121,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int* sel_b = dense ? nullptr : sel + static_cast<size_t>(b) * bd.n_stride;
   auto pos_of = [&](int r) -> int {          // request position of row r of R (padding rows: 0, never stored)
     if (r >= n_rows) return 0;
-    return dense ? r : (r < ns ? __ldg(sel_b + r) : N + (r - ns));
+    return dense ? r : (r < ns ? ld_ca_s32(sel_b + r) : N + (r - ns));
   };
   const int p_min = pos_of(ridx0);
   const int p_max = pos_of(min(ridx0 + PT, n_rows) - 1);
@@ -532,13 +534,15 @@ cudaError_t launch_attn_tc(const qcf_ctx* ctx, const qcf_batch* b, const int32_t
   cfg.gridDim = grid;
   cfg.blockDim = dim3(kThreads);
   cfg.stream = stream;
-  cudaLaunchAttribute attrs[1];
+  cudaLaunchAttribute attrs[2];
+  attrs[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attrs[1].val.programmaticStreamSerializationAllowed = 1;
   attrs[0].id = cudaLaunchAttributeClusterDimension;
   attrs[0].val.clusterDim.x = static_cast<unsigned>(ncl);
   attrs[0].val.clusterDim.y = 1;
   attrs[0].val.clusterDim.z = 1;
   cfg.attrs = attrs;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = ctx->pdl ? 2 : 1;
   const BatchDev bd = b->dev;
   const int hq = L.hq, hkv = L.hkv;
   if (L.d == 128) {

@@ -57,6 +57,7 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   const size_t src_row = static_cast<size_t>(bd.chunk_row[c]) + row0;
   const size_t dst_row = static_cast<size_t>(req) * bd.t_stride + off + row0;
 
+  pdl_trigger();
   const int slot = threadIdx.x % slots;
   const int rsub = threadIdx.x / slots;
   const int rows_per_pass = blockDim.x / slots;
@@ -67,7 +68,9 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   // ---- K: rotate by the chunk's offset angle.  A rotation position of 0 is the identity and is copied bit-exactly.
   const __nv_bfloat16* ks = k_pool + src_row * row_elems;
   __nv_bfloat16* kd = k_f + dst_row * row_elems;
-  if (bd.chunk_rot[c] == 0) {
+  const bool identity = bd.chunk_rot[c] == 0;
+  pdl_wait();                          // before the first pool read / cache write (descriptor reads above are constant)
+  if (identity) {
     for (int r = rsub; r < rows; r += rows_per_pass) {
       const uint4 a = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0);
       const uint4 b = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0 + D / 2);
@@ -134,10 +137,8 @@ cudaError_t launch_reposition(const qcf_ctx* ctx, const qcf_batch* b, const __nv
   if (rpp > kRepoRows) rpp = kRepoRows;
   const int threads = slots * rpp;     // slots <= 512 is enforced at qcf_create
   if (ctx->lay.d == 128)
-    reposition_kernel<128><<<b->repo_blocks, threads, 0, stream>>>(b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
-  else
-    reposition_kernel<64><<<b->repo_blocks, threads, 0, stream>>>(b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
-  return cudaGetLastError();
+    return launch_pdl(ctx->pdl, reposition_kernel<128>, dim3(b->repo_blocks), dim3(threads), 0, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
+  return launch_pdl(ctx->pdl, reposition_kernel<64>, dim3(b->repo_blocks), dim3(threads), 0, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
 }
 
 }  // namespace qcf

@@ -13,15 +13,17 @@ __global__ void __launch_bounds__(256) scatter_kernel(BatchDev bd, int row_vec, 
                                                       const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
                                                       int rows_by_position, uint4* __restrict__ k_f,
                                                       uint4* __restrict__ v_f) {
+  pdl_trigger();
   const int b = blockIdx.y;
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
-  const int ns = n_sel[b];
+  pdl_wait();
+  const int ns = __ldcg(n_sel + b);         // coherent loads: written by a predecessor this kernel may overlap (PDL)
   const int n_rows = ns + Lq;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int warps = blockDim.x >> 5;
   const size_t base = static_cast<size_t>(b) * bd.t_stride;
   for (int r = blockIdx.x * warps + warp; r < n_rows; r += gridDim.x * warps) {
-    const int p = r < ns ? sel[static_cast<size_t>(b) * bd.n_stride + r] : N + (r - ns);
+    const int p = r < ns ? __ldcg(sel + static_cast<size_t>(b) * bd.n_stride + r) : N + (r - ns);
     const size_t src = (base + (rows_by_position ? p : r)) * row_vec;
     const size_t dst = (base + p) * row_vec;
     for (int i = lane; i < row_vec; i += 128) {
@@ -47,10 +49,9 @@ cudaError_t launch_scatter(const qcf_ctx* ctx, const qcf_batch* b, const int32_t
   int blocks = (max_rows + 7) / 8;
   const int cap = ctx->n_sm * 8;
   if (blocks > cap) blocks = cap;
-  scatter_kernel<<<dim3(blocks, b->batch), 256, 0, stream>>>(
+  return launch_pdl(ctx->pdl, scatter_kernel, dim3(blocks, b->batch), dim3(256), 0, stream,
       b->dev, row_vec, sel, n_sel, reinterpret_cast<const uint4*>(k_new), reinterpret_cast<const uint4*>(v_new),
       rows_by_position, reinterpret_cast<uint4*>(k_f), reinterpret_cast<uint4*>(v_f));
-  return cudaGetLastError();
 }
 
 }  // namespace qcf

@@ -104,10 +104,12 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   } else if (warp == 1) {
     tmem_alloc<kTmemCols>(sbase + S::oTmem);
   }
+  pdl_trigger();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  pdl_wait();          // barrier init, TMEM allocation and descriptor prefetch above overlap the predecessor's tail
 
   // TMA coordinates of a 128-row tile of query rows / of keys
   auto load_q_tile = [&](uint32_t dst, uint32_t mbar, int tile) {
@@ -351,14 +353,12 @@ cudaError_t launch(const qcf_ctx* ctx, const qcf_batch* b, const CUtensorMap& tm
   if (row_tiles > 0) {
     auto k1 = score_tc_kernel<D, 1>;
     cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    k1<<<dim3(a.n_splits, row_tiles, b->batch * a.hkv), kThreads, smem, stream>>>(tm_q, tm_k, b->dev, a);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = launch_pdl(ctx->pdl, k1, dim3(a.n_splits, row_tiles, b->batch * a.hkv), dim3(kThreads), smem, stream, tm_q, tm_k, b->dev, a);
     if (e != cudaSuccess) return e;
   }
   auto k2 = score_tc_kernel<D, 2>;
   cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-  k2<<<dim3(key_tiles, a.hkv, b->batch), kThreads, smem, stream>>>(tm_q, tm_k, b->dev, a);
-  return cudaGetLastError();
+  return launch_pdl(ctx->pdl, k2, dim3(key_tiles, a.hkv, b->batch), dim3(kThreads), smem, stream, tm_q, tm_k, b->dev, a);
 }
 
 }  // namespace

@@ -24,8 +24,10 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   __shared__ unsigned int hist[256];
   __shared__ unsigned int s_prefix, s_remaining;
   __shared__ unsigned int warp_cnt[32];                          // packed (gt << 16) | eq per warp
+  pdl_trigger();
   const int b = blockIdx.x;
   const int N = bd.n_ctx[b];
+  pdl_wait();
   const int k = static_cast<int>(floor(ratio * static_cast<double>(N) + 1e-6));    // reading (g)
   const float* s = scores + static_cast<size_t>(b) * bd.n_stride;
   int32_t* out = sel + static_cast<size_t>(b) * bd.n_stride;
@@ -47,7 +49,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
     const uint32_t prefix = s_prefix;
     const uint32_t mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
     for (int i = tid; i < N; i += kThreads) {
-      const uint32_t key = order_key(s[i]);
+      const uint32_t key = order_key(__ldcg(s + i));
       if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 0xffu], 1u);
     }
     __syncthreads();
@@ -87,7 +89,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
     const int i = base + tid;
     uint32_t key = 0u;
     const bool valid = i < N;
-    if (valid) key = order_key(s[i]);
+    if (valid) key = order_key(__ldcg(s + i));
     const bool gt = valid && key > T, eq = valid && key == T;
     const unsigned int bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
     if (lane == 0) warp_cnt[warp] = (static_cast<unsigned int>(__popc(bg)) << 16) | static_cast<unsigned int>(__popc(be));
@@ -117,11 +119,10 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
 
 }  // namespace
 
-cudaError_t launch_topk(const qcf_ctx*, const qcf_batch* b, const float* scores, double ratio, int32_t* sel,
+cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* scores, double ratio, int32_t* sel,
                         int32_t* n_sel, cudaStream_t stream) {
   if (b->batch == 0) return cudaSuccess;
-  topk_kernel<<<b->batch, kThreads, 0, stream>>>(b->dev, scores, ratio, sel, n_sel);
-  return cudaGetLastError();
+  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), 0, stream, b->dev, scores, ratio, sel, n_sel);
 }
 
 }  // namespace qcf

@@ -353,6 +353,26 @@ def test_layer_step_chain(name):
         _check_recompute(wl, dw, b, got_sel, sentinel=False)        # outputs checked against the oracle run on the GPU's selection
 
 
+def test_layer_step_back_to_back_is_race_free():
+    """The step's kernels are chained with programmatic dependent launch: kernel n+1 may start while kernel n drains,
+    and the next step's first kernel while this step's attention drains.  30 steps issued back to back (no host sync,
+    buffers reused, a foreign kernel scribbling over the outputs in between) must reproduce a lone step bit for bit."""
+    wl, ctx, dw = _setup("t_mid")
+    args = dw.layer_args(lse=dw.lse)
+    ctx.qcf_layer_step(dw.batch, args)
+    torch.cuda.synchronize()
+    ref = [t.clone() for t in (dw.scores, dw.sel, dw.n_sel, dw.out, dw.k_fused, dw.v_fused, dw.lse)]
+    for i in range(30):
+        if i % 3 == 0:
+            dw.out.fill_(float(i)); dw.sel.fill_(0); dw.n_sel.fill_(0); dw.scores.fill_(-1.0)
+        ctx.qcf_layer_step(dw.batch, args)
+    torch.cuda.synchronize()
+    k = int(ref[2][0])
+    n_r = k + wl.requests[0].n_query
+    assert torch.equal(ref[0], dw.scores) and torch.equal(ref[1][0, :k], dw.sel[0, :k]) and torch.equal(ref[2], dw.n_sel)
+    assert torch.equal(ref[3][0, :n_r], dw.out[0, :n_r]) and torch.equal(ref[4], dw.k_fused) and torch.equal(ref[5], dw.v_fused)
+
+
 def test_layer_step_profiling_and_noncritical():
     wl, ctx, dw = _setup("t_mid")
     ctx.qcf_set_profiling(True)
