@@ -34,7 +34,13 @@ constexpr int kTmemCols = 256;  // S_0, S_1 (BN fp32 columns each; bf16 P_j alia
 constexpr int kColO = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
-constexpr float kRescaleThreshold = 8.0f;     // log2 units: P stays <= 2^8
+constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (relative to the reference max) exceeds 2^8
+#ifndef QCF_ATTN_MUFU_PAIRS
+#define QCF_ATTN_MUFU_PAIRS 4
+#endif
+// Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Measured on c2: 4 -> 84 us,
+// 3 -> 91 us, 2 -> 104 us: the sweep is issue-bound, not MUFU-bound, so every exponential goes to the MUFU.
+constexpr int kMufuPairs = QCF_ATTN_MUFU_PAIRS;
 
 // Two CTAs are resident per SM (96 KB of shared memory, 256 TMEM columns and <= 168 registers each).  Inside a CTA
 // S_{j+1} = Q K_{j+1}^T is issued before P_j V_j, so the softmax of tile j overlaps it; across the two CTAs the
@@ -107,7 +113,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int crank = static_cast<int>(cluster_ctarank());
   const int item = static_cast<int>(blockIdx.x) / ncl;
   const int n_gb = hkv * bd.batch;
-  const int tile = max_tiles - 1 - item / n_gb;
+  const int t_idx = item / n_gb;                   // 0 = this request's heaviest (last) row tile
   const int gb = item % n_gb;
   const int b = gb / hkv, g = gb % hkv;
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
@@ -115,7 +121,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int ns = dense ? 0 : ld_ca_s32(n_sel + b);     // coherent loads for everything a predecessor wrote (PDL)
   const int n_rows = dense ? N + Lq : ns + Lq;
   const int n_tiles = (n_rows + PT - 1) / PT;
-  if (tile >= n_tiles) return;
+  // Heaviest first RELATIVE TO THE REQUEST'S OWN tile count: the CTAs without work (the grid is sized for t_stride rows,
+  // a selective launch fills a third of it) come last and retire under the tail instead of delaying the heavy tiles.
+  if (t_idx >= n_tiles) return;
+  const int tile = n_tiles - 1 - t_idx;
   const int ridx0 = tile * PT;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int* sel_b = dense ? nullptr : sel + static_cast<size_t>(b) * bd.n_stride;
@@ -246,48 +255,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
       tc_fence_after();
 
       uint32_t pk[BN / 2];      // P_j as bf16 pairs, kept in registers until the reference max is known to be valid
-      float tile_max, tile_sum;
-      // One sweep over the S row: p = 2^(s*scale - m_ref) against the REFERENCE max of the previous tiles, while the
-      // true row max of this tile is tracked on the ALU pipe.  3 of 4 exponentials go to MUFU.EX2, the 4th is a
-      // Cody-Waite + degree-3 polynomial on the FMA pipe (MUFU, at 16/clk/SM, is as tight as the tensor pipe here).
-      auto sweep = [&](float m_ref) {
-        float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
-        uint32_t sa[32], sb[32];
-        tmem_ld32(s_addr, sa);
-        tmem_ld32(s_addr + 32, sb);
-#pragma unroll
-        for (int c = 0; c < BN / 32; ++c) {
-          uint32_t(&cur)[32] = (c & 1) ? sb : sa;
-          if (c == 0) tmem_wait_ld();
-#pragma unroll
-          for (int i = 0; i < 32; i += 4) {
-            float v0 = __uint_as_float(cur[i]), v1 = __uint_as_float(cur[i + 1]);
-            float v2 = __uint_as_float(cur[i + 2]), v3 = __uint_as_float(cur[i + 3]);
-            if (need_mask) {
-              const int k = key0 + c * 32 + i;
-              if (k > pos) v0 = -INFINITY;
-              if (k + 1 > pos) v1 = -INFINITY;
-              if (k + 2 > pos) v2 = -INFINITY;
-              if (k + 3 > pos) v3 = -INFINITY;
-            }
-            mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1); mx2 = fmaxf(mx2, v2); mx3 = fmaxf(mx3, v3);
-            const float p0 = ex2(fmaf(v0, scale_log2, -m_ref));
-            const float p1 = ex2(fmaf(v1, scale_log2, -m_ref));
-            const float p2 = ex2(fmaf(v2, scale_log2, -m_ref));
-            const float p3 = ex2_poly(fmaf(v3, scale_log2, -m_ref));
-            l0 += p0; l1 += p1; l2 += p2; l3 += p3;
-            pk[c * 16 + (i >> 1)] = pack_bf16(p0, p1);
-            pk[c * 16 + (i >> 1) + 1] = pack_bf16(p2, p3);
-          }
-        }
-        tile_max = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
-        tile_sum = (l0 + l1) + (l2 + l3);
-      };
-
-      if (j == 0) {
-        // first tile: the reference is its own max.  Key 0 is visible to every row, so it is finite on rank 0; on a
-        // split-KV rank > 0 a row may see none of this CTA's keys: the clamp keeps the reference finite (p = 0, l = 0).
+      float tile_sum;
+      // max over this row's visible scores of the tile, in log2 units (only the first tile and the rare rescale need it)
+      auto row_max = [&]() -> float {
         float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
         for (int c = 0; c < BN / 32; ++c) {
@@ -304,17 +274,89 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
             mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1);
           }
         }
-        m_used = fmaxf(fmaxf(mx0, mx1) * scale_log2, -1e30f);
+        return fmaxf(mx0, mx1) * scale_log2;
+      };
+      // One sweep over the S row: p = 2^(s*scale - m_ref) against the REFERENCE max of the previous tiles; returns whether
+      // the reference max is stale (see the test at the end).  The sweep is issue-bound, so the unmasked tiles (all but the
+      // diagonal ones) run on packed pairs: FFMA2 for scale-and-subtract, FADD2 for the row sum, MUFU.EX2 for the exponentials.
+      auto sweep = [&](float m_ref) -> bool {
+        uint32_t sa[32], sb[32];
+        tmem_ld32(s_addr, sa);
+        tmem_ld32(s_addr + 32, sb);
+        if (!need_mask) {
+          const uint64_t sc2 = f2_pack(scale_log2, scale_log2), nm2 = f2_pack(-m_ref, -m_ref);
+          uint64_t l2a = 0ull, l2b = 0ull;
+#pragma unroll
+          for (int c = 0; c < BN / 32; ++c) {
+            uint32_t(&cur)[32] = (c & 1) ? sb : sa;
+            if (c == 0) tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; i += 8) {
+              float p[8];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                const uint64_t t = f2_fma(f2_pack(__uint_as_float(cur[i + 2 * q]), __uint_as_float(cur[i + 2 * q + 1])), sc2, nm2);
+                if (q < kMufuPairs) {
+                  float t0, t1;
+                  f2_unpack(t, t0, t1);
+                  p[2 * q] = ex2(t0); p[2 * q + 1] = ex2(t1);
+                } else {
+                  ex2_poly2(t, p[2 * q], p[2 * q + 1]);
+                }
+              }
+              l2a = f2_add(l2a, f2_add(f2_pack(p[0], p[1]), f2_pack(p[2], p[3])));
+              l2b = f2_add(l2b, f2_add(f2_pack(p[4], p[5]), f2_pack(p[6], p[7])));
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                const uint32_t w = pack_bf16(p[2 * q], p[2 * q + 1]);
+                pk[c * 16 + (i >> 1) + q] = w;
+              }
+            }
+          }
+          float s0, s1;
+          f2_unpack(f2_add(l2a, l2b), s0, s1);
+          tile_sum = s0 + s1;
+        } else {
+          float l0 = 0.f, l1 = 0.f;
+          tmem_wait_ld();
+#pragma unroll
+          for (int c = 0; c < BN / 32; ++c) {
+            uint32_t(&cur)[32] = (c & 1) ? sb : sa;
+#pragma unroll
+            for (int i = 0; i < 32; i += 2) {
+              float v0 = __uint_as_float(cur[i]), v1 = __uint_as_float(cur[i + 1]);
+              const int k = key0 + c * 32 + i;
+              if (k > pos) v0 = -INFINITY;
+              if (k + 1 > pos) v1 = -INFINITY;
+              const float p0 = ex2(fmaf(v0, scale_log2, -m_ref));
+              const float p1 = ex2(fmaf(v1, scale_log2, -m_ref));
+              l0 += p0; l1 += p1;
+              const uint32_t w = pack_bf16(p0, p1);
+              pk[c * 16 + (i >> 1)] = w;
+            }
+          }
+          tile_sum = l0 + l1;
+        }
+        // Staleness test at no cost per element: any p > 2^8 (or an inf / NaN from an overflowed p) makes the row sum
+        // exceed 2^8, and with an exact reference the sum is at most BN = 64, so P stays <= 2^8 as with a per-element
+        // test (a 2^14 bound — BN * 2^8 — was tried and cost accuracy on the heavy-hitter config: 2.8e-2 vs <= 2e-2).
+        return !(tile_sum <= kRescaleSum);
+      };
+
+      if (j == 0) {
+        // first tile: the reference is its own max.  Key 0 is visible to every row, so it is finite on rank 0; on a
+        // split-KV rank > 0 a row may see none of this CTA's keys: the clamp keeps the reference finite (p = 0, l = 0).
+        m_used = fmaxf(row_max(), -1e30f);
         sweep(m_used);
       } else {
-        sweep(m_used);
-        if (__any_sync(0xffffffffu, tile_max > m_used + kRescaleThreshold)) {
+        const bool grow = sweep(m_used);
+        if (__any_sync(0xffffffffu, grow)) {
           // lazy correction: O and l are relative to m_used; move the reference only when the max grew by > 2^8
           // P_{j-1} V_{j-1} has landed in O.  (Two alternating barriers: a warp may run one tile ahead of the
           // slowest warp, and a single barrier's parity would then alias two phases.)
           mbar_wait(bar(kODone + ((j - 1) & 1)), ((j - 1) >> 1) & 1);
           tc_fence_after();
-          const float m_t = fmaxf(m_used, tile_max);
+          const float m_t = fmaxf(m_used, row_max());
           const float f = ex2(m_used - m_t);
           m_used = m_t;
           l *= f;
@@ -512,7 +554,7 @@ cudaError_t launch_attn_tc(const qcf_ctx* ctx, const qcf_batch* b, const int32_t
   const int PT = BM / L.g;
   const int max_tiles = (b->t_stride + PT - 1) / PT;
   // Split-KV width (cluster size).  Splitting costs a second prologue/epilogue per item and a cluster rendezvous, and
-  // measured on c2 (400 items for 296 resident CTAs) it loses to the unsplit launch (112 -> 131 us at 2, 201 us at 4),
+  // measured on c2 (400 items for 296 resident CTAs, where the SMs are throughput-bound) it loses to the unsplit launch,
   // so it is used only where the unsplit grid leaves most of the machine empty: few rows against a long cache
   // (rho ~ 0: the Lq query rows alone give Lq*G/128 items per kv-head).  A scheduling hint only — the selected rows
   // are device-side: rows ~ ratio_hint * N + Lq in selective mode.

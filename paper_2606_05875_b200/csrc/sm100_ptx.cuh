@@ -163,6 +163,51 @@ __device__ __forceinline__ float ex2_poly(float x) {
   return __uint_as_float(__float_as_uint(p) + (__float_as_uint(r) << 23));
 }
 
+// ------------------------------------------------------------------------------------------------ packed fp32x2 / bf16x2
+// sm_100 executes two fp32 FMAs / adds per instruction on register pairs (FFMA2 / FADD2): the softmax sweeps are issue-bound,
+// so halving the instruction count of the scale-and-subtract, the row sum and the polynomial is worth the pair plumbing.
+__device__ __forceinline__ uint64_t f2_pack(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint32_t bf16x2_max(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("max.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+// 2^x for a PAIR (x <= ~8 each) on the FMA pipe with packed ops: same Cody-Waite + cubic as ex2_poly
+__device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p_lo, float& p_hi) {
+  float x0, x1;
+  f2_unpack(x2, x0, x1);
+  x2 = f2_pack(fmaxf(x0, -125.f), fmaxf(x1, -125.f));
+  const uint64_t c = f2_pack(12582912.f, 12582912.f);
+  const uint64_t r2 = f2_add(x2, c);
+  const uint64_t n2 = f2_add(r2, f2_pack(-12582912.f, -12582912.f));
+  const uint64_t f2 = f2_fma(n2, f2_pack(-1.f, -1.f), x2);
+  uint64_t p2 = f2_fma(f2_pack(0.0551716685f, 0.0551716685f), f2, f2_pack(0.2426111251f, 0.2426111251f));
+  p2 = f2_fma(p2, f2, f2_pack(0.6932609677f, 0.6932609677f));
+  p2 = f2_fma(p2, f2, f2_pack(0.9999280572f, 0.9999280572f));
+  float q0, q1, r0, r1;
+  f2_unpack(p2, q0, q1);
+  f2_unpack(r2, r0, r1);
+  p_lo = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(r0) << 23));
+  p_hi = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(r1) << 23));
+}
+
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile(
