@@ -38,6 +38,14 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 #ifndef QCF_ATTN_MUFU_PAIRS
 #define QCF_ATTN_MUFU_PAIRS 4
 #endif
+// Measured dead ends on this kernel (all parity-green, all slower on c2; kept out of the code):
+//   * two threads per row (8 softmax warps, 32 key columns each, barrier.red agreement per tile): 82 -> 92 us, and a lone
+//     CTA's tile step went 0.80 -> 0.89 us: the step is not sweep-bound — one warp-wide EX2 takes 8 cycles on its SMSP
+//     (16/clk/SM), so the 64 exponentials of a row are ~512 cycles however the row is divided;
+//   * splitting every item's keys over 2 / 4 CTAs (cluster + DSMEM merge, or global partials merged by the last
+//     arriver): 107 -> 127 / 158 us — at c2 the SMs are throughput-bound, a split only adds prologues and merge traffic
+//     (it does pay when the grid under-fills the machine: rho = 0, 16 items: 82 -> 53 us, hence the heuristic below);
+//   * a persistent work-list kernel (recompute_attn_ptc.cu).
 // Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Measured on c2: 4 -> 84 us,
 // 3 -> 91 us, 2 -> 104 us: the sweep is issue-bound, not MUFU-bound, so every exponential goes to the MUFU.
 constexpr int kMufuPairs = QCF_ATTN_MUFU_PAIRS;
@@ -55,14 +63,14 @@ struct Smem {
   static constexpr int oK = oQ + kQ;
   static constexpr int oV = oK + kStages * kTile;
   static constexpr int oBar = oV + kStages * kTile;        // mbarriers (8 B each)
-  static constexpr int kNumBar = 4 * kStages + 6;
+  static constexpr int kNumBar = 4 * kStages + 7;
   static constexpr int oTmem = oBar + kNumBar * 8;
   static constexpr int oStat = oTmem + 16;                 // split-KV: (m, l) of this CTA's 128 rows
   static constexpr int kBytes = oStat + 2 * BM * 4;
   static_assert(2 * kStages * kTile >= BM * D * 4, "the K/V rings must hold one fp32 O tile for the split-KV merge");
 };
 enum { kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages, kSFull = 4 * kStages,
-       kPReady = 4 * kStages + 2, kODone = 4 * kStages + 4 };
+       kPReady = 4 * kStages + 2, kODone = 4 * kStages + 4, kQFull = 4 * kStages + 6 };
 
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
@@ -150,13 +158,17 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     if (lane == 0) {
       prefetch_tensormap(&tm_k);
       prefetch_tensormap(&tm_v);
-      for (int i = 0; i < S::kNumBar; ++i) mbar_init(bar(i), (i == kPReady || i == kPReady + 1) ? 128 : 1);
+      for (int i = 0; i < S::kNumBar; ++i) mbar_init(bar(i), (i == kPReady || i == kPReady + 1 || i == kQFull) ? 128 : 1);
       fence_barrier_init();
     }
   } else if (warp == 1) {
     tmem_alloc<kTmemCols>(sbase + S::oTmem);
-  } else {
-    // Q tile -> smem in the K-major 128B-swizzle layout: row r at r*128 in each 64-column block, chunk c at c ^ (r & 7)
+  }
+  // Q tile: the gathered rows are requested from global memory BEFORE the CTA-wide sync and land in shared memory after
+  // it, signalled on their own barrier, so the producer's first K / V TMA loads (issued right after the sync) and the
+  // TMEM allocation overlap the gather latency instead of queueing behind it.
+  uint4 qv[D / 8];
+  if (warp >= 2) {
     const int r = (warp & 3) * 32 + lane;
     const int pl = r / G, hl = r % G;
     const int ridx = ridx0 + pl;
@@ -166,16 +178,22 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
       src = reinterpret_cast<const uint4*>(q + ((static_cast<size_t>(b) * bd.t_stride + src_row) * hq + g * G + hl) * D);
     }
 #pragma unroll
-    for (int c = 0; c < D / 8; ++c) {
-      const uint4 v = src ? __ldg(src + c) : make_uint4(0u, 0u, 0u, 0u);
-      unsigned char* dst = smem + S::oQ + (c >> 3) * S::kQBlk + r * 128 + (((c & 7) ^ (r & 7)) << 4);
-      *reinterpret_cast<uint4*>(dst) = v;
-    }
-    fence_proxy_async_smem();
+    for (int c = 0; c < D / 8; ++c) qv[c] = src ? __ldg(src + c) : make_uint4(0u, 0u, 0u, 0u);
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  if (warp >= 2) {
+    // K-major 128B-swizzle layout: row r at r*128 in each 64-column block, chunk c at c ^ (r & 7)
+    const int r = (warp & 3) * 32 + lane;
+#pragma unroll
+    for (int c = 0; c < D / 8; ++c) {
+      unsigned char* dst = smem + S::oQ + (c >> 3) * S::kQBlk + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+      *reinterpret_cast<uint4*>(dst) = qv[c];
+    }
+    fence_proxy_async_smem();
+    mbar_arrive(bar(kQFull));
+  }
   const uint32_t tmem_base = *tmem_slot;
   const uint32_t tmem_o = tmem_base + kColO;
 
@@ -219,6 +237,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         umma_commit(bar(kEmptyK + st));
         umma_commit(bar(kSFull + (j & 1)));
       };
+      mbar_wait(bar(kQFull), 0);
+      tc_fence_after();
       if (n_kt > 0) issue_qk(0);
       for (int j = 0; j < n_kt; ++j) {
         if (j + 1 < n_kt) issue_qk(j + 1);

@@ -24,7 +24,7 @@ constexpr int BT = 128;            // rows of A, rows of one B tile, fp32 column
 constexpr int kThreads = 192;
 constexpr int kTmemCols = 256;
 constexpr float kLog2e = 1.4426950408889634f;
-constexpr float kRescaleThreshold = 8.0f;
+constexpr float kStaleSum = 1099511627776.0f;      // 2^40
 
 template <int D>
 struct Smem {
@@ -174,46 +174,83 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         const bool tail = key0 + BT > k_end;
         mbar_wait(bar(kSFull + st), (j >> 1) & 1);
         tc_fence_after();
-        float tile_max, tile_sum;
-        auto sweep = [&](float ref, bool with_sum) {
-          float mx0 = -INFINITY, mx1 = -INFINITY, l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+        // max of this row's scores over the tile's valid keys, log2 units (first tile and the rare rescale only)
+        auto tile_rowmax = [&]() -> float {
+          float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
           for (int c = 0; c < BT / 32; ++c) {
             uint32_t s[32];
             tmem_ld32(lane_addr + st * BT + c * 32, s);
             tmem_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 32; i += 4) {
+            for (int i = 0; i < 32; i += 2) {
               float v0 = __uint_as_float(s[i]), v1 = __uint_as_float(s[i + 1]);
-              float v2 = __uint_as_float(s[i + 2]), v3 = __uint_as_float(s[i + 3]);
               if (tail) {
                 const int k = key0 + c * 32 + i;
                 if (k >= k_end) v0 = -INFINITY;
                 if (k + 1 >= k_end) v1 = -INFINITY;
-                if (k + 2 >= k_end) v2 = -INFINITY;
-                if (k + 3 >= k_end) v3 = -INFINITY;
               }
-              mx0 = fmaxf(mx0, fmaxf(v0, v1)); mx1 = fmaxf(mx1, fmaxf(v2, v3));
-              if (with_sum) {
-                l0 += ex2(fmaf(v0, a.scale_log2, -ref)); l1 += ex2(fmaf(v1, a.scale_log2, -ref));
-                l2 += ex2(fmaf(v2, a.scale_log2, -ref)); l3 += ex2_poly(fmaf(v3, a.scale_log2, -ref));
-              }
+              mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1);
             }
           }
-          tile_max = fmaxf(mx0, mx1) * a.scale_log2;
-          tile_sum = (l0 + l1) + (l2 + l3);
+          return fmaxf(mx0, mx1) * a.scale_log2;
         };
+        // sum_k 2^(s_k * scale - ref) over the tile.  Issue-bound, so full tiles run on packed pairs (FFMA2 / FADD2) with
+        // every exponential on the MUFU; no per-element max: a stale reference shows up as a huge (or inf) sum.
+        auto sweep_sum = [&](float ref) -> float {
+          float total;
+          if (!tail) {
+            const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2), nr2 = f2_pack(-ref, -ref);
+            uint64_t la = 0ull, lb = 0ull;
+#pragma unroll
+            for (int c = 0; c < BT / 32; ++c) {
+              uint32_t s[32];
+              tmem_ld32(lane_addr + st * BT + c * 32, s);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; i += 4) {
+                float t0, t1, t2, t3;
+                f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i]), __uint_as_float(s[i + 1])), sc2, nr2), t0, t1);
+                f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i + 2]), __uint_as_float(s[i + 3])), sc2, nr2), t2, t3);
+                la = f2_add(la, f2_pack(ex2(t0), ex2(t1)));
+                lb = f2_add(lb, f2_pack(ex2(t2), ex2(t3)));
+              }
+            }
+            float s0, s1;
+            f2_unpack(f2_add(la, lb), s0, s1);
+            total = s0 + s1;
+          } else {
+            float l0 = 0.f, l1 = 0.f;
+#pragma unroll
+            for (int c = 0; c < BT / 32; ++c) {
+              uint32_t s[32];
+              tmem_ld32(lane_addr + st * BT + c * 32, s);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; i += 2) {
+                const int k = key0 + c * 32 + i;
+                const float v0 = k < k_end ? __uint_as_float(s[i]) : -INFINITY;
+                const float v1 = k + 1 < k_end ? __uint_as_float(s[i + 1]) : -INFINITY;
+                l0 += ex2(fmaf(v0, a.scale_log2, -ref));
+                l1 += ex2(fmaf(v1, a.scale_log2, -ref));
+              }
+            }
+            total = l0 + l1;
+          }
+          return total;
+        };
+        float tile_sum;
         if (j == 0) {
-          sweep(0.f, false);
-          m_ref = tile_max;                       // the first tile of a non-empty range has >= 1 valid key: finite
-          sweep(m_ref, true);
+          m_ref = tile_rowmax();                  // the first tile of a non-empty range has >= 1 valid key: finite
+          tile_sum = sweep_sum(m_ref);
         } else {
-          sweep(m_ref, true);
-          if (__any_sync(0xffffffffu, tile_max > m_ref + kRescaleThreshold)) {
-            const float m_t = fmaxf(m_ref, tile_max);
+          tile_sum = sweep_sum(m_ref);
+          // fp32 sums do not care how stale the reference is until they overflow: move it when a tile's sum passes 2^40
+          if (__any_sync(0xffffffffu, !(tile_sum <= kStaleSum))) {
+            const float m_t = fmaxf(m_ref, tile_rowmax());
             l *= ex2(m_ref - m_t);
             m_ref = m_t;
-            sweep(m_ref, true);
+            tile_sum = sweep_sum(m_ref);
           }
         }
         l += tile_sum;
@@ -228,14 +265,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
       }
     } else {
       // lane = key: sum over the streamed query rows of 2^(s * scale - lse_row)
-      float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
+      uint64_t acc01 = 0ull, acc23 = 0ull;               // packed fp32 pairs of partial column sums
       for (int j = 0; j < n_j; ++j) {
         const int st = j & 1;
         {
           // lse2 of this thread's row of the chunk: combine the pass-1 partials (log2 domain); overlaps the TMA / UMMA
           // latency of the chunk.  The slot was last read two chunks ago; the barrier of the chunk in between orders it.
           const int row = j * BT + r;
-          float lse = INFINITY;                              // rows past the end contribute 2^(-inf) = 0
+          float lse = INFINITY;                              // rows past the end contribute 2^(-inf) = 0 (stored negated)
           if (row < rows) {
             // partials are laid out [split][row]: for a fixed split the 128 threads read consecutive words
             const size_t o = static_cast<size_t>(b) * a.n_splits * a.stats_rows + static_cast<size_t>(g) * rows + row;
@@ -250,40 +287,56 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             }
             lse = M + log2f(L);
           }
-          s_lse[st * BT + r] = lse;
+          s_lse[st * BT + r] = -lse;
           asm volatile("bar.sync 1, 128;" ::: "memory");
         }
         mbar_wait(bar(kSFull + st), (j >> 1) & 1);
         tc_fence_after();
-        const float4* lse4 = reinterpret_cast<const float4*>(s_lse + st * BT);
+        const float4* lse4 = reinterpret_cast<const float4*>(s_lse + st * BT);      // holds -lse of the chunk's rows
         const int n_valid = rows - j * BT;                   // < BT only in the last chunk
+        if (n_valid >= BT) {
+          const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2);
 #pragma unroll
-        for (int c = 0; c < BT / 32; ++c) {
-          uint32_t s[32];
-          tmem_ld32(lane_addr + st * BT + c * 32, s);
-          tmem_wait_ld();
+          for (int c = 0; c < BT / 32; ++c) {
+            uint32_t s[32];
+            tmem_ld32(lane_addr + st * BT + c * 32, s);
+            tmem_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 32; i += 4) {
-            const float4 z = lse4[c * 8 + (i >> 2)];         // same address in every lane: broadcast
-            float p0 = ex2(fmaf(__uint_as_float(s[i]), a.scale_log2, -z.x));
-            float p1 = ex2(fmaf(__uint_as_float(s[i + 1]), a.scale_log2, -z.y));
-            float p2 = ex2(fmaf(__uint_as_float(s[i + 2]), a.scale_log2, -z.z));
-            float p3 = ex2_poly(fmaf(__uint_as_float(s[i + 3]), a.scale_log2, -z.w));
-            if (n_valid < BT) {                              // rows past the end hold whatever the buffer holds
-              const int col = c * 32 + i;
-              if (col >= n_valid) p0 = 0.f;
-              if (col + 1 >= n_valid) p1 = 0.f;
-              if (col + 2 >= n_valid) p2 = 0.f;
-              if (col + 3 >= n_valid) p3 = 0.f;
+            for (int i = 0; i < 32; i += 4) {
+              const float4 z = lse4[c * 8 + (i >> 2)];       // same address in every lane: broadcast
+              float t0, t1, t2, t3;
+              f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i]), __uint_as_float(s[i + 1])), sc2, f2_pack(z.x, z.y)), t0, t1);
+              f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i + 2]), __uint_as_float(s[i + 3])), sc2, f2_pack(z.z, z.w)), t2, t3);
+              acc01 = f2_add(acc01, f2_pack(ex2(t0), ex2(t1)));
+              acc23 = f2_add(acc23, f2_pack(ex2(t2), ex2(t3)));
             }
-            acc0 += p0; acc1 += p1; acc2 += p2; acc3 += p3;
+          }
+        } else {
+#pragma unroll
+          for (int c = 0; c < BT / 32; ++c) {
+            uint32_t s[32];
+            tmem_ld32(lane_addr + st * BT + c * 32, s);
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; i += 4) {
+              const float4 z = lse4[c * 8 + (i >> 2)];
+              const int col = c * 32 + i;                    // rows past the end hold whatever the buffer holds
+              const float p0 = col < n_valid ? ex2(fmaf(__uint_as_float(s[i]), a.scale_log2, z.x)) : 0.f;
+              const float p1 = col + 1 < n_valid ? ex2(fmaf(__uint_as_float(s[i + 1]), a.scale_log2, z.y)) : 0.f;
+              const float p2 = col + 2 < n_valid ? ex2(fmaf(__uint_as_float(s[i + 2]), a.scale_log2, z.z)) : 0.f;
+              const float p3 = col + 3 < n_valid ? ex2(fmaf(__uint_as_float(s[i + 3]), a.scale_log2, z.w)) : 0.f;
+              acc01 = f2_add(acc01, f2_pack(p0, p1));
+              acc23 = f2_add(acc23, f2_pack(p2, p3));
+            }
           }
         }
         tc_fence_before();
         mbar_arrive(bar(kSEmpty + st));
       }
       const int key = key_tile * BT + r;
-      if (key < N) a.part[(static_cast<size_t>(b) * a.hkv + g) * a.part_stride + key] = (acc0 + acc1) + (acc2 + acc3);
+      float a0, a1;
+      f2_unpack(f2_add(acc01, acc23), a0, a1);
+      if (key < N) a.part[(static_cast<size_t>(b) * a.hkv + g) * a.part_stride + key] = a0 + a1;
     }
   }
 
