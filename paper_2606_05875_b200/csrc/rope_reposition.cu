@@ -70,6 +70,15 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   __nv_bfloat16* kd = k_f + dst_row * row_elems;
   const bool identity = bd.chunk_rot[c] == 0;
   pdl_wait();                          // before the first pool read / cache write (descriptor reads above are constant)
+  // V rows of this work item (byte copy): the first sweep's loads are issued BEFORE the K section so that a thread has
+  // all of its bytes (K pairs + V vectors, 128 B at 8 x 128) in flight at once — at c2 the whole 21 MB input is then
+  // outstanding across the grid and the kernel is one HBM round trip plus the launch.
+  const uint4* vs = v_pool ? reinterpret_cast<const uint4*>(v_pool + src_row * row_elems) : nullptr;
+  const int n_vec = v_pool ? rows * (row_elems / 8) : 0;
+  uint4 tv[4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+    if (static_cast<int>(threadIdx.x + u * blockDim.x) < n_vec) tv[u] = ld_nc_v4(vs + threadIdx.x + u * blockDim.x);
   if (identity) {
     for (int r = rsub; r < rows; r += rows_per_pass) {
       const uint4 a = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0);
@@ -111,10 +120,11 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
 
   // ---- V: stitched in the same token order (byte copy); skipped for the K-only scoring prefetch
   if (v_pool == nullptr) return;
-  const uint4* vs = reinterpret_cast<const uint4*>(v_pool + src_row * row_elems);
   uint4* vd = reinterpret_cast<uint4*>(v_f + dst_row * row_elems);
-  const int n_vec = rows * (row_elems / 8);
-  for (int i = threadIdx.x; i < n_vec; i += blockDim.x * 4) {
+#pragma unroll
+  for (int u = 0; u < 4; ++u)
+    if (static_cast<int>(threadIdx.x + u * blockDim.x) < n_vec) st_na_v4(vd + threadIdx.x + u * blockDim.x, tv[u]);
+  for (int i = threadIdx.x + blockDim.x * 4; i < n_vec; i += blockDim.x * 4) {
     uint4 t[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u)

@@ -20,7 +20,8 @@ __device__ __forceinline__ uint32_t order_key(float f) {
 }
 
 __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float* __restrict__ scores, double ratio,
-                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel) {
+                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached) {
+  extern __shared__ uint32_t s_keys[];                           // order keys of the first n_cached scores
   __shared__ unsigned int hist[256];
   __shared__ unsigned int s_prefix, s_remaining;
   __shared__ unsigned int warp_cnt[32];                          // packed (gt << 16) | eq per warp
@@ -39,6 +40,12 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
     return;
   }
 
+  // the five sweeps below read every score; one coalesced global read fills shared memory, the rest stay on chip
+  const int n_sm_keys = min(N, n_cached);
+  for (int i = tid; i < n_sm_keys; i += kThreads) s_keys[i] = order_key(__ldcg(s + i));
+  auto key_of = [&](int i) -> uint32_t { return i < n_sm_keys ? s_keys[i] : order_key(__ldcg(s + i)); };
+  __syncthreads();
+
   // ---- radix select: after pass p the top 8(p+1) bits of the k-th largest key are known
   if (tid == 0) { s_prefix = 0u; s_remaining = static_cast<unsigned int>(k); }
 #pragma unroll 1
@@ -49,7 +56,8 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
     const uint32_t prefix = s_prefix;
     const uint32_t mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
     for (int i = tid; i < N; i += kThreads) {
-      const uint32_t key = order_key(__ldcg(s + i));
+      const uint32_t key = key_of(i);
+      // (warp-aggregating these atomics with match.any was measured: 12.6 -> 16.7 us on c2, 41 -> 63 us on c5)
       if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 0xffu], 1u);
     }
     __syncthreads();
@@ -89,7 +97,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
     const int i = base + tid;
     uint32_t key = 0u;
     const bool valid = i < N;
-    if (valid) key = order_key(__ldcg(s + i));
+    if (valid) key = key_of(i);
     const bool gt = valid && key > T, eq = valid && key == T;
     const unsigned int bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
     if (lane == 0) warp_cnt[warp] = (static_cast<unsigned int>(__popc(bg)) << 16) | static_cast<unsigned int>(__popc(be));
@@ -122,7 +130,15 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
 cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* scores, double ratio, int32_t* sel,
                         int32_t* n_sel, cudaStream_t stream) {
   if (b->batch == 0) return cudaSuccess;
-  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), 0, stream, b->dev, scores, ratio, sel, n_sel);
+  // up to 48 K keys (192 KB) are cached in shared memory; longer contexts read the remainder from L2
+  const int n_cached = b->n_stride < 49152 ? b->n_stride : 49152;
+  const size_t smem = static_cast<size_t>(n_cached) * sizeof(uint32_t);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
+    attr_set = true;
+  }
+  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached);
 }
 
 }  // namespace qcf
