@@ -35,7 +35,7 @@ KERNELS_PER_STEP = 6           # reposition, score_stats, score_colsum, topk, sc
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one attn_kernel launch on c2, from the ncu --set full capture
 # summarised in profiles/ (None until a capture of the current kernel is committed)
-A5_DRAM_TRAFFIC_BYTES = 34451712   # profiles/r01_c2_attn_tc_ncu.csv (read + write)
+A5_DRAM_TRAFFIC_BYTES = 34614784   # profiles/r01_c2_attn_tc_ncu.csv (34 429 184 read + 185 600 written)
 
 
 def parse_args():
@@ -319,7 +319,7 @@ def run_qcf(args) -> None:
     a5_ms = float(stage_ms[4])
     achieved = flops / (a5_ms * 1e-3) / 1e12
     peak = float(peaks["bf16_tflops"])
-    roofline = {"kernel": "attn_kernel (a5 recompute attention)", "bound": "tensor", "achieved": achieved,
+    roofline = {"kernel": "attn_tc_kernel (a5 recompute attention)", "bound": "tensor", "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": A5_DRAM_TRAFFIC_BYTES,
                 "peak_source": "%s bf16_tflops (burst: the kernel is timed alone between events in a sub-ms step)" % peak_kind,
                 "algorithmic_flops_per_launch": flops, "ms_per_launch": a5_ms}
