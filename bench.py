@@ -142,6 +142,15 @@ def config_dict(wl, args, l2: str) -> dict:
             "l2": l2}
 
 
+def max_over_ranks(values, dist, device) -> list:
+    """MAX over ranks of a list of floats (device timings): every rank contributes, every rank gets the result."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -296,10 +305,7 @@ def run_qcf(args) -> None:
     clocks = sampler.stop() if rank == 0 else None
 
     # ---- max over ranks
-    t = torch.tensor([total_ms, e2e[0] if e2e else 0.0, full_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_s, full_ms = float(t[0]), float(t[1]), float(t[2])
+    total_ms, e2e_s, full_ms = max_over_ranks([total_ms, e2e[0] if e2e else 0.0, full_ms], dist if world > 1 else None, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

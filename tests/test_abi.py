@@ -71,3 +71,39 @@ def test_create_fails_loudly_without_device_or_on_bad_layout(lib):
         assert st == binding.QCF_ERR_UNSUPPORTED and not h.value, "no CPU fallback: creation must fail without a GPU"
         with pytest.raises(binding.QcfError):
             binding.Context(8, 2, 128, 1e6, 1, 128, 8)
+
+
+def test_bench_reference_arm_under_two_gloo_ranks(tmp_path):
+    """The N > 1 launch contract on CPU: `torch.distributed.run` with two ranks (no GPU, gloo rendezvous on 127.0.0.1):
+    rank 0 alone runs the reference arm and prints ONE JSON line, the other rank exits 0 without work."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29731", os.path.join(root, "bench.py"), "--impl", "reference", "--workload", "c1", "--gpus", "2",
+           "--steps", "2", "--warmup", "1"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
+    assert d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_max_over_ranks_two_gloo_ranks():
+    """bench.py reduces its timings with a MAX over ranks; the same reduction on a 2-rank gloo group."""
+    import torch.multiprocessing as mp
+    mp.spawn(_gloo_worker, args=(2, 29733), nprocs=2, join=True)
+
+
+def _gloo_worker(rank, world, port):
+    import torch
+    import torch.distributed as dist
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    import bench
+    t = bench.max_over_ranks([10.0 + rank, 3.0 - rank], dist, "cpu")
+    assert t == [11.0, 3.0], t
+    dist.barrier()
+    dist.destroy_process_group()
