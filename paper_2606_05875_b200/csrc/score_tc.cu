@@ -25,6 +25,13 @@ constexpr int kThreads = 192;
 constexpr int kTmemCols = 256;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kStaleSum = 1099511627776.0f;      // 2^40
+#ifndef QCF_SCORE_MUFU_PAIRS
+#define QCF_SCORE_MUFU_PAIRS 3
+#endif
+// Of every 4 pairs, how many take MUFU.EX2 (the rest: the packed polynomial on the FMA pipe).  Unlike attention (no P V, no
+// P packing) these sweeps are MUFU-bound — 128 x 128 exponentials against a 256-cycle MMA per tile — so a quarter of them
+// moves to the FMA pipe: a2 on c4 600 -> 530 us, c5 295 -> 262 us, c2 30.8 -> 29.1 us (a half: 570 / 273 / 29.6).
+constexpr int kMufuPairs = QCF_SCORE_MUFU_PAIRS;
 
 template <int D>
 struct Smem {
@@ -208,12 +215,21 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
               tmem_ld32(lane_addr + st * BT + c * 32, s);
               tmem_wait_ld();
 #pragma unroll
-              for (int i = 0; i < 32; i += 4) {
-                float t0, t1, t2, t3;
-                f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i]), __uint_as_float(s[i + 1])), sc2, nr2), t0, t1);
-                f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i + 2]), __uint_as_float(s[i + 3])), sc2, nr2), t2, t3);
-                la = f2_add(la, f2_pack(ex2(t0), ex2(t1)));
-                lb = f2_add(lb, f2_pack(ex2(t2), ex2(t3)));
+              for (int i = 0; i < 32; i += 8) {
+                float p[8];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                  const uint64_t t = f2_fma(f2_pack(__uint_as_float(s[i + 2 * q]), __uint_as_float(s[i + 2 * q + 1])), sc2, nr2);
+                  if (q < kMufuPairs) {
+                    float t0, t1;
+                    f2_unpack(t, t0, t1);
+                    p[2 * q] = ex2(t0); p[2 * q + 1] = ex2(t1);
+                  } else {
+                    ex2_poly2(t, p[2 * q], p[2 * q + 1]);
+                  }
+                }
+                la = f2_add(la, f2_add(f2_pack(p[0], p[1]), f2_pack(p[2], p[3])));
+                lb = f2_add(lb, f2_add(f2_pack(p[4], p[5]), f2_pack(p[6], p[7])));
               }
             }
             float s0, s1;
@@ -302,13 +318,23 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             tmem_ld32(lane_addr + st * BT + c * 32, s);
             tmem_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 32; i += 4) {
-              const float4 z = lse4[c * 8 + (i >> 2)];       // same address in every lane: broadcast
-              float t0, t1, t2, t3;
-              f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i]), __uint_as_float(s[i + 1])), sc2, f2_pack(z.x, z.y)), t0, t1);
-              f2_unpack(f2_fma(f2_pack(__uint_as_float(s[i + 2]), __uint_as_float(s[i + 3])), sc2, f2_pack(z.z, z.w)), t2, t3);
-              acc01 = f2_add(acc01, f2_pack(ex2(t0), ex2(t1)));
-              acc23 = f2_add(acc23, f2_pack(ex2(t2), ex2(t3)));
+            for (int i = 0; i < 32; i += 8) {
+              const float4 za = lse4[c * 8 + (i >> 2)], zb = lse4[c * 8 + (i >> 2) + 1];   // same address in every lane: broadcast
+              const uint64_t nz[4] = {f2_pack(za.x, za.y), f2_pack(za.z, za.w), f2_pack(zb.x, zb.y), f2_pack(zb.z, zb.w)};
+              float p[8];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                const uint64_t t = f2_fma(f2_pack(__uint_as_float(s[i + 2 * q]), __uint_as_float(s[i + 2 * q + 1])), sc2, nz[q]);
+                if (q < kMufuPairs) {
+                  float t0, t1;
+                  f2_unpack(t, t0, t1);
+                  p[2 * q] = ex2(t0); p[2 * q + 1] = ex2(t1);
+                } else {
+                  ex2_poly2(t, p[2 * q], p[2 * q + 1]);
+                }
+              }
+              acc01 = f2_add(acc01, f2_add(f2_pack(p[0], p[1]), f2_pack(p[2], p[3])));
+              acc23 = f2_add(acc23, f2_add(f2_pack(p[4], p[5]), f2_pack(p[6], p[7])));
             }
           }
         } else {
