@@ -49,7 +49,8 @@ typedef struct qcf_batch qcf_batch;   /* opaque: device-resident description of 
 typedef enum {
   QCF_OK = 0,
   QCF_ERR_INVALID_ARG = 1,  /* null pointer, negative size, ratio outside [0,1], mis-ordered offsets     */
-  QCF_ERR_UNSUPPORTED = 2,  /* head_dim not in {64,128}, Hq % Hkv != 0, G not in {1,2,4,8,16}, no sm_100 */
+  QCF_ERR_UNSUPPORTED = 2,  /* head_dim not in {64,128}, Hq % Hkv != 0, G not in {1,2,4,8,16}, max_query*G > 8192,
+                               no sm_100 device                                                          */
   QCF_ERR_WORKSPACE = 3,    /* batch exceeds the limits given to qcf_create                              */
   QCF_ERR_CUDA = 4          /* a CUDA runtime call failed; message holds cudaGetErrorString              */
 } qcf_status;

@@ -103,6 +103,8 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
     return fail(nullptr, QCF_ERR_UNSUPPORTED, "group size Hq/Hkv must be 1, 2, 4, 8 or 16");
   if (lay->n_kv_heads * lay->head_dim > 8192)
     return fail(nullptr, QCF_ERR_UNSUPPORTED, "Hkv * head_dim must be <= 8192");
+  if (static_cast<long long>(max_query) * g > 8192)
+    return fail(nullptr, QCF_ERR_UNSUPPORTED, "max_query * (Hq / Hkv) must be <= 8192 (query rows per kv-head kept in shared memory by qcf_score)");
   if (!(lay->rope_theta > 1.0f)) return fail(nullptr, QCF_ERR_INVALID_ARG, "rope_theta must be > 1");
   if (!(lay->softmax_scale >= 0.0f)) return fail(nullptr, QCF_ERR_INVALID_ARG, "softmax_scale must be >= 0");
 

@@ -11,6 +11,8 @@
 // threads that sweep their own TMEM lane.  GQA packing: a "query row" is (token i, head hl) of one kv-head,
 // r = i * G + hl, loaded by TMA boxes {64 elements, G heads, 128/G tokens}.  The Hkv per-head partial column sums are
 // combined in fixed order by the last CTA of each key tile (bit-reproducible scores, deterministic top-k).
+#include <cmath>
+
 #include "qcf_internal.cuh"
 #include "sm100_ptx.cuh"
 
@@ -39,18 +41,19 @@ struct Smem {
   static constexpr int kTile = BT * D * 2;
   static constexpr int oA = 0;
   static constexpr int oB = kTile;
-  static constexpr int oLse = oB + 2 * kTile;           // pass 2: lse of the 128 streamed query rows, double-buffered
-  static constexpr int oBar = oLse + 2 * BT * 4;
-  static constexpr int kNumBar = 9;
+  static constexpr int oBar = oB + 2 * kTile;
+  static constexpr int kNumBar = 10;
   static constexpr int oTmem = oBar + kNumBar * 8;
   static constexpr int oFlag = oTmem + 8;
-  static constexpr int kBytes = oFlag + 8;
+  static constexpr int oLse = oFlag + 8;                // pass 2: -lse of ALL query rows of the (request, kv-head), size set at launch
+  static constexpr int kBytes = oLse;
 };
-enum { kAFull = 0, kBFull = 1, kBEmpty = 3, kSFull = 5, kSEmpty = 7 };
+enum { kAFull = 0, kBFull = 1, kBEmpty = 3, kSFull = 5, kSEmpty = 7, kAEmpty = 9 };
 
 struct ScoreArgs {
   float scale_log2;
   int hq, hkv, n_splits;
+  int kt_per_cta;                                        // pass 2: key tiles walked by one CTA
   float* stats_m; float* stats_l; int stats_rows;        // [B][n_splits][stats_rows]
   float* part; int part_stride;                          // [B][Hkv][part_stride]
   unsigned int* counters;
@@ -73,11 +76,11 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   if (PASS == 1) {
     split = blockIdx.x; row_tile = blockIdx.y; g = blockIdx.z % a.hkv; b = blockIdx.z / a.hkv;
   } else {
-    key_tile = blockIdx.x; g = blockIdx.y; b = blockIdx.z;
+    key_tile = blockIdx.x * a.kt_per_cta; g = blockIdx.y; b = blockIdx.z;       // first key tile of this CTA
   }
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
   const int rows = Lq * G;
-  int k_begin = 0, k_end = 0, n_j = 0;
+  int k_begin = 0, k_end = 0, n_j = 0, n_kt = 1;          // n_kt: A tiles this CTA walks (pass 2: key tiles)
   if (PASS == 1) {
     if (row_tile * BT >= rows) return;
     const int span = (((N + a.n_splits - 1) / a.n_splits + BT - 1) / BT) * BT;
@@ -85,7 +88,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     k_end = min(N, k_begin + span);
     n_j = k_end > k_begin ? (k_end - k_begin + BT - 1) / BT : 0;
   } else {
-    if (key_tile * BT >= N) return;
+    n_kt = min(a.kt_per_cta, (N + BT - 1) / BT - key_tile);
+    if (n_kt <= 0) return;
     n_j = (rows + BT - 1) / BT;
   }
 
@@ -100,6 +104,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
       prefetch_tensormap(&tm_q);
       prefetch_tensormap(&tm_k);
       mbar_init(bar(kAFull), 1);
+      mbar_init(bar(kAEmpty), 1);
       for (int i = 0; i < 2; ++i) {
         mbar_init(bar(kBFull + i), 1);
         mbar_init(bar(kBEmpty + i), 1);
@@ -131,17 +136,17 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   if (warp == 0) {
     // ===================================================================== producer
     if (n_j > 0 && lane == 0) {
-      mbar_arrive_expect_tx(bar(kAFull), S::kTile);
-      if (PASS == 1) load_q_tile(sA, bar(kAFull), row_tile); else load_k_tile(sA, bar(kAFull), key_tile * BT);
-    }
-    for (int j = 0; j < n_j; ++j) {
-      const int st = j & 1;
-      const uint32_t ph = (j >> 1) & 1;
-      if (lane == 0) {
-        mbar_wait(bar(kBEmpty + st), ph ^ 1);
-        mbar_arrive_expect_tx(bar(kBFull + st), S::kTile);
-        if (PASS == 1) load_k_tile(sB + st * S::kTile, bar(kBFull + st), k_begin + j * BT);
-        else load_q_tile(sB + st * S::kTile, bar(kBFull + st), j);
+      for (int kt = 0, it = 0; kt < n_kt; ++kt) {
+        if (kt > 0) mbar_wait(bar(kAEmpty), (kt - 1) & 1);      // every MMA that read the previous A tile has completed
+        mbar_arrive_expect_tx(bar(kAFull), S::kTile);
+        if (PASS == 1) load_q_tile(sA, bar(kAFull), row_tile); else load_k_tile(sA, bar(kAFull), (key_tile + kt) * BT);
+        for (int j = 0; j < n_j; ++j, ++it) {
+          const int st = it & 1;
+          mbar_wait(bar(kBEmpty + st), ((it >> 1) & 1) ^ 1);
+          mbar_arrive_expect_tx(bar(kBFull + st), S::kTile);
+          if (PASS == 1) load_k_tile(sB + st * S::kTile, bar(kBFull + st), k_begin + j * BT);
+          else load_q_tile(sB + st * S::kTile, bar(kBFull + st), j);
+        }
       }
     }
     __syncwarp();
@@ -149,21 +154,24 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     // ===================================================================== UMMA issuer
     if (lane == 0 && n_j > 0) {
       constexpr uint32_t idesc = umma_idesc_bf16(BT, BT, false, false);
-      mbar_wait(bar(kAFull), 0);
-      for (int j = 0; j < n_j; ++j) {
-        const int st = j & 1;
-        const uint32_t ph = (j >> 1) & 1;
-        mbar_wait(bar(kSEmpty + st), ph ^ 1);               // consumers have released S_{j-2}
-        mbar_wait(bar(kBFull + st), ph);
-        tc_fence_after();
+      for (int kt = 0, it = 0; kt < n_kt; ++kt) {
+        mbar_wait(bar(kAFull), kt & 1);
+        for (int j = 0; j < n_j; ++j, ++it) {
+          const int st = it & 1;
+          const uint32_t ph = (it >> 1) & 1;
+          mbar_wait(bar(kSEmpty + st), ph ^ 1);               // consumers have released the S buffer used two steps ago
+          mbar_wait(bar(kBFull + st), ph);
+          tc_fence_after();
 #pragma unroll
-        for (int ks = 0; ks < D / 16; ++ks) {
-          const uint32_t koff = (ks >> 2) * S::kBlk + (ks & 3) * 32;
-          umma_ss(tmem_base + st * BT, umma_smem_desc_sw128(sA + koff, 16, 1024),
-                  umma_smem_desc_sw128(sB + st * S::kTile + koff, 16, 1024), idesc, ks > 0 ? 1u : 0u);
+          for (int ks = 0; ks < D / 16; ++ks) {
+            const uint32_t koff = (ks >> 2) * S::kBlk + (ks & 3) * 32;
+            umma_ss(tmem_base + st * BT, umma_smem_desc_sw128(sA + koff, 16, 1024),
+                    umma_smem_desc_sw128(sB + st * S::kTile + koff, 16, 1024), idesc, ks > 0 ? 1u : 0u);
+          }
+          umma_commit(bar(kBEmpty + st));
+          umma_commit(bar(kSFull + st));
         }
-        umma_commit(bar(kBEmpty + st));
-        umma_commit(bar(kSFull + st));
+        umma_commit(bar(kAEmpty));
       }
     }
     __syncwarp();
@@ -210,10 +218,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2), nr2 = f2_pack(-ref, -ref);
             uint64_t la = 0ull, lb = 0ull;
 #pragma unroll
+            uint32_t sa[32], sb[32];                   // chunk c + 1 is in flight while chunk c is processed
+            tmem_ld32(lane_addr + st * BT, sa);
+#pragma unroll
             for (int c = 0; c < BT / 32; ++c) {
-              uint32_t s[32];
-              tmem_ld32(lane_addr + st * BT + c * 32, s);
+              uint32_t(&s)[32] = (c & 1) ? sb : sa;
               tmem_wait_ld();
+              if (c + 1 < BT / 32) tmem_ld32(lane_addr + st * BT + (c + 1) * 32, (c & 1) ? sa : sb);
 #pragma unroll
               for (int i = 0; i < 32; i += 8) {
                 float p[8];
@@ -280,43 +291,48 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         a.stats_l[o] = l;
       }
     } else {
-      // lane = key: sum over the streamed query rows of 2^(s * scale - lse_row)
-      uint64_t acc01 = 0ull, acc23 = 0ull;               // packed fp32 pairs of partial column sums
-      for (int j = 0; j < n_j; ++j) {
-        const int st = j & 1;
-        {
-          // lse2 of this thread's row of the chunk: combine the pass-1 partials (log2 domain); overlaps the TMA / UMMA
-          // latency of the chunk.  The slot was last read two chunks ago; the barrier of the chunk in between orders it.
-          const int row = j * BT + r;
-          float lse = INFINITY;                              // rows past the end contribute 2^(-inf) = 0 (stored negated)
-          if (row < rows) {
-            // partials are laid out [split][row]: for a fixed split the 128 threads read consecutive words
-            const size_t o = static_cast<size_t>(b) * a.n_splits * a.stats_rows + static_cast<size_t>(g) * rows + row;
-            float M = -INFINITY, L = 0.f;
+      // lane = key: sum over the streamed query rows of 2^(s * scale - lse_row).  The CTA walks n_kt key tiles of one
+      // (request, kv-head); -lse of every query row is combined from the pass-1 partials ONCE (log2 domain) and kept
+      // in shared memory.
+      for (int row = r; row < n_j * BT; row += BT) {
+        float lse = INFINITY;                                // rows past the end contribute 2^(-inf) = 0
+        if (row < rows) {
+          // partials are laid out [split][row]: for a fixed split the 128 threads read consecutive words
+          const size_t o = static_cast<size_t>(b) * a.n_splits * a.stats_rows + static_cast<size_t>(g) * rows + row;
+          float M = -INFINITY, L = 0.f;
 #pragma unroll 8
-            for (int sidx = 0; sidx < a.n_splits; ++sidx) {
-              const float m_s = __ldcg(a.stats_m + o + static_cast<size_t>(sidx) * a.stats_rows);
-              const float l_s = __ldcg(a.stats_l + o + static_cast<size_t>(sidx) * a.stats_rows);
-              const float Mn = fmaxf(M, m_s);
-              if (Mn > -INFINITY) L = L * ex2(M - Mn) + l_s * ex2(m_s - Mn);
-              M = Mn;
-            }
-            lse = M + log2f(L);
+          for (int sidx = 0; sidx < a.n_splits; ++sidx) {
+            const float m_s = __ldcg(a.stats_m + o + static_cast<size_t>(sidx) * a.stats_rows);
+            const float l_s = __ldcg(a.stats_l + o + static_cast<size_t>(sidx) * a.stats_rows);
+            const float Mn = fmaxf(M, m_s);
+            if (Mn > -INFINITY) L = L * ex2(M - Mn) + l_s * ex2(m_s - Mn);
+            M = Mn;
           }
-          s_lse[st * BT + r] = -lse;
-          asm volatile("bar.sync 1, 128;" ::: "memory");
+          lse = M + log2f(L);
         }
-        mbar_wait(bar(kSFull + st), (j >> 1) & 1);
+        s_lse[row] = -lse;
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      volatile int* s_last = reinterpret_cast<volatile int*>(smem + S::oFlag);
+      const int n_tiles_b = (bd.n_stride + BT - 1) / BT;
+      for (int kt = 0, it = 0; kt < n_kt; ++kt) {
+      uint64_t acc01 = 0ull, acc23 = 0ull;               // packed fp32 pairs of partial column sums
+      for (int j = 0; j < n_j; ++j, ++it) {
+        const int st = it & 1;
+        mbar_wait(bar(kSFull + st), (it >> 1) & 1);
         tc_fence_after();
-        const float4* lse4 = reinterpret_cast<const float4*>(s_lse + st * BT);      // holds -lse of the chunk's rows
+        const float4* lse4 = reinterpret_cast<const float4*>(s_lse + j * BT);       // -lse of the chunk's rows
         const int n_valid = rows - j * BT;                   // < BT only in the last chunk
         if (n_valid >= BT) {
           const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2);
 #pragma unroll
+          uint32_t sa[32], sb[32];                     // chunk c + 1 is in flight while chunk c is processed
+          tmem_ld32(lane_addr + st * BT, sa);
+#pragma unroll
           for (int c = 0; c < BT / 32; ++c) {
-            uint32_t s[32];
-            tmem_ld32(lane_addr + st * BT + c * 32, s);
+            uint32_t(&s)[32] = (c & 1) ? sb : sa;
             tmem_wait_ld();
+            if (c + 1 < BT / 32) tmem_ld32(lane_addr + st * BT + (c + 1) * 32, (c & 1) ? sa : sb);
 #pragma unroll
             for (int i = 0; i < 32; i += 8) {
               const float4 za = lse4[c * 8 + (i >> 2)], zb = lse4[c * 8 + (i >> 2) + 1];   // same address in every lane: broadcast
@@ -359,35 +375,33 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         tc_fence_before();
         mbar_arrive(bar(kSEmpty + st));
       }
-      const int key = key_tile * BT + r;
+      const int kt_abs = key_tile + kt;
+      const int key = kt_abs * BT + r;
       float a0, a1;
       f2_unpack(f2_add(acc01, acc23), a0, a1);
       if (key < N) a.part[(static_cast<size_t>(b) * a.hkv + g) * a.part_stride + key] = a0 + a1;
+      // last CTA of this key tile sums the Hkv partials in fixed order (deterministic)
+      __threadfence();
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      unsigned int* ctr = a.counters + static_cast<size_t>(b) * n_tiles_b + kt_abs;
+      if (r == 0) *s_last = (atomicAdd(ctr, 1u) == static_cast<unsigned int>(a.hkv - 1));
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      if (*s_last) {
+        __threadfence();
+        if (key < N) {
+          float sum = 0.f;
+          for (int gg = 0; gg < a.hkv; ++gg) sum += __ldcg(a.part + (static_cast<size_t>(b) * a.hkv + gg) * a.part_stride + key);
+          const float v = rows > 0 ? sum / static_cast<float>(a.hq * Lq) : 0.f;
+          float* dst = a.scores + static_cast<size_t>(b) * bd.n_stride + key;
+          *dst = a.accumulate ? *dst + v : v;
+        }
+        if (r == 0) *ctr = 0u;
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");           // s_last is rewritten by the next key tile
+      }   // key tiles
     }
   }
 
-  if (PASS == 2) {
-    // last CTA of this key tile sums the Hkv partials in fixed order (deterministic)
-    volatile int* s_last = reinterpret_cast<volatile int*>(smem + S::oFlag);
-    __threadfence();
-    __syncthreads();
-    const int n_tiles_b = (bd.n_stride + BT - 1) / BT;
-    unsigned int* ctr = a.counters + static_cast<size_t>(b) * n_tiles_b + key_tile;
-    if (threadIdx.x == 0) *s_last = (atomicAdd(ctr, 1u) == static_cast<unsigned int>(a.hkv - 1));
-    __syncthreads();
-    if (*s_last) {
-      __threadfence();
-      const int key = key_tile * BT + static_cast<int>(threadIdx.x);
-      if (threadIdx.x < BT && key < N) {
-        float sum = 0.f;
-        for (int gg = 0; gg < a.hkv; ++gg) sum += __ldcg(a.part + (static_cast<size_t>(b) * a.hkv + gg) * a.part_stride + key);
-        const float v = rows > 0 ? sum / static_cast<float>(a.hq * Lq) : 0.f;
-        float* dst = a.scores + static_cast<size_t>(b) * bd.n_stride + key;
-        *dst = a.accumulate ? *dst + v : v;
-      }
-      if (threadIdx.x == 0) *ctr = 0u;
-    }
-  }
   tc_fence_before();
   __syncthreads();
   if (warp == 1) {
@@ -428,16 +442,18 @@ bool make_map(CUtensorMap* m, const void* base, int batch, int t_stride, int hea
 template <int D>
 cudaError_t launch(const qcf_ctx* ctx, const qcf_batch* b, const CUtensorMap& tm_q, const CUtensorMap& tm_k,
                    ScoreArgs a, int row_tiles, int key_tiles, cudaStream_t stream) {
-  const int smem = Smem<D>::kBytes + 1024;
+  const int smem1 = Smem<D>::kBytes + 1024;
+  const int smem = smem1 + row_tiles * BT * 4;          // pass 2 keeps -lse of every query row of a (request, kv-head)
   if (row_tiles > 0) {
     auto k1 = score_tc_kernel<D, 1>;
-    cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaError_t e = launch_pdl(ctx->pdl, k1, dim3(a.n_splits, row_tiles, b->batch * a.hkv), dim3(kThreads), smem, stream, tm_q, tm_k, b->dev, a);
+    cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, smem1);
+    cudaError_t e = launch_pdl(ctx->pdl, k1, dim3(a.n_splits, row_tiles, b->batch * a.hkv), dim3(kThreads), smem1, stream, tm_q, tm_k, b->dev, a);
     if (e != cudaSuccess) return e;
   }
   auto k2 = score_tc_kernel<D, 2>;
   cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-  return launch_pdl(ctx->pdl, k2, dim3(key_tiles, a.hkv, b->batch), dim3(kThreads), smem, stream, tm_q, tm_k, b->dev, a);
+  const int groups = (key_tiles + a.kt_per_cta - 1) / a.kt_per_cta;
+  return launch_pdl(ctx->pdl, k2, dim3(groups, a.hkv, b->batch), dim3(kThreads), smem, stream, tm_q, tm_k, b->dev, a);
 }
 
 }  // namespace
@@ -449,14 +465,37 @@ cudaError_t launch_score_tc(const qcf_ctx* ctx, const qcf_batch* b, const __nv_b
   const int max_rows = b->max_query * L.g;
   const int row_tiles = (max_rows + BT - 1) / BT;
   const int key_tiles = (b->max_ctx + BT - 1) / BT;
-  // enough key splits in pass 1 to fill the machine twice, at least one 128-key tile each
+  if (row_tiles * BT * 4 > 32768) return cudaErrorInvalidValue;       // Lq * G <= 8192 query rows per kv-head (checked at qcf_create)
+  const int slots = 2 * ctx->n_sm;                                     // resident CTAs (2 per SM)
+  // pass 1: key splits.  Few CTAs: split until one resident wave is full.  More than a wave: the split count (<= 8) with
+  // the best wave efficiency (512 CTAs on 296 slots is 2 waves at 86 %; 4 splits make it 7 waves at 99 %).
   int n_splits = 1;
   if (row_tiles > 0) {
     const int ctas = row_tiles * L.hkv * b->batch;
-    n_splits = (2 * ctx->n_sm) / ctas;            // one resident wave (2 CTAs per SM)
+    if (ctas <= slots) {
+      n_splits = slots / ctas;
+    } else {
+      double best = 0.0;
+      for (int sp = 1; sp <= 8; ++sp) {
+        const double w = static_cast<double>(ctas) * sp / slots;
+        const double eff = w / std::ceil(w);
+        if (eff > best + 0.02) { best = eff; n_splits = sp; }
+      }
+    }
     if (n_splits > key_tiles) n_splits = key_tiles;
     if (n_splits > kScoreSplitsMax) n_splits = kScoreSplitsMax;
     if (n_splits < 1) n_splits = 1;
+  }
+  // pass 2: key tiles per CTA.  A CTA per key tile is 4 tile steps under a full prologue at c4 (8192 CTAs): walk several.
+  // Small problems: one resident wave; large ones: at most three waves' worth of CTAs.
+  int kt_per_cta = 1;
+  {
+    const int pairs = L.hkv * b->batch;
+    const int items = pairs * key_tiles;
+    const int budget = items <= 3 * slots ? slots : 3 * slots;
+    int per_pair = budget / pairs;
+    if (per_pair < 1) per_pair = 1;
+    kt_per_cta = (key_tiles + per_pair - 1) / per_pair;
   }
   CUtensorMap tm_q, tm_k;
   // q_probe may be NULL when no request has query tokens: map a valid dummy address (never dereferenced: n_j == 0)
@@ -466,7 +505,7 @@ cudaError_t launch_score_tc(const qcf_ctx* ctx, const qcf_batch* b, const __nv_b
     return cudaErrorInvalidValue;
   ScoreArgs a;
   a.scale_log2 = L.scale * kLog2e;
-  a.hq = L.hq; a.hkv = L.hkv; a.n_splits = n_splits;
+  a.hq = L.hq; a.hkv = L.hkv; a.n_splits = n_splits; a.kt_per_cta = kt_per_cta;
   a.stats_m = ctx->stats_m; a.stats_l = ctx->stats_l; a.stats_rows = L.hq * ctx->max_query;
   a.part = ctx->score_part; a.part_stride = ctx->max_ctx;
   a.counters = ctx->counters;
