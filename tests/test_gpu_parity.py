@@ -449,6 +449,9 @@ def test_error_reporting():
     assert e.value.status == binding.QCF_ERR_UNSUPPORTED
     with pytest.raises(binding.QcfError):
         binding.Context(8, 2, 96, 1e6, 1, 128, 8)
+    with pytest.raises(binding.QcfError) as e:
+        binding.Context(64, 8, 128, 1e6, 1, 128, 2048)   # 2048 * 8 query rows per kv-head > 8192
+    assert e.value.status == binding.QCF_ERR_UNSUPPORTED
     ctx = binding.Context(8, 2, 128, 1e6, 1, 128, 8)
     with pytest.raises(binding.QcfError) as e:
         ctx.batch([[200]], [[0]], [4])                   # exceeds max_ctx
