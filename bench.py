@@ -415,6 +415,7 @@ def run_c3(args) -> None:
     def use(pools):
         run.k_pic, run.v_pic, run.k_anchor, run.v_anchor = pools
 
+    kv_row_b = sp.n_kv_heads * sp.head_dim * 2
     warm = max(args.warmup, 3)
     use(dev_pools)
     fuse_ms = timed(lambda: run.fuse(True), args.steps, warm)
@@ -424,6 +425,20 @@ def run_c3(args) -> None:
     t1 = time.perf_counter()
     e2e_ms = timed(lambda: (run.fuse(True), run.hidden[-sp.n_query:].cpu(), run.sel.cpu()), n_e2e, 2)
     e2e_serial_ms = timed(lambda: (run.fuse(False), run.hidden[-sp.n_query:].cpu(), run.sel.cpu()), max(3, min(args.steps, 5)), 1)
+    # selector views on the same kernels: stage 1 alone and the whole pipeline, pools in pinned host
+    # memory (the paper's setting: selection-time data movement is what the compressed view saves)
+    selectors = {}
+    for view in ("qcfuse", "fullview", "final"):
+        use([host_k, host_v, host_ak, host_av])
+        run.use_selector(view)
+        s1 = timed(lambda: run.fuse(True, stages=1), 5, 2)
+        tot = timed(lambda: run.fuse(True), 5, 1)
+        l_pr = max(run.crit) + 1
+        selectors[view] = {"stage1_ms": float(s1.mean()), "pipeline_ms": float(tot.mean()), "probe_layers": l_pr,
+                           "scored_layers": len(run.crit), "anchor_rows": run.anchor_rows,
+                           "stage1_h2d_bytes": int(2 * kv_row_b * (run.anchor_rows * l_pr + sp.n_ctx * len(run.crit)))}
+    use([host_k, host_v, host_ak, host_av])
+    run.use_selector("qcfuse")
     kc = [torch.zeros_like(k) for k in run.k_fused]
     vc = [torch.zeros_like(k) for k in run.k_fused]
     full_ms = timed(lambda: run.full_prefill(kc, vc), max(3, min(args.steps, 10)), 2)
@@ -463,7 +478,7 @@ def run_c3(args) -> None:
                      "speedup_over_full_prefill": float(full_ms.mean()) / t_fuse,
                      "whole_pipeline_TFLOPps": ach, "whole_pipeline_frac_tensor_peak": ach / peak,
                      "full_prefill_TFLOPps": (fl["gemm_full"] + fl["attn_full"]) / (float(full_ms.mean()) * 1e-3) / 1e12,
-                     "phase1_build_s": phase1_s},
+                     "phase1_build_s": phase1_s, "selectors_pinned_host": selectors},
         "e2e": {"value": sp.n_ctx / (float(e2e_ms.mean()) * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(sp.n_query * sp.hidden * 2 + sp.n_ctx * 4), "ms_per_step": float(e2e_ms.mean()),
                 "ms_per_step_serial_loader": float(e2e_serial_ms.mean()),

@@ -308,7 +308,10 @@ QCF_API qcf_status qcf_stack_layer(qcf_stack* s, int32_t layer, const qcf_batch*
  *            (Eq. 17); for l in L*: load PIC pool l, stitch (a1), score (a2, Eq. 18/20); then top-k (a3, Eq. 11)
  *   stage 2  for every layer: load PIC pool l+1.. and stitch them on a second stream WHILE layer l recomputes the
  *            rows R on `stream` (a8: PAPER.md:23, 341-342), a4 + a5 + a7 per layer
- * Pools may live in pinned host memory (the paper's setting) or on the device (cudaMemcpyDefault). */
+ * Pools may live in pinned host memory (the paper's setting) or on the device (cudaMemcpyDefault).
+ * The compressed view is an argument, not a mode: anchor pools = the PIC pools with a probe batch that lists whole chunks
+ * and crit_layers = every layer gives full-view (ProphetKV-style) selection (Eq. 9-11); an empty anchor
+ * pool with crit_layers = {L-1} gives query-only final-layer selection. */
 typedef struct {
   const void* const* k_pic;      /* host array [L] of pointers to [pool_rows][Hkv][d] bf16 PIC pools              */
   const void* const* v_pic;
@@ -327,6 +330,8 @@ typedef struct {
   int32_t* n_sel;                /* dev [1]                                                                         */
   void* hidden_out;              /* dev [n_R][hidden] out: final hidden states of the rows R (P ascending, then U)  */
   int32_t overlap;               /* != 0: layer-ahead loading on a second stream (a8); 0: serial, for the ablation  */
+  int32_t stages;                /* 0 or 3: both stages; 1: stage 1 only (scores, sel, n_sel are produced, no layer is
+                                    recomputed); 2: stage 2 only (sel / n_sel are INPUTS, e.g. from another selector)   */
 } qcf_fuse_args;
 QCF_API qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* main_batch, const qcf_batch* probe_batch,
                                   const qcf_fuse_args* args, void* stream);

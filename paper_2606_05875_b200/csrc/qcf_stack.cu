@@ -257,6 +257,8 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
   STK_REQUIRE(ctx, n_rows <= s->max_rows && Lq <= s->max_rows && N + Lq <= s->max_pos,
               "qcf_stack_fuse: request exceeds max_rows / max_pos of qcf_stack_create");
   const int l_max = a->crit_layers[a->n_crit - 1];
+  STK_REQUIRE(ctx, a->stages >= 0 && a->stages <= 3, "qcf_stack_fuse: stages must be 0..3");
+  const bool do1 = a->stages == 0 || (a->stages & 1), do2 = a->stages == 0 || (a->stages & 2);
   cudaStream_t cs = static_cast<cudaStream_t>(stream);
   cudaStream_t ls = a->overlap ? s->loader : cs;
   const size_t kv_row = static_cast<size_t>(L.hkv) * L.d * 2;
@@ -297,6 +299,7 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
     if (is_crit(l)) if (qcf_status e = load_pic(l)) return e;
     return QCF_OK;
   };
+  if (do1) {
   if (qcf_status e = issue_stage1_loads(0)) return e;
   STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, nullptr, nullptr, 0, N, Lq, s->dims.hidden, s->x, cs));
   bool first = true;
@@ -313,11 +316,13 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
     STK_CUDA(ctx, cudaEventRecord(s->ev_done[l], cs));
   }
   if (qcf_status e = qcf_select_topk(ctx, mb, a->scores, a->ratio, a->sel, a->n_sel, cs)) return e;               // Eq. 11
+  }
+  if (!do2) return QCF_OK;
 
   // ---- stage 2: pipeline cache fusion.  The loader runs ahead through all remaining layers
   // (every layer has its own destination cache); the compute stream consumes them in order.
   for (int l = 0; l < n_l; ++l)
-    if (!is_crit(l) || l > l_max) { if (qcf_status e = load_pic(l)) return e; }
+    if (!do1 || !is_crit(l)) { if (qcf_status e = load_pic(l)) return e; }       // critical layers were stitched in stage 1
   STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, a->sel, a->n_sel, N, 0, n_rows, s->dims.hidden, s->x, cs));
   for (int l = 0; l < n_l; ++l) {
     if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(cs, s->ev_ready[slot_pic0 + l], 0));

@@ -91,13 +91,35 @@ class StackRun:
             self.v_pic.append(park(pool_v[l]))
         torch.cuda.synchronize()
 
-    def fuse(self, overlap: bool = True, stream=None):
+    def use_selector(self, kind: str):
+        """Which view stage 1 sees (include/qcf.h, qcf_stack_fuse): 'qcfuse' = per-chunk anchors + the critical layers
+        (the default, set by build_phase1), 'fullview' = every token of every chunk as an anchor + every layer
+        (ProphetKV-style, Eq. 9-11), 'final' = no anchors, last layer only.  Call after build_phase1."""
+        sp, ctx = self.sp, self.ctx
+        lens = [sp.chunk_len] * sp.n_chunks
+        off = [i * sp.chunk_len for i in range(sp.n_chunks)]
+        if not hasattr(self, "_qcfuse_view"):
+            self._qcfuse_view = (self.probe, self.k_anchor, self.v_anchor, self.anchor_rows, tuple(sp.crit_layers))
+        if kind == "qcfuse":
+            self.probe, self.k_anchor, self.v_anchor, self.anchor_rows, self.crit = self._qcfuse_view
+        elif kind == "fullview":
+            self.probe = ctx.batch([lens], [off], [sp.n_query], chunk_pos=[off])
+            self.k_anchor, self.v_anchor, self.anchor_rows = self.k_pic, self.v_pic, sp.n_ctx
+            self.crit = tuple(range(sp.n_layers))
+        elif kind == "final":
+            self.probe = ctx.batch([[0] * sp.n_chunks], [[0] * sp.n_chunks], [sp.n_query], chunk_pos=[off])
+            self.k_anchor, self.v_anchor, self.anchor_rows = self.k_pic, self.v_pic, 0
+            self.crit = (sp.n_layers - 1,)
+        else:
+            raise ValueError(kind)
+
+    def fuse(self, overlap: bool = True, stream=None, stages: int = 0):
         sp = self.sp
         self.stack.qcf_stack_fuse(self.main, self.probe, k_pic=self.k_pic, v_pic=self.v_pic, pool_rows=sp.n_ctx,
                                   k_anchor=self.k_anchor, v_anchor=self.v_anchor, anchor_rows=self.anchor_rows,
-                                  crit_layers=sp.crit_layers, ratio=sp.ratio, tokens=self.tokens, k_fused=self.k_fused,
+                                  crit_layers=getattr(self, "crit", sp.crit_layers), ratio=sp.ratio, tokens=self.tokens, k_fused=self.k_fused,
                                   v_fused=self.v_fused, scores=self.scores, sel=self.sel, n_sel=self.n_sel,
-                                  hidden_out=self.hidden, overlap=overlap, stream=stream)
+                                  hidden_out=self.hidden, overlap=overlap, stages=stages, stream=stream)
 
     def full_prefill(self, k_cache, v_cache, hidden_out=None, stream=None):
         self.stack.qcf_stack_prefill(self.full, self.tokens, k_cache, v_cache, hidden_out, stream)

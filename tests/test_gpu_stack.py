@@ -331,3 +331,55 @@ def test_stack_prefill_builds_pic_like_the_oracle():
     assert _close_bf16(_f64(kc[0]), ks[0], extra=5e-3) and _close_bf16(_f64(vc[0]), vs[0], extra=5e-3)
     for l in range(1, sp.n_layers):
         assert _rel_rms_err(_f64(kc[l]).reshape(len(toks), -1), ks[l].reshape(len(toks), -1)) <= 5e-2
+
+
+# ----------------------------------------------------------------------------------------------- selector views (§8(f).1)
+
+@pytest.mark.parametrize("view", ["fullview", "final"])
+def test_stack_fuse_other_selector_views(view):
+    """The compressed view is an argument of qcf_stack_fuse: full-view (every token an anchor, every layer scored:
+    ProphetKV-style, Eq. 9-11) and query-only final-layer selection run on the same kernels and match the
+    oracle's probe_stage given the same view; stage 1 and stage 2 issued separately reproduce the fused call bit for bit."""
+    from paper_2606_05875_b200 import stack_device
+    binding = _binding()
+    wl = inputs.make_stack_workload("s_small")
+    sp = wl.spec
+    ctx = binding.Context(sp.n_q_heads, sp.n_kv_heads, sp.head_dim, sp.rope_theta, 1, max(sp.n_ctx, 1024), sp.n_query)
+    run = stack_device.StackRun(wl, ctx, _device_layers(wl), _dev(wl.embed))
+    cfg, layers = _oracle_stack(wl)
+    emb, k_pic, v_pic = _pic_from_oracle(wl, cfg, layers)
+    L, n = sp.n_layers, sp.n_ctx
+    run.k_pic = [_dev(_to_bits(np.concatenate(k_pic[l], 0))) for l in range(L)]      # device-resident pools
+    run.v_pic = [_dev(_to_bits(np.concatenate(v_pic[l], 0))) for l in range(L)]
+    run.k_anchor, run.v_anchor = run.k_pic, run.v_pic                                  # replaced by use_selector
+    run.use_selector(view)
+    run.fuse()
+    torch.cuda.synchronize()
+    ref = [t.clone() for t in (run.scores, run.sel, run.hidden)] + [k.clone() for k in run.k_fused]
+    if view == "fullview":
+        lens = [sp.chunk_len] * sp.n_chunks
+        a_idx = np.concatenate([np.arange(ln) for ln in lens]).astype(np.int32)
+        a_ptr = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+        crit = list(range(L))
+    else:
+        a_idx = np.empty(0, np.int32)
+        a_ptr = np.zeros(sp.n_chunks + 1, np.int32)
+        crit = [L - 1]
+    pr = S.probe_stage(emb[wl.query_tokens], k_pic, v_pic, a_idx, a_ptr, layers, cfg, crit, sp.ratio)
+    got = run.scores.cpu().numpy().astype(np.float64)
+    assert abs(got.sum() - len(crit)) < 1e-3
+    np.testing.assert_allclose(got, pr["scores"], rtol=5e-2, atol=1e-7)          # free-running bound (DESIGN.md §5)
+    k_sel = run.k_sel
+    got_sel = run.sel[:k_sel].cpu().numpy().astype(np.int64)
+    assert np.array_equal(got_sel, O.select_topk(run.scores.cpu().numpy(), k_sel))
+    assert len(np.intersect1d(got_sel, pr["sel"])) >= 0.9 * k_sel
+    # stages issued separately
+    run.scores.zero_(); run.hidden.zero_()
+    run.fuse(stages=1)
+    torch.cuda.synchronize()
+    assert torch.equal(run.scores, ref[0]) and torch.equal(run.sel[:k_sel], ref[1][:k_sel])
+    assert torch.all(run.hidden == 0), "stage 1 alone recomputes nothing"
+    run.fuse(stages=2)
+    torch.cuda.synchronize()
+    assert torch.equal(run.hidden, ref[2])
+    assert all(torch.equal(a, b) for a, b in zip(run.k_fused, ref[3:]))
