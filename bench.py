@@ -437,6 +437,11 @@ def run_c3(args) -> None:
         selectors[view] = {"stage1_ms": float(s1.mean()), "pipeline_ms": float(tot.mean()), "probe_layers": l_pr,
                            "scored_layers": len(run.crit), "anchor_rows": run.anchor_rows,
                            "stage1_h2d_bytes": int(2 * kv_row_b * (run.anchor_rows * l_pr + sp.n_ctx * len(run.crit)))}
+    # bandwidth-constrained loading (Fig. 13): the loader emulates a KV store of the given GB/s
+    sweep = {}
+    for view in ("qcfuse", "fullview"):
+        run.use_selector(view)
+        sweep[view] = {str(g): float(timed(lambda: run.fuse(True, load_gbps=g), 2, 1).mean()) for g in (3.0, 6.0, 12.0, 25.0, 50.0)}
     use([host_k, host_v, host_ak, host_av])
     run.use_selector("qcfuse")
     kc = [torch.zeros_like(k) for k in run.k_fused]
@@ -478,7 +483,8 @@ def run_c3(args) -> None:
                      "speedup_over_full_prefill": float(full_ms.mean()) / t_fuse,
                      "whole_pipeline_TFLOPps": ach, "whole_pipeline_frac_tensor_peak": ach / peak,
                      "full_prefill_TFLOPps": (fl["gemm_full"] + fl["attn_full"]) / (float(full_ms.mean()) * 1e-3) / 1e12,
-                     "phase1_build_s": phase1_s, "selectors_pinned_host": selectors},
+                     "phase1_build_s": phase1_s, "selectors_pinned_host": selectors,
+                     "pipeline_ms_vs_load_gbps": sweep},
         "e2e": {"value": sp.n_ctx / (float(e2e_ms.mean()) * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(sp.n_query * sp.hidden * 2 + sp.n_ctx * 4), "ms_per_step": float(e2e_ms.mean()),
                 "ms_per_step_serial_loader": float(e2e_serial_ms.mean()),

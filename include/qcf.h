@@ -332,6 +332,9 @@ typedef struct {
   int32_t overlap;               /* != 0: layer-ahead loading on a second stream (a8); 0: serial, for the ablation  */
   int32_t stages;                /* 0 or 3: both stages; 1: stage 1 only (scores, sel, n_sel are produced, no layer is
                                     recomputed); 2: stage 2 only (sel / n_sel are INPUTS, e.g. from another selector)   */
+  double load_gbps;              /* > 0: emulate a KV store of this bandwidth (GB/s): every pool load on the loader stream
+                                    is held until bytes / load_gbps have elapsed since it started (the
+                                    bandwidth-constrained loading experiment); 0: unthrottled                            */
 } qcf_fuse_args;
 QCF_API qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* main_batch, const qcf_batch* probe_batch,
                                   const qcf_fuse_args* args, void* stream);

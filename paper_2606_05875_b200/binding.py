@@ -73,7 +73,7 @@ class qcf_fuse_args(C.Structure):
         ("k_anchor", C.POINTER(C.c_void_p)), ("v_anchor", C.POINTER(C.c_void_p)), ("anchor_rows", C.c_int64),
         ("crit_layers", C.POINTER(C.c_int32)), ("n_crit", C.c_int32), ("ratio", C.c_double), ("tokens", C.c_void_p),
         ("k_fused", C.POINTER(C.c_void_p)), ("v_fused", C.POINTER(C.c_void_p)), ("scores", C.c_void_p),
-        ("sel", C.c_void_p), ("n_sel", C.c_void_p), ("hidden_out", C.c_void_p), ("overlap", C.c_int32), ("stages", C.c_int32),
+        ("sel", C.c_void_p), ("n_sel", C.c_void_p), ("hidden_out", C.c_void_p), ("overlap", C.c_int32), ("stages", C.c_int32), ("load_gbps", C.c_double),
     ]
 
 
@@ -325,10 +325,10 @@ class Stack:
 
     def qcf_stack_fuse(self, main: Batch, probe: Batch, *, k_pic, v_pic, pool_rows: int, k_anchor, v_anchor,
                        anchor_rows: int, crit_layers, ratio: float, tokens, k_fused, v_fused, scores, sel, n_sel,
-                       hidden_out=None, overlap: bool = True, stages: int = 0, stream=None):
+                       hidden_out=None, overlap: bool = True, stages: int = 0, load_gbps: float = 0.0, stream=None):
         crit = (C.c_int32 * len(crit_layers))(*[int(c) for c in crit_layers])
         keep = [_ptr_array(x) for x in (k_pic, v_pic, k_anchor, v_anchor, k_fused, v_fused)]
         a = qcf_fuse_args(keep[0], keep[1], pool_rows, keep[2], keep[3], anchor_rows, crit, len(crit_layers), ratio,
                           _ptr(tokens), keep[4], keep[5], _ptr(scores), _ptr(sel), _ptr(n_sel), _ptr(hidden_out),
-                          1 if overlap else 0, int(stages))
+                          1 if overlap else 0, int(stages), float(load_gbps))
         self.ctx._check(self.lib.qcf_stack_fuse(self.handle, main.handle, probe.handle, C.byref(a), _stream(stream)))

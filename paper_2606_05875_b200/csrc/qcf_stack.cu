@@ -30,6 +30,7 @@ struct qcf_stack {
   cudaStream_t loader;
   std::vector<cudaEvent_t> ev_ready, ev_done;      // per pipeline slot
   cudaEvent_t ev_fork, ev_join;
+  unsigned long long* load_t0;                     // device stamp of the bandwidth emulation (load_gbps)
   int32_t* zero_i32;                               // device zeros: the probe stage's empty selection
 };
 
@@ -158,6 +159,8 @@ qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_
     for (int i = 0; i < 2 && ok; ++i)
       ok = dalloc(&s->probe_k[i], s->probe_rows * kv) == cudaSuccess && dalloc(&s->probe_v[i], s->probe_rows * kv) == cudaSuccess;
   }
+  s->load_t0 = nullptr;
+  ok = ok && dalloc(&s->load_t0, 2) == cudaSuccess;
   ok = ok && dalloc(&s->zero_i32, 4) == cudaSuccess && cudaMemset(s->zero_i32, 0, 16) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&s->loader, cudaStreamNonBlocking) == cudaSuccess &&
        cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
@@ -191,6 +194,7 @@ void qcf_stack_destroy(qcf_stack* s) {
   for (cudaEvent_t e : s->ev_done) if (e) cudaEventDestroy(e);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
+  if (s->load_t0) cudaFree(s->load_t0);
   if (s->zero_i32) cudaFree(s->zero_i32);
   if (s->loader) cudaStreamDestroy(s->loader);
   delete s;
@@ -271,12 +275,21 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
 
   // Loader jobs, in the order the pipeline consumes them.  The staging buffer of a job is read by the stitch kernel
   // issued right behind it on the same stream, so ring reuse needs no cross-stream wait; destinations are per layer.
+  STK_REQUIRE(ctx, a->load_gbps >= 0.0, "qcf_stack_fuse: load_gbps must be >= 0");
+  // bandwidth emulation (load_gbps > 0): stamp before a job's copies, hold the loader until bytes / load_gbps have passed
+  auto throttle_begin = [&]() -> cudaError_t { return a->load_gbps > 0.0 ? launch_stamp(s->load_t0, ls) : cudaSuccess; };
+  auto throttle_end = [&](size_t bytes) -> cudaError_t {
+    if (!(a->load_gbps > 0.0)) return cudaSuccess;
+    return launch_hold(s->load_t0, static_cast<unsigned long long>(static_cast<double>(bytes) / a->load_gbps), ls);   // B / (GB/s) = ns
+  };
   auto load_pic = [&](int l) -> qcf_status {
     STK_REQUIRE(ctx, a->k_pic[l] && a->v_pic[l] && a->k_fused[l] && a->v_fused[l], "qcf_stack_fuse: NULL pool / cache pointer");
     __nv_bfloat16 *sk = s->stage_k[ring], *sv = s->stage_v[ring];
     ring = (ring + 1) % qcf_stack::kRing;
+    STK_CUDA(ctx, throttle_begin());
     STK_CUDA(ctx, cudaMemcpyAsync(sk, a->k_pic[l], a->pool_rows * kv_row, cudaMemcpyDefault, ls));
     STK_CUDA(ctx, cudaMemcpyAsync(sv, a->v_pic[l], a->pool_rows * kv_row, cudaMemcpyDefault, ls));
+    STK_CUDA(ctx, throttle_end(2 * a->pool_rows * kv_row));
     if (qcf_status e = qcf_rope_reposition(ctx, mb, sk, sv, a->k_fused[l], a->v_fused[l], ls)) return e;      // a1
     STK_CUDA(ctx, cudaEventRecord(s->ev_ready[slot_pic0 + l], ls));
     return QCF_OK;
@@ -285,8 +298,10 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
     STK_REQUIRE(ctx, a->k_anchor[l] && a->v_anchor[l], "qcf_stack_fuse: NULL anchor pool pointer");
     __nv_bfloat16 *sk = s->stage_k[ring], *sv = s->stage_v[ring];
     ring = (ring + 1) % qcf_stack::kRing;
+    STK_CUDA(ctx, throttle_begin());
     STK_CUDA(ctx, cudaMemcpyAsync(sk, a->k_anchor[l], a->anchor_rows * kv_row, cudaMemcpyDefault, ls));
     STK_CUDA(ctx, cudaMemcpyAsync(sv, a->v_anchor[l], a->anchor_rows * kv_row, cudaMemcpyDefault, ls));
+    STK_CUDA(ctx, throttle_end(2 * a->anchor_rows * kv_row));
     if (l >= 2 && ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(ls, s->ev_done[l - 2], 0));   // probe cache l&1 is free again
     if (qcf_status e = qcf_rope_reposition(ctx, pb, sk, sv, s->probe_k[l & 1], s->probe_v[l & 1], ls)) return e;   // a1'
     STK_CUDA(ctx, cudaEventRecord(s->ev_ready[l], ls));

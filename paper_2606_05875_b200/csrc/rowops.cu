@@ -123,7 +123,32 @@ __global__ void __launch_bounds__(256) qknorm_rope_kernel(const __nv_bfloat16* _
   }
 }
 
+// Bandwidth emulation for the loader stream: stamp the start of a load, then hold the stream until `budget_ns` have
+// elapsed since the stamp (the copy itself runs in between; if it took longer, no wait).
+__global__ void stamp_kernel(unsigned long long* t0) {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  *t0 = t;
+}
+__global__ void hold_kernel(const unsigned long long* t0, unsigned long long budget_ns) {
+  const unsigned long long until = *t0 + budget_ns;
+  unsigned long long t;
+  do {
+    __nanosleep(2000);
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  } while (t < until);
+}
+
 }  // namespace
+
+cudaError_t launch_stamp(unsigned long long* t0, cudaStream_t stream) {
+  stamp_kernel<<<1, 1, 0, stream>>>(t0);
+  return cudaGetLastError();
+}
+cudaError_t launch_hold(const unsigned long long* t0, unsigned long long budget_ns, cudaStream_t stream) {
+  hold_kernel<<<1, 1, 0, stream>>>(t0, budget_ns);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_rope_table(float2* table, int n_pos, int d, double theta, cudaStream_t stream) {
   const int n = n_pos * (d / 2);

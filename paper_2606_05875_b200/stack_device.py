@@ -113,13 +113,13 @@ class StackRun:
         else:
             raise ValueError(kind)
 
-    def fuse(self, overlap: bool = True, stream=None, stages: int = 0):
+    def fuse(self, overlap: bool = True, stream=None, stages: int = 0, load_gbps: float = 0.0):
         sp = self.sp
         self.stack.qcf_stack_fuse(self.main, self.probe, k_pic=self.k_pic, v_pic=self.v_pic, pool_rows=sp.n_ctx,
                                   k_anchor=self.k_anchor, v_anchor=self.v_anchor, anchor_rows=self.anchor_rows,
                                   crit_layers=getattr(self, "crit", sp.crit_layers), ratio=sp.ratio, tokens=self.tokens, k_fused=self.k_fused,
                                   v_fused=self.v_fused, scores=self.scores, sel=self.sel, n_sel=self.n_sel,
-                                  hidden_out=self.hidden, overlap=overlap, stages=stages, stream=stream)
+                                  hidden_out=self.hidden, overlap=overlap, stages=stages, load_gbps=load_gbps, stream=stream)
 
     def full_prefill(self, k_cache, v_cache, hidden_out=None, stream=None):
         self.stack.qcf_stack_prefill(self.full, self.tokens, k_cache, v_cache, hidden_out, stream)

@@ -383,3 +383,14 @@ def test_stack_fuse_other_selector_views(view):
     torch.cuda.synchronize()
     assert torch.equal(run.hidden, ref[2])
     assert all(torch.equal(a, b) for a, b in zip(run.k_fused, ref[3:]))
+    # bandwidth emulation changes timing only: same bits, and the call takes at least bytes / bandwidth
+    import time
+    kv_row = sp.n_kv_heads * sp.head_dim * 2
+    bytes_min = 2 * kv_row * n * L                            # every PIC pool is loaded once
+    gbps = 0.5
+    t0 = time.perf_counter()
+    run.fuse(load_gbps=gbps)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    assert torch.equal(run.hidden, ref[2]) and torch.equal(run.scores, ref[0])
+    assert dt >= 0.9 * bytes_min / (gbps * 1e9)
