@@ -113,6 +113,34 @@ def anchor_stitch(k_pic: Sequence[np.ndarray], v_pic: Sequence[np.ndarray],
     return np.concatenate(ks, 0), np.concatenate(vs, 0), np.concatenate(ps, 0).astype(np.int64)
 
 
+# --------------------------------------------------------------------------- Phase I: anchors (Eq. 14)
+
+
+def n_anchor(chunk_len: int, r_a: float) -> int:
+    """ceil(r_a |c_i|) (Eq. 14), evaluated in double with a 1e-6 guard against r_a * len landing a hair
+    above an integer (0.1 * 512 = 51.2 -> 52; 0.25 * 64 = 16 exactly -> 16)."""
+    return int(min(chunk_len, np.ceil(np.float64(r_a) * np.float64(chunk_len) - 1e-6)))
+
+
+def anchor_scores(k_chunk: np.ndarray, rule: str) -> np.ndarray:
+    """G_i(r) of Eq. 14 for the two key-statistics rules the paper names:
+         'sink'  keeps tokens near the beginning of the chunk:  G(r) = -r
+         'knorm' ranks positions by the norm of their key-cache rows.  The paper does not say which end is kept; the rule
+                 it cites keeps LOW-norm keys, so G(r) = -||K_i[r]||_2 over all kv-heads and dims (reading (o')).
+    k_chunk [len, Hkv, d] (one layer's PIC keys of the chunk; RoPE does not change the norm)."""
+    ln = k_chunk.shape[0]
+    if rule == "sink":
+        return -np.arange(ln, dtype=np.float64)
+    if rule == "knorm":
+        return -np.sqrt(np.sum(np.square(np.asarray(k_chunk, dtype=np.float64).reshape(ln, -1)), axis=1))
+    raise ValueError(rule)
+
+
+def anchor_select(k_chunk: np.ndarray, r_a: float, rule: str) -> np.ndarray:
+    """A_i = TopK(G_i, ceil(r_a |c_i|)) (Eq. 14), ties to the lower position, ascending chunk-local positions."""
+    return select_topk(anchor_scores(k_chunk, rule), n_anchor(k_chunk.shape[0], r_a))
+
+
 # --------------------------------------------------------------------------- score (Eq. 18, 20)
 
 

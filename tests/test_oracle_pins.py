@@ -296,3 +296,31 @@ def test_future_rows_do_not_influence_a_row_and_lse():
     # lse is the log of the softmax denominator: exp(s - lse) sums to 1 over the visible prefix
     s = (qn[rows[r0], 0] @ kf[: p + 1, 0].T) / np.sqrt(qn.shape[-1])
     assert abs(np.exp(s - lse[r0, 0]).sum() - 1.0) < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------- Phase I anchors (Eq. 14)
+
+def test_anchor_count_is_ceil_eq14():
+    # 20 chunks x ceil(0.1 * 512) = 1040 anchor rows; exact products are not bumped
+    assert O.n_anchor(512, 0.1) == 52 and 20 * O.n_anchor(512, 0.1) == 1040
+    assert O.n_anchor(64, 0.25) == 16 and O.n_anchor(10, 0.1) == 1 and O.n_anchor(7, 1.0) == 7 and O.n_anchor(5, 0.0) == 0
+    assert O.n_anchor(131, 0.1) == 14
+
+
+def test_anchor_rules_sink_and_knorm():
+    rng = np.random.default_rng(4)
+    k = rng.standard_normal((97, 2, 16))
+    # sink: the first ceil(r_a len) positions
+    assert np.array_equal(O.anchor_select(k, 0.1, "sink"), np.arange(10))
+    # knorm: brute force over explicit norms (lowest norms kept), ascending output
+    norms = np.array([np.linalg.norm(k[r]) for r in range(97)])
+    want = np.sort(np.argsort(norms, kind="stable")[:10])
+    assert np.array_equal(O.anchor_select(k, 0.1, "knorm"), want)
+    # shrinking one row's key makes it an anchor; the norm ignores a rotation of the pairs (RoPE-invariant)
+    k2 = k.copy(); k2[50] *= 1e-3
+    assert 50 in O.anchor_select(k2, 0.1, "knorm")
+    phi = O.rope_angles(np.arange(97) + 1234, 16, 1e4)
+    assert np.array_equal(O.anchor_select(O.rotate(k, phi), 0.1, "knorm"), want)
+    # ties go to the lower position
+    k3 = np.ones((8, 1, 4))
+    assert np.array_equal(O.anchor_select(k3, 0.5, "knorm"), np.arange(4))
