@@ -194,6 +194,23 @@ QCF_API qcf_status qcf_full_prefill_attn(qcf_ctx* ctx, const qcf_batch* b, const
  * the probe cache KV^A(C_A) [B][t_stride][Hkv][d] (t_stride of that batch = max_b (|C_A|_b + Lq_b)).  With
  * v_pool == NULL and v_fused == NULL only K is re-positioned (scoring prefetch of the critical layers reads no V). */
 
+/* ------------------------------------------------------------------------------------- Phase I: anchors */
+
+/* Eq. 14: A_i = TopK(G_i, ceil(r_a |c_i|)) for every chunk of the batch, which must list ONE chunk
+ * per request (n_chunks = 1, n_query = 0; chunk_row = the chunk's first row in k_pool).
+ *   rule QCF_ANCHOR_SINK : G_i(r) = -r                  (the first positions of the chunk)
+ *   rule QCF_ANCHOR_KNORM: G_i(r) = -||K_i[r]||_2       over all kv-heads and dims of the layer's PIC keys (the paper
+ *                          does not say which end of the norm ranking is kept; low-norm keys, reading (o'))
+ *   k_pool   : dev [pool_rows][Hkv][d] bf16 (ignored for SINK; may be NULL)
+ *   scores   : dev [B][n_stride] fp32 workspace, receives G_i; accumulate != 0 adds to it (norms summed over layers:
+ *              call once per layer with select_now = 0, then once with select_now != 0)
+ *   anchor_idx : dev [B][n_stride] int32, chunk-local positions ascending; n_anchor : dev [B] int32
+ * KVzip (a reconstruction probe over a trained model) is out of scope. */
+typedef enum { QCF_ANCHOR_SINK = 0, QCF_ANCHOR_KNORM = 1 } qcf_anchor_rule;
+QCF_API qcf_status qcf_anchor_rank(qcf_ctx* ctx, const qcf_batch* chunks, const void* k_pool, int32_t rule, double r_a,
+                                   float* scores, int32_t accumulate, int32_t select_now, int32_t* anchor_idx,
+                                   int32_t* n_anchor, void* stream);
+
 /* ------------------------------------------------------------------------------------------------ a6 */
 
 /* Everything one layer needs, by name.  Pointers as documented at the stage entry points. */

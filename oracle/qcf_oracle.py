@@ -12,7 +12,8 @@ is silent the reading is the one listed in DESIGN.md ("Readings", letters (a)..(
 
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): closed-form RoPE composition, complex-number
 restatement, relative-position invariance, softmax sums, torch fp64 SDPA for rho=1 / rho=0 /
-single-chunk cases, brute-force top-k, hand-computed fixtures under tests/golden/.
+single-chunk cases, brute-force top-k, hand-computed fixtures under tests/golden/, anchor counts and
+brute-force Sink / Knorm rankings (Eq. 14).
 Parity unpinned: none of the functions below; *selection quality versus the paper's
 Recall@10% / F1 claims* is unpinned (needs the datasets and trained weights).
 

@@ -22,10 +22,11 @@ EXPORTS = (
     "qcf_create", "qcf_destroy", "qcf_last_error", "qcf_version", "qcf_batch_create", "qcf_batch_destroy",
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms",
-    "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse",
+    "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse",
 )
 
 QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
+QCF_ANCHOR_SINK, QCF_ANCHOR_KNORM = 0, 1
 
 
 class QcfError(RuntimeError):
@@ -110,6 +111,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_layer_step_host": (i32, [vp, vp, C.POINTER(qcf_layer_args), i64, vp]),
         "qcf_set_profiling": (i32, [vp, i32]),
         "qcf_get_stage_ms": (i32, [vp, C.POINTER(C.c_float)]),
+        "qcf_anchor_rank": (i32, [vp, vp, vp, i32, f64, vp, i32, i32, vp, vp, vp]),
         "qcf_linear": (i32, [vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]),
         "qcf_stack_create": (i32, [vp, C.POINTER(qcf_stack_dims), C.POINTER(qcf_layer_weights), vp, i32, i32, i64,
                                    C.POINTER(vp)]),
@@ -224,6 +226,12 @@ class Context:
 
     def batch(self, chunk_lens, chunk_rows, n_query, chunk_pos=None) -> Batch:
         return Batch(self, chunk_lens, chunk_rows, n_query, chunk_pos)
+
+    def qcf_anchor_rank(self, chunks: Batch, k_pool, rule: int, r_a: float, scores, anchor_idx, n_anchor,
+                        accumulate: bool = False, select_now: bool = True, stream=None):
+        self._check(self.lib.qcf_anchor_rank(self.handle, chunks.handle, _ptr(k_pool), int(rule), float(r_a), _ptr(scores),
+                                             int(bool(accumulate)), int(bool(select_now)), _ptr(anchor_idx), _ptr(n_anchor),
+                                             _stream(stream)))
 
     def qcf_linear(self, a, w, residual, c, M: int, N: int, K: int, epilogue: int = QCF_EPI_STORE, stream=None):
         self._check(self.lib.qcf_linear(self.handle, _ptr(a), _ptr(w), _ptr(residual), _ptr(c), M, N, K, epilogue,

@@ -362,6 +362,25 @@ qcf_status qcf_select_topk(qcf_ctx* ctx, const qcf_batch* b, const float* scores
   return QCF_OK;
 }
 
+qcf_status qcf_anchor_rank(qcf_ctx* ctx, const qcf_batch* b, const void* k_pool, int32_t rule, double r_a, float* scores,
+                           int32_t accumulate, int32_t select_now, int32_t* anchor_idx, int32_t* n_anchor, void* stream) {
+  if (qcf_status st = check_ctx_batch(ctx, b)) return st;
+  QCF_REQUIRE(ctx, rule == QCF_ANCHOR_SINK || rule == QCF_ANCHOR_KNORM, "qcf_anchor_rank: unknown rule");
+  QCF_REQUIRE(ctx, r_a >= 0.0 && r_a <= 1.0, "qcf_anchor_rank: r_a must be in [0, 1]");
+  QCF_REQUIRE(ctx, b->n_chunks <= b->batch && b->q_stride == 0, "qcf_anchor_rank: the batch must list one chunk per request and no query");
+  if (b->batch == 0) return QCF_OK;
+  QCF_REQUIRE(ctx, scores || b->n_stride == 0, "qcf_anchor_rank: scores is NULL");
+  QCF_REQUIRE(ctx, rule == QCF_ANCHOR_SINK || k_pool, "qcf_anchor_rank: k_pool is NULL");
+  QCF_REQUIRE(ctx, aligned16(k_pool), "qcf_anchor_rank: k_pool must be 16-byte aligned");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  QCF_CUDA(ctx, launch_anchor_scores(ctx, b, static_cast<const __nv_bfloat16*>(k_pool), rule, accumulate != 0, scores, s));
+  if (select_now) {
+    QCF_REQUIRE(ctx, n_anchor && (anchor_idx || b->n_stride == 0), "qcf_anchor_rank: NULL output pointer");
+    QCF_CUDA(ctx, launch_topk(ctx, b, scores, r_a, anchor_idx, n_anchor, s, /*ceil_mode=*/1));
+  }
+  return QCF_OK;
+}
+
 qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
                               const void* q_new, const void* k_new, const void* v_new, int32_t rows_by_position,
                               void* k_fused, void* v_fused, void* out, float* lse, void* stream) {

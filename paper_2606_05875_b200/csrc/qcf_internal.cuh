@@ -108,7 +108,10 @@ cudaError_t launch_reposition(const qcf_ctx*, const qcf_batch*, const __nv_bfloa
 cudaError_t launch_score(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* q_probe, const __nv_bfloat16* k_f,
                          float* scores, int accumulate, cudaStream_t);
 cudaError_t launch_topk(const qcf_ctx*, const qcf_batch*, const float* scores, double ratio, int32_t* sel,
-                        int32_t* n_sel, cudaStream_t);
+                        int32_t* n_sel, cudaStream_t, int ceil_mode = 0);
+// G_i(r) of Eq. 14 for every chunk row of the batch (rule 0: sink, 1: knorm) into scores[B][n_stride]
+cudaError_t launch_anchor_scores(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool, int rule, int accumulate,
+                                 float* scores, cudaStream_t);
 cudaError_t launch_scatter(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                            const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, int rows_by_position,
                            __nv_bfloat16* k_f, __nv_bfloat16* v_f, cudaStream_t);

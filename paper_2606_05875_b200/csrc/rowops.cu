@@ -123,6 +123,42 @@ __global__ void __launch_bounds__(256) qknorm_rope_kernel(const __nv_bfloat16* _
   }
 }
 
+// Phase I, Eq. 14: anchor ranking scores of the two key-statistics rules, one warp per chunk row.
+//   rule 0 (Sink):  G(r) = -r                       keeps the first positions of the chunk
+//   rule 1 (Knorm): G(r) = -||K_i[r]||_2            over all kv-heads and dims (low-norm keys are kept, reading (o'))
+// Every request of the batch is ONE chunk; scores[b][r], r < len_b.  accumulate != 0 adds (norms summed over layers).
+__global__ void __launch_bounds__(256) anchor_score_kernel(BatchDev bd, int row_vec, const uint4* __restrict__ k_pool, int rule,
+                                                           int accumulate, float* __restrict__ scores) {
+  const int b = blockIdx.y;
+  const int len = bd.n_ctx[b];
+  const int r = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (r >= len) return;
+  float g;
+  if (rule == 0) {
+    g = -static_cast<float>(r);
+  } else {
+    // the request's single chunk is entry b of the chunk arrays only if no request was empty: find it by owner
+    int c = b < bd.n_chunks ? b : bd.n_chunks - 1;
+    while (c > 0 && bd.chunk_req[c] > b) --c;
+    while (c + 1 < bd.n_chunks && bd.chunk_req[c] < b) ++c;
+    const uint4* src = k_pool + (static_cast<size_t>(bd.chunk_row[c]) + r) * row_vec;
+    float ss = 0.f;
+    for (int i = lane; i < row_vec; i += 32) {
+      const uint4 v = ld_nc_v4(src + i);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { const float x = bf16lo(w[k]), y = bf16hi(w[k]); ss = fmaf(x, x, ss); ss = fmaf(y, y, ss); }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    g = -sqrtf(ss);
+  }
+  if (lane == 0) {
+    float* dst = scores + static_cast<size_t>(b) * bd.n_stride + r;
+    *dst = accumulate ? *dst + g : g;
+  }
+}
+
 // Bandwidth emulation for the loader stream: stamp the start of a load, then hold the stream until `budget_ns` have
 // elapsed since the stamp (the copy itself runs in between; if it took longer, no wait).
 __global__ void stamp_kernel(unsigned long long* t0) {
@@ -140,6 +176,14 @@ __global__ void hold_kernel(const unsigned long long* t0, unsigned long long bud
 }
 
 }  // namespace
+
+cudaError_t launch_anchor_scores(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* k_pool, int rule, int accumulate,
+                                 float* scores, cudaStream_t stream) {
+  if (b->batch == 0 || b->n_stride == 0) return cudaSuccess;
+  anchor_score_kernel<<<dim3((b->n_stride + 7) / 8, b->batch), 256, 0, stream>>>(
+      b->dev, ctx->lay.hkv * ctx->lay.d / 8, reinterpret_cast<const uint4*>(k_pool), rule, accumulate, scores);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_stamp(unsigned long long* t0, cudaStream_t stream) {
   stamp_kernel<<<1, 1, 0, stream>>>(t0);

@@ -20,7 +20,7 @@ __device__ __forceinline__ uint32_t order_key(float f) {
 }
 
 __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float* __restrict__ scores, double ratio,
-                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached) {
+                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached, int ceil_mode) {
   extern __shared__ uint32_t s_keys[];                           // order keys of the first n_cached scores
   __shared__ unsigned int hist[256];
   __shared__ unsigned int s_prefix, s_remaining;
@@ -29,7 +29,9 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   const int b = blockIdx.x;
   const int N = bd.n_ctx[b];
   pdl_wait();
-  const int k = static_cast<int>(floor(ratio * static_cast<double>(N) + 1e-6));    // reading (g)
+  // floor(rho N + 1e-6) for the recompute set (Eq. 8, reading (g)); ceil(r_a N - 1e-6) for anchors (Eq. 14)
+  const int k = ceil_mode ? min(N, static_cast<int>(ceil(ratio * static_cast<double>(N) - 1e-6)))
+                          : static_cast<int>(floor(ratio * static_cast<double>(N) + 1e-6));
   const float* s = scores + static_cast<size_t>(b) * bd.n_stride;
   int32_t* out = sel + static_cast<size_t>(b) * bd.n_stride;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -128,7 +130,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
 }  // namespace
 
 cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* scores, double ratio, int32_t* sel,
-                        int32_t* n_sel, cudaStream_t stream) {
+                        int32_t* n_sel, cudaStream_t stream, int ceil_mode) {
   if (b->batch == 0) return cudaSuccess;
   // up to 48 K keys (192 KB) are cached in shared memory; longer contexts read the remainder from L2
   const int n_cached = b->n_stride < 49152 ? b->n_stride : 49152;
@@ -138,7 +140,7 @@ cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* sco
     cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
     attr_set = true;
   }
-  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached);
+  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode);
 }
 
 }  // namespace qcf

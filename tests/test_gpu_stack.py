@@ -394,3 +394,47 @@ def test_stack_fuse_other_selector_views(view):
     dt = time.perf_counter() - t0
     assert torch.equal(run.hidden, ref[2]) and torch.equal(run.scores, ref[0])
     assert dt >= 0.9 * bytes_min / (gbps * 1e9)
+
+
+# ----------------------------------------------------------------------------------------------- Phase I anchors (§8(f).2)
+
+@pytest.mark.parametrize("rule", ["sink", "knorm"])
+def test_anchor_rank_parity(rule):
+    """Eq. 14 on the GPU: per-chunk anchor ranking (Sink / Knorm) + segmented top-ceil(r_a len) against the oracle."""
+    binding = _binding()
+    wl = inputs.make_workload("t_ragged")                      # chunk lengths 131 / 64 / 1 / 257 / 77
+    cfg = wl.cfg
+    lens = [k.shape[0] for k in wl.pool_k]
+    starts = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    ctx = binding.Context(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, len(lens), 1024, 8)
+    chunks = ctx.batch([[ln] for ln in lens], [[int(s)] for s in starts[:-1]], [0] * len(lens))
+    pool = _dev(np.concatenate(wl.pool_k, 0))
+    pool2 = _dev(np.concatenate(wl.pool_v, 0))                 # stands in for a second layer's keys
+    B, Nn = len(lens), chunks.n_stride
+    scores = torch.full((B, Nn), 7.0, device="cuda")
+    idx = torch.full((B, Nn), -1, dtype=torch.int32, device="cuda")
+    n_a = torch.zeros(B, dtype=torch.int32, device="cuda")
+    r_a = 0.1
+    code = binding.QCF_ANCHOR_SINK if rule == "sink" else binding.QCF_ANCHOR_KNORM
+    ctx.qcf_anchor_rank(chunks, pool, code, r_a, scores, idx, n_a)
+    torch.cuda.synchronize()
+    for i, ln in enumerate(lens):
+        want = O.anchor_select(O.widen_bf16(wl.pool_k[i]), r_a, rule)
+        k = O.n_anchor(ln, r_a)
+        assert int(n_a[i]) == k == len(want)
+        got = idx[i, :k].cpu().numpy().astype(np.int64)
+        g = scores[i, :ln].cpu().numpy()
+        assert np.array_equal(got, O.select_topk(g, k)), "exact on the kernel's own scores"
+        np.testing.assert_allclose(g, O.anchor_scores(O.widen_bf16(wl.pool_k[i]), rule), rtol=1e-5, atol=0)
+        _check_sel = len(np.intersect1d(got, want))
+        assert _check_sel >= np.ceil(0.99 * k)
+        assert torch.all(idx[i, k:] == -1) and torch.all(scores[i, ln:] == 7.0)
+    if rule == "knorm":                                        # norms summed over two layers, selection on the second call
+        ctx.qcf_anchor_rank(chunks, pool, code, r_a, scores, idx, n_a, accumulate=False, select_now=False)
+        ctx.qcf_anchor_rank(chunks, pool2, code, r_a, scores, idx, n_a, accumulate=True, select_now=True)
+        torch.cuda.synchronize()
+        for i, ln in enumerate(lens):
+            g2 = O.anchor_scores(O.widen_bf16(wl.pool_k[i]), rule) + O.anchor_scores(O.widen_bf16(wl.pool_v[i]), rule)
+            k = O.n_anchor(ln, r_a)
+            got = idx[i, :k].cpu().numpy().astype(np.int64)
+            assert len(np.intersect1d(got, O.select_topk(g2, k))) >= np.ceil(0.99 * k)
