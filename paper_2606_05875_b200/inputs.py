@@ -280,13 +280,17 @@ class StackWorkload:
     anchor_ptr: np.ndarray                       # int32 [m+1]
 
 
-def make_stack_workload(name: str, *, ratio: Optional[float] = None, with_weights: bool = True) -> StackWorkload:
+def make_stack_workload(name: str, *, ratio: Optional[float] = None, with_weights: bool = True,
+                        n_layers: Optional[int] = None) -> StackWorkload:
     """Seeded stack + request.  Weights ~ N(0, 0.02^2), embeddings ~ N(0, 1), norm gains 1 + 0.1 N(0, 1) (so that a
     dropped gain is visible to the parity tests), all rounded to bf16 (both the oracle and the library read these
     bit patterns); token ids uniform over the synthetic vocabulary; anchors as in make_workload (reading (o))."""
     sp = STACKS[name]
     if ratio is not None:
         sp = StackSpec(**{**sp.__dict__, "ratio": ratio})
+    if n_layers is not None:          # the first n_layers layers of the same seeded stack (full-size single-layer tests)
+        sp = StackSpec(**{**sp.__dict__, "n_layers": n_layers,
+                          "crit_layers": tuple(c for c in sp.crit_layers if c < n_layers) or (0,)})
     ss = np.random.SeedSequence(sp.seed)
     s_emb, s_w, s_tok, s_anchor = ss.spawn(4)
     rng_e, rng_w = np.random.default_rng(s_emb), np.random.default_rng(s_w)

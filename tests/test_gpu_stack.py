@@ -438,3 +438,52 @@ def test_anchor_rank_parity(rule):
             k = O.n_anchor(ln, r_a)
             got = idx[i, :k].cpu().numpy().astype(np.int64)
             assert len(np.intersect1d(got, O.select_topk(g2, k))) >= np.ceil(0.99 * k)
+
+
+# ----------------------------------------------------------------------------------------------- config 3 at full size
+
+def test_stack_layer_full_size_c3_sampled():
+    """BASELINE configs[2] at its own sizes (N = 10240, Lq = 64, n_R = 3136, hidden 4096, FFN 12288, 32/8 heads), one
+    layer, teacher-forced: refreshed K/V of ALL rows against the oracle, the layer output on a declared row sample (all
+    query rows, first / last 32 selected rows, 64 seeded random rows) — rows are independent given the fused cache."""
+    binding = _binding()
+    wl = inputs.make_stack_workload("c3", n_layers=1)
+    sp = wl.spec
+    cfg, layers = _oracle_stack(wl)
+    w = layers[0]
+    n, lq, hkv, d = sp.n_ctx, sp.n_query, sp.n_kv_heads, sp.head_dim
+    t = n + lq
+    ctx = binding.Context(sp.n_q_heads, hkv, d, sp.rope_theta, 1, n, lq)
+    stack = binding.Stack(ctx, 1, sp.hidden, sp.ffn, sp.vocab, sp.rms_eps, _device_layers(wl), _dev(wl.embed), t, t,
+                          max_pool_rows=n)
+    rng = np.random.default_rng(303)
+    pool_k = inputs.f32_to_bf16_bits(rng.standard_normal((n, hkv, d), dtype=np.float32))
+    pool_v = inputs.f32_to_bf16_bits(rng.standard_normal((n, hkv, d), dtype=np.float32))
+    mb = ctx.batch([[sp.chunk_len] * sp.n_chunks], [[i * sp.chunk_len for i in range(sp.n_chunks)]], [lq])
+    k_sel = binding.qcf_n_select(n, sp.ratio)
+    assert k_sel == 3072
+    sel = np.sort(rng.choice(n, size=k_sel, replace=False)).astype(np.int32)
+    rows = np.concatenate([sel, np.arange(n, n + lq)]).astype(np.int64)
+    x_bits = inputs.f32_to_bf16_bits(rng.standard_normal((len(rows), sp.hidden), dtype=np.float32))
+    kf = torch.zeros((1, mb.t_stride, hkv, d), dtype=torch.bfloat16, device="cuda")
+    vf = torch.zeros_like(kf)
+    ctx.qcf_rope_reposition(mb, _dev(pool_k), _dev(pool_v), kf, vf)
+    torch.cuda.synchronize()
+    k_ctx, v_ctx = _f64(kf[0, :n]), _f64(vf[0, :n])
+    x = _dev(x_bits)
+    stack.qcf_stack_layer(0, mb, torch.from_numpy(sel).cuda(), torch.tensor([k_sel], dtype=torch.int32, device="cuda"),
+                          len(rows), x, kf, vf)
+    torch.cuda.synchronize()
+    x_in = O.widen_bf16(x_bits)
+    q, k_new, v_new = S.layer_qkv(x_in, rows, w, cfg)                     # all rows: the fused cache needs every refresh
+    assert _close_bf16(_f64(kf[0])[rows], k_new, extra=5e-3)
+    assert _close_bf16(_f64(vf[0])[rows], v_new, extra=5e-3)
+    k_pos = np.zeros((t, hkv, d)); v_pos = np.zeros((t, hkv, d))
+    k_pos[rows], v_pos[rows] = k_new, v_new
+    k_f, v_f = O.fuse(k_ctx, v_ctx, sel.astype(np.int64), k_pos, v_pos)
+    samp = np.unique(np.concatenate([np.arange(32), np.arange(k_sel - 32, k_sel), rng.choice(k_sel, 64, replace=False),
+                                     np.arange(k_sel, k_sel + lq)]))
+    a = O.recompute_attn(q[samp], rows[samp], k_f, v_f)
+    want = S.layer_finish(x_in[samp], a, w, cfg)
+    err = _rel_rms_err(_f64(x)[samp], want)
+    assert err <= 3e-2, err
