@@ -373,6 +373,30 @@ def test_layer_step_back_to_back_is_race_free():
     assert torch.equal(ref[3][0, :n_r], dw.out[0, :n_r]) and torch.equal(ref[4], dw.k_fused) and torch.equal(ref[5], dw.v_fused)
 
 
+def test_layer_step_is_cuda_graph_capturable():
+    """include/qcf.h: hot-path calls launch kernels only (no copies, no syncs, PDL attributes included), so a whole
+    qcf_layer_step can be captured in a CUDA graph and replayed."""
+    wl, ctx, dw = _setup("t_mid")
+    args = dw.layer_args(lse=dw.lse)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        ctx.qcf_layer_step(dw.batch, args)
+        torch.cuda.synchronize()
+        ref = [t.clone() for t in (dw.scores, dw.sel, dw.out, dw.k_fused)]
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ctx.qcf_layer_step(dw.batch, args)
+        for t in (dw.scores, dw.out):
+            t.fill_(9.0)
+        g.replay()
+        g.replay()
+        torch.cuda.synchronize()
+    k = int(dw.n_sel[0])
+    n_r = k + wl.requests[0].n_query
+    assert torch.equal(ref[0], dw.scores) and torch.equal(ref[1][0, :k], dw.sel[0, :k])
+    assert torch.equal(ref[2][0, :n_r], dw.out[0, :n_r]) and torch.equal(ref[3], dw.k_fused)
+
+
 def test_layer_step_profiling_and_noncritical():
     wl, ctx, dw = _setup("t_mid")
     ctx.qcf_set_profiling(True)
