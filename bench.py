@@ -444,9 +444,30 @@ def run_c3(args) -> None:
         sweep[view] = {str(g): float(timed(lambda: run.fuse(True, load_gbps=g), 2, 1).mean()) for g in (3.0, 6.0, 12.0, 25.0, 50.0)}
     use([host_k, host_v, host_ak, host_av])
     run.use_selector("qcfuse")
+    # time to first token: pipeline + final norm + LM head + argmax of the last query row
+    gen = torch.Generator(device=dev); gen.manual_seed(sp.seed + 7)
+    w_lm = (torch.randn((sp.vocab, sp.hidden), generator=gen, device=dev) * 0.02).to(torch.bfloat16)
+    g_fin = torch.ones(sp.hidden, device=dev, dtype=torch.bfloat16)
+    logits = torch.zeros(sp.vocab, device=dev)
+    tok = torch.zeros(1, dtype=torch.int32, device=dev)
+    hid_full = torch.zeros((run.t, sp.hidden), dtype=torch.bfloat16, device=dev)
+
+    def ttft_fuse():
+        run.fuse(True)
+        run.stack.qcf_stack_first_token(run.hidden, run.n_rows - 1, g_fin, w_lm, logits, tok)
+        return int(tok.cpu()[0])                     # the token is read back: the request's TTFT ends here
+
+    ttft_ms = timed(ttft_fuse, max(3, min(args.steps, 10)), 1)
     kc = [torch.zeros_like(k) for k in run.k_fused]
     vc = [torch.zeros_like(k) for k in run.k_fused]
     full_ms = timed(lambda: run.full_prefill(kc, vc), max(3, min(args.steps, 10)), 2)
+
+    def ttft_full():
+        run.full_prefill(kc, vc, hid_full)
+        run.stack.qcf_stack_first_token(hid_full, run.t - 1, g_fin, w_lm, logits, tok)
+        return int(tok.cpu()[0])
+
+    ttft_full_ms = timed(ttft_full, max(3, min(args.steps, 5)), 1)
     clocks = sampler.stop()
 
     fl = run.flops()
@@ -483,6 +504,7 @@ def run_c3(args) -> None:
                      "speedup_over_full_prefill": float(full_ms.mean()) / t_fuse,
                      "whole_pipeline_TFLOPps": ach, "whole_pipeline_frac_tensor_peak": ach / peak,
                      "full_prefill_TFLOPps": (fl["gemm_full"] + fl["attn_full"]) / (float(full_ms.mean()) * 1e-3) / 1e12,
+                     "ttft_ms_pinned_host": float(ttft_ms.mean()), "ttft_full_prefill_ms": float(ttft_full_ms.mean()),
                      "phase1_build_s": phase1_s, "selectors_pinned_host": selectors,
                      "pipeline_ms_vs_load_gbps": sweep},
         "e2e": {"value": sp.n_ctx / (float(e2e_ms.mean()) * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),

@@ -320,6 +320,14 @@ QCF_API qcf_status qcf_stack_layer(qcf_stack* s, int32_t layer, const qcf_batch*
                                    const int32_t* n_sel, int32_t n_rows, int32_t query_pos0, void* x, void* k_fused,
                                    void* v_fused, void* q_tap, void* stream);
 
+/* The end of time-to-first-token: the first generated token from the final hidden state of the LAST query
+ * row:   token = argmax_v ( RMSNorm(hidden[row]; g_final) . w_lm[v] ),  ties to the lower token id.
+ *   hidden : dev [rows][hidden] bf16 (hidden_out of qcf_stack_fuse: row = n_R - 1; of qcf_stack_prefill: row = T - 1)
+ *   g_final: dev [hidden] bf16;  w_lm: dev [vocab][hidden] bf16 (vocab = dims.vocab)
+ *   logits : dev [vocab] fp32, written (needed as workspace);  token : dev [1] int32 */
+QCF_API qcf_status qcf_stack_first_token(qcf_stack* s, const void* hidden, int32_t row, const void* g_final, const void* w_lm,
+                                         float* logits, int32_t* token, void* stream);
+
 /* The whole online pipeline of Fig. 9 for one request.
  *   stage 1  for l = 0..max(L*): load anchor pool l, stitch (a1'), run U through layer l over the anchor cache
  *            (Eq. 17); for l in L*: load PIC pool l, stitch (a1), score (a2, Eq. 18/20); then top-k (a3, Eq. 11)

@@ -224,3 +224,13 @@ def fuse_stage(x_rows0: np.ndarray, sel: np.ndarray, n_ctx: int, k_pic, v_pic, l
         k_ctx, v_ctx = O.reposition(k_pic[l], v_pic[l], cfg.rope_theta)
         x = fuse_layer(x, rows, len(sel), k_ctx, v_ctx, w, cfg)["x"]
     return (x, hid) if return_hidden else x
+
+
+# --------------------------------------------------------------------------- first token (end of TTFT)
+
+
+def first_token(x_last: np.ndarray, g_final: np.ndarray, w_lm: np.ndarray, eps: float):
+    """The first generated token (TTFT) from the final hidden state of the last query row:
+    logits = RMSNorm(x_last; g_final) W_lm^T, token = argmax (ties to the lower id).  Returns (token, logits)."""
+    logits = linear(rms_norm(np.asarray(x_last, dtype=np.float64), g_final, eps), w_lm)
+    return int(np.argmax(logits)), logits

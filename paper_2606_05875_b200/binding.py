@@ -22,7 +22,7 @@ EXPORTS = (
     "qcf_create", "qcf_destroy", "qcf_last_error", "qcf_version", "qcf_batch_create", "qcf_batch_destroy",
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms",
-    "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse",
+    "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
 )
 
 QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
@@ -119,6 +119,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_stack_prefill": (i32, [vp, vp, vp, C.POINTER(vp), C.POINTER(vp), vp, vp]),
         "qcf_stack_layer": (i32, [vp, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp]),
         "qcf_stack_fuse": (i32, [vp, vp, vp, C.POINTER(qcf_fuse_args), vp]),
+        "qcf_stack_first_token": (i32, [vp, vp, i32, vp, vp, vp, vp, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(lib, name)
@@ -330,6 +331,10 @@ class Stack:
         self.ctx._check(self.lib.qcf_stack_layer(self.handle, layer, b.handle, _ptr(sel), _ptr(n_sel), n_rows,
                                                  query_pos0, _ptr(x), _ptr(k_fused), _ptr(v_fused), _ptr(q_tap),
                                                  _stream(stream)))
+
+    def qcf_stack_first_token(self, hidden, row: int, g_final, w_lm, logits, token, stream=None):
+        self.ctx._check(self.lib.qcf_stack_first_token(self.handle, _ptr(hidden), int(row), _ptr(g_final), _ptr(w_lm),
+                                                       _ptr(logits), _ptr(token), _stream(stream)))
 
     def qcf_stack_fuse(self, main: Batch, probe: Batch, *, k_pic, v_pic, pool_rows: int, k_anchor, v_anchor,
                        anchor_rows: int, crit_layers, ratio: float, tokens, k_fused, v_fused, scores, sel, n_sel,

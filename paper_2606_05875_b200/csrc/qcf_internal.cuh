@@ -129,6 +129,8 @@ int attn_ptc_slots(const qcf_ctx*);
 size_t attn_ptc_slot_bytes(const qcf_ctx*);
 cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
                         __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
+cudaError_t launch_lm_head(const qcf_ctx*, const __nv_bfloat16* w_lm, const __nv_bfloat16* h, int vocab, int hidden, float* logits,
+                           int32_t* token, cudaStream_t);
 cudaError_t launch_stamp(unsigned long long* t0, cudaStream_t);
 cudaError_t launch_hold(const unsigned long long* t0, unsigned long long budget_ns, cudaStream_t);
 cudaError_t launch_rope_table(float2* table, int n_pos, int d, double theta, cudaStream_t);

@@ -217,6 +217,21 @@ qcf_status qcf_stack_layer(qcf_stack* s, int32_t layer, const qcf_batch* b, cons
                    static_cast<cudaStream_t>(stream));
 }
 
+qcf_status qcf_stack_first_token(qcf_stack* s, const void* hidden, int32_t row, const void* g_final, const void* w_lm,
+                                 float* logits, int32_t* token, void* stream) {
+  if (!s) return set_error(nullptr, QCF_ERR_INVALID_ARG, "qcf_stack_first_token: stack is NULL");
+  qcf_ctx* ctx = s->ctx;
+  STK_REQUIRE(ctx, hidden && g_final && w_lm && logits && token, "qcf_stack_first_token: NULL argument");
+  STK_REQUIRE(ctx, row >= 0, "qcf_stack_first_token: row must be >= 0");
+  STK_REQUIRE(ctx, aligned16(hidden) && aligned16(g_final) && aligned16(w_lm), "qcf_stack_first_token: pointers must be 16-byte aligned");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int hid = s->dims.hidden;
+  const __nv_bfloat16* x = static_cast<const __nv_bfloat16*>(hidden) + static_cast<size_t>(row) * hid;
+  STK_CUDA(ctx, launch_rmsnorm(x, static_cast<const __nv_bfloat16*>(g_final), s->dims.rms_eps, 1, hid, s->h, st));
+  STK_CUDA(ctx, launch_lm_head(ctx, static_cast<const __nv_bfloat16*>(w_lm), s->h, s->dims.vocab, hid, logits, token, st));
+  return QCF_OK;
+}
+
 qcf_status qcf_stack_prefill(qcf_stack* s, const qcf_batch* b, const int32_t* tokens, void* const* k_cache,
                              void* const* v_cache, void* hidden_out, void* stream) {
   if (qcf_status e = check_stack_batch(s, b, "qcf_stack_prefill")) return e;

@@ -159,6 +159,58 @@ __global__ void __launch_bounds__(256) anchor_score_kernel(BatchDev bd, int row_
   }
 }
 
+// First generated token (the end of TTFT): logits[v] = h . W_lm[v] for one normalised hidden row — a 268 MB
+// weight stream at config 3, one warp per vocabulary row, 128-bit loads, h held in shared memory — then an argmax with ties
+// to the lower token id.
+__global__ void __launch_bounds__(256) lm_head_kernel(const uint4* __restrict__ w, const uint4* __restrict__ h, int vocab,
+                                                      int row_vec, float* __restrict__ logits) {
+  extern __shared__ uint4 s_h[];
+  for (int i = threadIdx.x; i < row_vec; i += blockDim.x) s_h[i] = h[i];
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  for (int v = blockIdx.x * 8 + (threadIdx.x >> 5); v < vocab; v += gridDim.x * 8) {
+    const uint4* src = w + static_cast<size_t>(v) * row_vec;
+    float acc = 0.f;
+    for (int i = lane; i < row_vec; i += 32) {
+      const uint4 a = ld_nc_v4(src + i), b = s_h[i];
+      const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { acc = fmaf(bf16lo(aw[k]), bf16lo(bw[k]), acc); acc = fmaf(bf16hi(aw[k]), bf16hi(bw[k]), acc); }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) logits[v] = acc;
+  }
+}
+__global__ void __launch_bounds__(1024) argmax_kernel(const float* __restrict__ logits, int vocab, int32_t* __restrict__ token) {
+  __shared__ float s_v[32];
+  __shared__ int s_i[32];
+  float best = -INFINITY;
+  int idx = 0x7fffffff;
+  for (int v = threadIdx.x; v < vocab; v += blockDim.x) {
+    const float x = __ldcg(logits + v);
+    if (x > best || (x == best && v < idx)) { best = x; idx = v; }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, idx, o);
+    if (ob > best || (ob == best && oi < idx)) { best = ob; idx = oi; }
+  }
+  if ((threadIdx.x & 31) == 0) { s_v[threadIdx.x >> 5] = best; s_i[threadIdx.x >> 5] = idx; }
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    best = s_v[threadIdx.x]; idx = s_i[threadIdx.x];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+      const int oi = __shfl_xor_sync(0xffffffffu, idx, o);
+      if (ob > best || (ob == best && oi < idx)) { best = ob; idx = oi; }
+    }
+    if (threadIdx.x == 0) *token = idx;
+  }
+}
+
 // Bandwidth emulation for the loader stream: stamp the start of a load, then hold the stream until `budget_ns` have
 // elapsed since the stamp (the copy itself runs in between; if it took longer, no wait).
 __global__ void stamp_kernel(unsigned long long* t0) {
@@ -182,6 +234,19 @@ cudaError_t launch_anchor_scores(const qcf_ctx* ctx, const qcf_batch* b, const _
   if (b->batch == 0 || b->n_stride == 0) return cudaSuccess;
   anchor_score_kernel<<<dim3((b->n_stride + 7) / 8, b->batch), 256, 0, stream>>>(
       b->dev, ctx->lay.hkv * ctx->lay.d / 8, reinterpret_cast<const uint4*>(k_pool), rule, accumulate, scores);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_lm_head(const qcf_ctx* ctx, const __nv_bfloat16* w_lm, const __nv_bfloat16* h, int vocab, int hidden,
+                           float* logits, int32_t* token, cudaStream_t stream) {
+  if (vocab <= 0) return cudaSuccess;
+  int blocks = (vocab + 7) / 8;
+  if (blocks > ctx->n_sm * 8) blocks = ctx->n_sm * 8;
+  lm_head_kernel<<<blocks, 256, static_cast<size_t>(hidden) * 2, stream>>>(reinterpret_cast<const uint4*>(w_lm),
+                                                                           reinterpret_cast<const uint4*>(h), vocab, hidden / 8, logits);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  argmax_kernel<<<1, 1024, 0, stream>>>(logits, vocab, token);
   return cudaGetLastError();
 }
 

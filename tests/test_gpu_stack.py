@@ -487,3 +487,31 @@ def test_stack_layer_full_size_c3_sampled():
     want = S.layer_finish(x_in[samp], a, w, cfg)
     err = _rel_rms_err(_f64(x)[samp], want)
     assert err <= 3e-2, err
+
+
+def test_first_token_parity():
+    """End of TTFT: RMSNorm + LM head + argmax of the last query row against the oracle.  The decision is an integer taken
+    from fp32 logits: exact where the oracle's top-2 gap exceeds the logit tolerance, else the chosen token must be within it."""
+    binding = _binding()
+    wl, ctx, stack = _make("s_d128")
+    sp = wl.spec
+    rng = np.random.default_rng(12)
+    rows = 37
+    hid_bits = inputs.f32_to_bf16_bits(rng.standard_normal((rows, sp.hidden), dtype=np.float32) * np.float32(3.0))
+    g_bits = inputs.f32_to_bf16_bits(np.float32(1.0) + np.float32(0.1) * rng.standard_normal(sp.hidden, dtype=np.float32))
+    w_bits = inputs.f32_to_bf16_bits(rng.standard_normal((sp.vocab, sp.hidden), dtype=np.float32) * np.float32(0.05))
+    logits = torch.zeros(sp.vocab, device="cuda")
+    token = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+    stack.qcf_stack_first_token(_dev(hid_bits), rows - 1, _dev(g_bits), _dev(w_bits), logits, token)
+    torch.cuda.synchronize()
+    tok, want = S.first_token(O.widen_bf16(hid_bits[rows - 1]), O.widen_bf16(g_bits), O.widen_bf16(w_bits), sp.rms_eps)
+    got = logits.cpu().numpy().astype(np.float64)
+    tol = 2e-2 * max(1.0, np.abs(want).max())               # h is rounded to bf16 on the GPU (2^-9 relative per term)
+    assert np.max(np.abs(got - want)) <= tol
+    t = int(token[0])
+    assert t == int(np.argmax(logits.cpu().numpy())), "argmax of its own logits, ties to the lower id"
+    top2 = np.sort(want)[-2:]
+    if top2[1] - top2[0] > 2 * tol:
+        assert t == tok
+    else:
+        assert want[t] >= top2[1] - 2 * tol

@@ -207,3 +207,15 @@ def test_probe_uses_only_anchor_rows_and_original_positions():
     q0 = O.rotate(q, -phi)
     xhat = q0 / layers[1].g_q
     np.testing.assert_allclose(np.sqrt(np.mean(xhat ** 2, -1)), 1.0, rtol=1e-4)
+
+
+def test_first_token_matches_torch_and_argmax_ties():
+    rng = np.random.default_rng(8)
+    x = rng.standard_normal(48); g = 1 + 0.1 * rng.standard_normal(48); w = rng.standard_normal((33, 48))
+    tok, logits = S.first_token(x, g, w, 1e-6)
+    t = torch.from_numpy
+    want = F.linear(F.rms_norm(t(x), (48,), t(g), 1e-6), t(w)).numpy()
+    np.testing.assert_allclose(logits, want, rtol=1e-12, atol=1e-13)
+    assert tok == int(np.argmax(want))
+    w2 = w.copy(); w2[7] = w2[tok]                      # an exact tie: the lower id wins
+    assert S.first_token(x, g, w2, 1e-6)[0] == min(7, tok)
