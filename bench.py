@@ -300,7 +300,9 @@ def run_qcf(args) -> None:
         e2e_s = (time.perf_counter() - t0) / n_e2e
         nb = lambda t: t.numel() * t.element_size()
         h2d = nb(hw.k_pool) + nb(hw.v_pool) + nb(hw.q_probe) + nb(hw.q_new) + nb(hw.k_new) + nb(hw.v_new)
-        d2h = nb(hw.out) + nb(hw.sel) + nb(hw.n_sel) + nb(hw.scores)
+        q_row_b = cfg.n_q_heads * cfg.head_dim * 2
+        out_rows = sum(binding.qcf_n_select(n, cfg.ratio) + lq for n, lq in zip(hw.batch.n_ctx, hw.batch.n_query))
+        d2h = out_rows * q_row_b + nb(hw.sel) + nb(hw.n_sel) + nb(hw.scores)      # only the |R_b| written rows of `out` come back
         e2e = (e2e_s, h2d, d2h, n_e2e)
     clocks = sampler.stop() if rank == 0 else None
 

@@ -240,7 +240,7 @@ typedef struct {
 QCF_API qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* args, void* stream);
 
 /* Same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe
- * and fresh rows, runs qcf_layer_step on the context's internal device buffers, downloads `out`, `sel`,
+ * and fresh rows, runs qcf_layer_step on the context's internal device buffers, downloads the |R_b| written rows of `out`, `sel`,
  * `n_sel` (and the fused cache if k_fused / v_fused are non-NULL), and synchronises `stream` before
  * returning.  Pointer fields of `host` are host pointers with the same shapes; `pool_rows` is the number of
  * rows of host->k_pool / v_pool.  Device staging buffers are allocated on first use and kept by the ctx. */

@@ -1,5 +1,6 @@
 // C ABI of libqcf (include/qcf.h): context / batch lifetime, host-side argument validation, stage chaining.
 // Everything that touches tensor data runs in the CUDA kernels of the sibling translation units.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -534,7 +535,16 @@ qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer
   d.lse = h->lse ? static_cast<float*>(S.lse.p) : nullptr;
   if (qcf_status st = qcf_layer_step(ctx, b, &d, stream)) return st;
 
-  QCF_CUDA(ctx, cudaMemcpyAsync(h->out, S.out.p, qnew_bytes, cudaMemcpyDeviceToHost, s));
+  // only the |R_b| = k_b + Lq_b rows the step wrote are read back (k_b is known on the host: floor(rho N_b) when the step
+  // selects, the caller's n_sel otherwise)
+  for (int i = 0; i < b->batch; ++i) {
+    const int k_b = h->select_now ? qcf_n_select(b->h_n_ctx[i], h->ratio) : h->n_sel[i];
+    const size_t rows_b = static_cast<size_t>(k_b < 0 ? 0 : k_b) + b->h_n_query[i];
+    const size_t off = static_cast<size_t>(i) * b->t_stride * q_row;
+    if (rows_b > 0)
+      QCF_CUDA(ctx, cudaMemcpyAsync(static_cast<char*>(h->out) + off, static_cast<const char*>(S.out.p) + off,
+                                    std::min(rows_b, static_cast<size_t>(b->t_stride)) * q_row, cudaMemcpyDeviceToHost, s));
+  }
   QCF_CUDA(ctx, cudaMemcpyAsync(h->sel, S.sel.p, sel_bytes, cudaMemcpyDeviceToHost, s));
   QCF_CUDA(ctx, cudaMemcpyAsync(h->n_sel, S.n_sel.p, B * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
   if (h->scores && h->is_critical_layer)
