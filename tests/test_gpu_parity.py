@@ -548,3 +548,53 @@ def test_full_size_c4_batched_pool(ratio):
     torch.cuda.synchronize()
     for b in (0, 2):
         _check_full_size(wl, dw, b, 23 + b)
+
+
+# --------------------------------------------------------------------------------------------- ragged batch
+
+def test_layer_step_ragged_batch_parity():
+    """Requests of different shapes in one batch (1 / 3 / 5 chunks of 96 rows from a shared pool, Lq = 5 / 24 / 17): every
+    stage indexes through the batch strides; each request is checked against the oracle on its own."""
+    binding, _ = _binding()
+    wl = inputs.make_workload("t_batch")
+    cfg = wl.cfg
+    hq, hkv, d = cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim
+    pool_k, pool_v = np.concatenate(wl.pool_k, 0), np.concatenate(wl.pool_v, 0)
+    chunk_ids = [[3], [0, 1, 2], [4, 5, 6, 7, 8]]
+    lqs = [5, 24, 17]
+    ratio = 0.3
+    ctx = binding.Context(hq, hkv, d, cfg.rope_theta, 3, 1024, 32)
+    b = ctx.batch([[96] * len(c) for c in chunk_ids], [[96 * i for i in c] for c in chunk_ids], lqs)
+    T, Nn, Q = b.t_stride, b.n_stride, b.q_stride
+    rng = np.random.default_rng(77)
+
+    def rnd(*shape):
+        return inputs.f32_to_bf16_bits(rng.standard_normal(shape, dtype=np.float32))
+
+    qp, qn, kn, vn = rnd(3, Q, hq, d), rnd(3, T, hq, d), rnd(3, T, hkv, d), rnd(3, T, hkv, d)
+    dev = lambda bits: torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16).cuda()
+    kf = torch.zeros((3, T, hkv, d), dtype=torch.bfloat16, device="cuda")
+    vf = torch.zeros_like(kf)
+    scores = torch.zeros((3, Nn), device="cuda")
+    sel = torch.zeros((3, Nn), dtype=torch.int32, device="cuda")
+    n_sel = torch.zeros(3, dtype=torch.int32, device="cuda")
+    out = torch.zeros((3, T, hq, d), dtype=torch.bfloat16, device="cuda")
+    args = ctx.layer_args(k_pool=dev(pool_k), v_pool=dev(pool_v), k_fused=kf, v_fused=vf, q_probe=dev(qp), scores=scores,
+                          sel=sel, n_sel=n_sel, q_new=dev(qn), k_new=dev(kn), v_new=dev(vn), out=out, ratio=ratio)
+    ctx.qcf_layer_step(b, args)
+    torch.cuda.synchronize()
+    for i, ids in enumerate(chunk_ids):
+        n, lq = 96 * len(ids), lqs[i]
+        k_pic = [O.widen_bf16(wl.pool_k[c]) for c in ids]
+        v_pic = [O.widen_bf16(wl.pool_v[c]) for c in ids]
+        k = O.n_select(n, ratio)
+        assert int(n_sel[i]) == k
+        got_sel = sel[i, :k].cpu().numpy().astype(np.int64)
+        k_ctx, _ = O.reposition(k_pic, v_pic, cfg.rope_theta)
+        want_sc = O.score(O.widen_bf16(qp[i, :lq]), k_ctx)
+        np.testing.assert_allclose(scores[i, :n].cpu().numpy().astype(np.float64), want_sc, rtol=1e-2, atol=0)
+        _check_selection(got_sel, want_sc, k)
+        ref = O.layer_step(k_pic, v_pic, cfg.rope_theta, None, 0.0, O.widen_bf16(qn[i, : n + lq]), O.widen_bf16(kn[i, : n + lq]),
+                           O.widen_bf16(vn[i, : n + lq]), sel=got_sel)
+        assert np.max(np.abs(_f64(out[i, : k + lq]) - ref["out"])) <= 2e-2
+        assert np.array_equal(_f64(vf[i, : n + lq]), ref["v_fused"])
