@@ -45,6 +45,8 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 //   * splitting every item's keys over 2 / 4 CTAs (cluster + DSMEM merge, or global partials merged by the last
 //     arriver): 107 -> 127 / 158 us — at c2 the SMs are throughput-bound, a split only adds prologues and merge traffic
 //     (it does pay when the grid under-fills the machine: rho = 0, 16 items: 82 -> 53 us, hence the heuristic below);
+//   * a second CTA for only the 4-24 heaviest row tiles of each (request, kv-head) ("tail trim", partials merged through a
+//     global workspace): 82 -> 84-92 us — trimming the 81-step tail buys nothing, the SMs are throughput-bound;
 //   * a persistent work-list kernel (recompute_attn_ptc.cu).
 // Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Measured on c2: 4 -> 84 us,
 // 3 -> 91 us, 2 -> 104 us: the sweep is issue-bound, not MUFU-bound, so every exponential goes to the MUFU.
