@@ -47,6 +47,12 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 //     (it does pay when the grid under-fills the machine: rho = 0, 16 items: 82 -> 53 us, hence the heuristic below);
 //   * a second CTA for only the 4-24 heaviest row tiles of each (request, kv-head) ("tail trim", partials merged through a
 //     global workspace): 82 -> 84-92 us — trimming the 81-step tail buys nothing, the SMs are throughput-bound;
+//   * ONE CTA per SM owning two items (the same row tile for two adjacent kv-heads: 512 TMEM columns, one producer, one
+//     issuer, two softmax groups), with or without FA-style turn taking between the groups on named barriers: c5 2675 ->
+//     3320-3400 us, c2 82 -> 127 us.  A lone warp does not saturate its SMSP's MUFU (a sweep alone takes ~1500 cycles, not
+//     the 512 the unit could do), so serialising the groups halves the MUFU rate, and a shared issuer blocks one item on
+//     the other's P; two independent CTAs per SM remain the best arrangement found;
+//   * halving the K/V loads (timing experiment, wrong results): c2 unchanged, c5 -9 %: L2 -> SM traffic is not the limiter;
 //   * a persistent work-list kernel (recompute_attn_ptc.cu).
 // Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Measured on c2: 4 -> 84 us,
 // 3 -> 91 us, 2 -> 104 us: the sweep is issue-bound, not MUFU-bound, so every exponential goes to the MUFU.
