@@ -207,28 +207,39 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
 
   if (warp == 0) {
     // ===================================================================== TMA producer
-    if (lane == 0) {
-      for (int j = 0; j < n_kt; ++j) {
-        const int st = j % kStages;
-        const uint32_t ph = (j / kStages) & 1;
-        mbar_wait(bar(kEmptyK + st), ph ^ 1);
+    // The whole warp walks the loop converged and ONE ELECTED lane issues (elect.sync): inside a divergent `if (lane == 0)`
+    // the compiler cannot prove uniformity and wraps every TMA / UMMA instruction (they take uniform registers) in a
+    // per-lane ELECT / BRA.U.ANY loop with vector-to-uniform moves — ~40 SASS instructions per UMMA on the issuer's
+    // critical path (traced: ~450 cycles to issue one tile's MMAs).
+    for (int j = 0; j < n_kt; ++j) {
+      const int st = j % kStages;
+      const uint32_t ph = (j / kStages) & 1;
+      mbar_wait(bar(kEmptyK + st), ph ^ 1);
+      if (elect_one()) {
         mbar_arrive_expect_tx(bar(kFullK + st), S::kTile);
 #pragma unroll
         for (int kb = 0; kb < D / 64; ++kb)
           tma_load_4d(sK + st * S::kTile + kb * S::kBlk, &tm_k, bar(kFullK + st), kb * 64, g, (jt0 + j) * BN, b);
-        mbar_wait(bar(kEmptyV + st), ph ^ 1);
+      }
+      mbar_wait(bar(kEmptyV + st), ph ^ 1);
+      if (elect_one()) {
         mbar_arrive_expect_tx(bar(kFullV + st), S::kTile);
 #pragma unroll
         for (int kb = 0; kb < D / 64; ++kb)
           tma_load_4d(sV + st * S::kTile + kb * S::kBlk, &tm_v, bar(kFullV + st), kb * 64, g, (jt0 + j) * BN, b);
       }
+      __syncwarp();
     }
-    __syncwarp();
   } else if (warp == 1) {
     // ===================================================================== UMMA issuer
-    if (lane == 0) {
+    {
+      // converged warp, one elected lane issues (see the producer)
       constexpr uint32_t idesc_qk = umma_idesc_bf16(BM, BN, false, false);
       constexpr uint32_t idesc_pv = umma_idesc_bf16(BM, D, false, true);
+      // base descriptors once; a tile's descriptors are base + (byte offset >> 4) (the start-address field is in 16-byte
+      // units and shared memory is far below its 256 KB range, so the add never carries out of the field)
+      const uint64_t dq = umma_smem_desc_sw128(sQ, 16, 1024), dk = umma_smem_desc_sw128(sK, 16, 1024);
+      const uint64_t dv = umma_smem_desc_sw128(sV, S::kBlk, 1024);
       auto issue_qk = [&](int j) {
         const int st = j % kStages;
         mbar_wait(bar(kFullK + st), (j / kStages) & 1);
@@ -236,14 +247,16 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         // S_j overwrites the buffer of S_{j-2} / P_{j-2}: P_{j-2} V_{j-2} was issued earlier and UMMAs of one CTA
         // execute in issue order; the softmax warps finished reading S_{j-2} before they signalled P_{j-2}.
         const uint32_t d_tmem = tmem_base + (j & 1) * BN;
+        if (elect_one()) {
+          const uint64_t dk_st = dk + static_cast<uint64_t>((st * S::kTile) >> 4);
 #pragma unroll
-        for (int ks = 0; ks < D / 16; ++ks) {
-          umma_ss(d_tmem, umma_smem_desc_sw128(sQ + (ks >> 2) * S::kQBlk + (ks & 3) * 32, 16, 1024),
-                  umma_smem_desc_sw128(sK + st * S::kTile + (ks >> 2) * S::kBlk + (ks & 3) * 32, 16, 1024), idesc_qk,
-                  ks > 0 ? 1u : 0u);
+          for (int ks = 0; ks < D / 16; ++ks)
+            umma_ss(d_tmem, dq + static_cast<uint64_t>(((ks >> 2) * S::kQBlk + (ks & 3) * 32) >> 4),
+                    dk_st + static_cast<uint64_t>(((ks >> 2) * S::kBlk + (ks & 3) * 32) >> 4), idesc_qk, ks > 0 ? 1u : 0u);
+          umma_commit(bar(kEmptyK + st));
+          umma_commit(bar(kSFull + (j & 1)));
         }
-        umma_commit(bar(kEmptyK + st));
-        umma_commit(bar(kSFull + (j & 1)));
+        __syncwarp();
       };
       mbar_wait(bar(kQFull), 0);
       tc_fence_after();
@@ -254,16 +267,18 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
         mbar_wait(bar(kPReady + (j & 1)), (j >> 1) & 1);
         mbar_wait(bar(kFullV + st), (j / kStages) & 1);
         tc_fence_after();
+        if (elect_one()) {
+          const uint64_t dv_st = dv + static_cast<uint64_t>((st * S::kTile) >> 4);
 #pragma unroll
-        for (int ks = 0; ks < BN / 16; ++ks)
-          umma_ts(tmem_o, tmem_base + (j & 1) * BN + ks * 8,
-                  umma_smem_desc_sw128(sV + st * S::kTile + ks * 2048, S::kBlk, 1024), idesc_pv,
-                  (j > 0 || ks > 0) ? 1u : 0u);
-        umma_commit(bar(kEmptyV + st));
-        umma_commit(bar(kODone + (j & 1)));
+          for (int ks = 0; ks < BN / 16; ++ks)
+            umma_ts(tmem_o, tmem_base + (j & 1) * BN + ks * 8, dv_st + static_cast<uint64_t>((ks * 2048) >> 4), idesc_pv,
+                    (j > 0 || ks > 0) ? 1u : 0u);
+          umma_commit(bar(kEmptyV + st));
+          umma_commit(bar(kODone + (j & 1)));
+        }
+        __syncwarp();
       }
     }
-    __syncwarp();
   } else {
     // ===================================================================== softmax / correction / epilogue
     const int quarter = warp & 3;
