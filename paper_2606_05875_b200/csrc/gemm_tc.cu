@@ -86,26 +86,32 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
 
   if (warp == 0) {
     // ===================================================================== TMA producer
-    if (lane == 0) {
+    // Converged warp, one ELECTED lane issues (elect.sync): inside a divergent `if (lane == 0)` every TMA / UMMA instruction
+    // (they take uniform registers) is wrapped in a per-lane ELECT / BRA.U.ANY loop with vector-to-uniform moves.
+    {
       int it = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         const int m0 = (t % n_mblk) * BM, n0 = (t / n_mblk) * BN;
         for (int kb = 0; kb < n_kb; ++kb, ++it) {
           const int st = it % S::kStages;
           mbar_wait(bar(kEmpty + st), ((it / S::kStages) & 1) ^ 1);
-          mbar_arrive_expect_tx(bar(kFull + st), S::kStage);
-          const uint32_t sa = sbase + st * S::kStage;
+          if (elect_one()) {
+            mbar_arrive_expect_tx(bar(kFull + st), S::kStage);
+            const uint32_t sa = sbase + st * S::kStage;
 #pragma unroll
-          for (int mt = 0; mt < MT; ++mt) tma_load_2d(sa + mt * (128 * BK * 2), &tm_a, bar(kFull + st), kb * BK, m0 + mt * 128);
-          tma_load_2d(sa + S::kA, &tm_w, bar(kFull + st), kb * BK, n0);
+            for (int mt = 0; mt < MT; ++mt) tma_load_2d(sa + mt * (128 * BK * 2), &tm_a, bar(kFull + st), kb * BK, m0 + mt * 128);
+            tma_load_2d(sa + S::kA, &tm_w, bar(kFull + st), kb * BK, n0);
+          }
+          __syncwarp();
         }
       }
     }
-    __syncwarp();
   } else if (warp == 1) {
-    // ===================================================================== UMMA issuer
-    if (lane == 0) {
+    // ===================================================================== UMMA issuer (converged warp, elected lane)
+    {
       constexpr uint32_t idesc = umma_idesc_bf16(128, BN, false, false);
+      // base descriptor once; a stage's operands are base + (byte offset >> 4) (16-byte units, no carry out of the field)
+      const uint64_t d0 = umma_smem_desc_sw128(sbase, 16, 1024);
       int it = 0, tile_i = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++tile_i) {
         const int buf = tile_i % kAccBufs;
@@ -115,21 +121,23 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
           const int st = it % S::kStages;
           mbar_wait(bar(kFull + st), (it / S::kStages) & 1);
           tc_fence_after();
-          const uint32_t sa = sbase + st * S::kStage, sb = sa + S::kA;
+          if (elect_one()) {
+            const uint64_t da = d0 + static_cast<uint64_t>((st * S::kStage) >> 4), db = da + static_cast<uint64_t>(S::kA >> 4);
 #pragma unroll
-          for (int mt = 0; mt < MT; ++mt) {
-            const uint32_t d_tmem = tmem_base + (buf * MT + mt) * BN;
+            for (int mt = 0; mt < MT; ++mt) {
+              const uint32_t d_tmem = tmem_base + (buf * MT + mt) * BN;
 #pragma unroll
-            for (int ks = 0; ks < BK / 16; ++ks)
-              umma_ss(d_tmem, umma_smem_desc_sw128(sa + mt * (128 * BK * 2) + ks * 32, 16, 1024),
-                      umma_smem_desc_sw128(sb + ks * 32, 16, 1024), idesc, (kb > 0 || ks > 0) ? 1u : 0u);
+              for (int ks = 0; ks < BK / 16; ++ks)
+                umma_ss(d_tmem, da + static_cast<uint64_t>((mt * (128 * BK * 2) + ks * 32) >> 4), db + static_cast<uint64_t>((ks * 32) >> 4),
+                        idesc, (kb > 0 || ks > 0) ? 1u : 0u);
+            }
+            umma_commit(bar(kEmpty + st));
+            if (kb == n_kb - 1) umma_commit(bar(kAccFull + buf));
           }
-          umma_commit(bar(kEmpty + st));
+          __syncwarp();
         }
-        umma_commit(bar(kAccFull + buf));
       }
     }
-    __syncwarp();
   } else {
     // ===================================================================== epilogue: thread = one output row
     const int ew = warp - 2;                        // 0..7

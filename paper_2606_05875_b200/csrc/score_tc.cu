@@ -135,25 +135,34 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
 
   if (warp == 0) {
     // ===================================================================== producer
-    if (n_j > 0 && lane == 0) {
+    // converged warp, one ELECTED lane issues: a divergent `if (lane == 0)` makes the compiler wrap every TMA / UMMA
+    // instruction (uniform-register operands) in a per-lane ELECT / BRA.U.ANY loop
+    if (n_j > 0) {
       for (int kt = 0, it = 0; kt < n_kt; ++kt) {
         if (kt > 0) mbar_wait(bar(kAEmpty), (kt - 1) & 1);      // every MMA that read the previous A tile has completed
-        mbar_arrive_expect_tx(bar(kAFull), S::kTile);
-        if (PASS == 1) load_q_tile(sA, bar(kAFull), row_tile); else load_k_tile(sA, bar(kAFull), (key_tile + kt) * BT);
+        if (elect_one()) {
+          mbar_arrive_expect_tx(bar(kAFull), S::kTile);
+          if (PASS == 1) load_q_tile(sA, bar(kAFull), row_tile); else load_k_tile(sA, bar(kAFull), (key_tile + kt) * BT);
+        }
+        __syncwarp();
         for (int j = 0; j < n_j; ++j, ++it) {
           const int st = it & 1;
           mbar_wait(bar(kBEmpty + st), ((it >> 1) & 1) ^ 1);
-          mbar_arrive_expect_tx(bar(kBFull + st), S::kTile);
-          if (PASS == 1) load_k_tile(sB + st * S::kTile, bar(kBFull + st), k_begin + j * BT);
-          else load_q_tile(sB + st * S::kTile, bar(kBFull + st), j);
+          if (elect_one()) {
+            mbar_arrive_expect_tx(bar(kBFull + st), S::kTile);
+            if (PASS == 1) load_k_tile(sB + st * S::kTile, bar(kBFull + st), k_begin + j * BT);
+            else load_q_tile(sB + st * S::kTile, bar(kBFull + st), j);
+          }
+          __syncwarp();
         }
       }
     }
-    __syncwarp();
   } else if (warp == 1) {
-    // ===================================================================== UMMA issuer
-    if (lane == 0 && n_j > 0) {
+    // ===================================================================== UMMA issuer (converged warp, elected lane)
+    if (n_j > 0) {
       constexpr uint32_t idesc = umma_idesc_bf16(BT, BT, false, false);
+      // base descriptors once; a k-step's operands are base + (byte offset >> 4) (16-byte units, no carry out of the field)
+      const uint64_t da0 = umma_smem_desc_sw128(sA, 16, 1024), db0 = umma_smem_desc_sw128(sB, 16, 1024);
       for (int kt = 0, it = 0; kt < n_kt; ++kt) {
         mbar_wait(bar(kAFull), kt & 1);
         for (int j = 0; j < n_j; ++j, ++it) {
@@ -162,19 +171,21 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           mbar_wait(bar(kSEmpty + st), ph ^ 1);               // consumers have released the S buffer used two steps ago
           mbar_wait(bar(kBFull + st), ph);
           tc_fence_after();
+          if (elect_one()) {
+            const uint64_t db = db0 + static_cast<uint64_t>((st * S::kTile) >> 4);
 #pragma unroll
-          for (int ks = 0; ks < D / 16; ++ks) {
-            const uint32_t koff = (ks >> 2) * S::kBlk + (ks & 3) * 32;
-            umma_ss(tmem_base + st * BT, umma_smem_desc_sw128(sA + koff, 16, 1024),
-                    umma_smem_desc_sw128(sB + st * S::kTile + koff, 16, 1024), idesc, ks > 0 ? 1u : 0u);
+            for (int ks = 0; ks < D / 16; ++ks) {
+              const uint64_t koff = static_cast<uint64_t>(((ks >> 2) * S::kBlk + (ks & 3) * 32) >> 4);
+              umma_ss(tmem_base + st * BT, da0 + koff, db + koff, idesc, ks > 0 ? 1u : 0u);
+            }
+            umma_commit(bar(kBEmpty + st));
+            umma_commit(bar(kSFull + st));
+            if (j == n_j - 1) umma_commit(bar(kAEmpty));
           }
-          umma_commit(bar(kBEmpty + st));
-          umma_commit(bar(kSFull + st));
+          __syncwarp();
         }
-        umma_commit(bar(kAEmpty));
       }
     }
-    __syncwarp();
   } else {
     // ===================================================================== consumers: one TMEM lane each
     const int quarter = warp & 3;
