@@ -2,7 +2,7 @@
 // the fused cache, as a warp-specialised tcgen05 / TMEM / TMA kernel.
 //
 //   tile      : 128 MMA rows = 128/G consecutive rows of R (ascending positions) x the G query heads of one kv-head,
-//               against key tiles of 128 positions of that kv-head (K/V fetched once serve all G heads)
+//               against key tiles of 64 positions of that kv-head (K/V fetched once serve all G heads)
 //   warp 0    : TMA producer — K and V tiles (4-D tensor maps over [B][T][Hkv][d], 128-byte swizzle) into 2-stage rings
 //   warp 1    : UMMA issuer  — S[j] = Q K_j^T (SS, fp32 in TMEM, double-buffered), O += P_j V_j (TS: P read from TMEM,
 //               V as an MN-major smem operand); S[j+1] is issued before P_j V_j so the softmax of tile j overlaps it
@@ -53,7 +53,18 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 //     the 512 the unit could do), so serialising the groups halves the MUFU rate, and a shared issuer blocks one item on
 //     the other's P; two independent CTAs per SM remain the best arrangement found;
 //   * halving the K/V loads (timing experiment, wrong results): c2 unchanged, c5 -9 %: L2 -> SM traffic is not the limiter;
-//   * a persistent work-list kernel (recompute_attn_ptc.cu).
+//   * a persistent work-list kernel (recompute_attn_ptc.cu);
+//   * S = Q K^T for PAIRS of key tiles as one 128 x 128 x 16 chain into a single 128-column S buffer (the TMEM budget of two
+//     CTAs per SM leaves no room to double-buffer it): c2 75.8 -> 90.1 us, c5 2.51 -> 2.90 ms — the serialised
+//     QK -> softmax -> PV chain costs more than the cheaper MMA saves;
+//   * pairing the heaviest tile of the first block round with the lightest of the second (equal pair sums): 75.8 -> 74.9 us.
+// What bounds it (microbenchmarks + knock-outs): a 128 x 64 x 16 SS MMA takes ~57 cycles, not the 32
+// its flops need (the 4 KB A read from shared memory; N = 128: 67, N = 256: 128, TS N = 128: 64), so one 64-key step is
+// 624 cycles of tensor pipe (8 SS + 4 TS), 82 % of peak at best.  A skeleton of this loop (MMAs and barrier handshakes
+// only) runs AT that floor with two CTAs per SM (607-631 cycles per step) and at 770-925 alone; the full kernel with the
+// loads, the exponentials and the S loads removed still takes 75.3 of its 75.8 us at c2: the step is bound by the tensor
+// pipe shared between the two CTAs plus ~0.1 us of sweep ALU work and ring barriers per CTA step, and the launch by the
+// heaviest tile's 81-step chain (3.3 us prologue + 81 x 0.80 us).
 // Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Measured on c2: 4 -> 84 us,
 // 3 -> 91 us, 2 -> 104 us: the sweep is issue-bound, not MUFU-bound, so every exponential goes to the MUFU.
 constexpr int kMufuPairs = QCF_ATTN_MUFU_PAIRS;
