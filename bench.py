@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--impl", default="qcf", choices=["qcf", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shard", default="requests", choices=["requests", "heads"],
+                    help="requests: one replica per rank, no collective (default, weak scaling); heads: ONE request set split "
+                         "over the ranks by kv-head groups with an all-reduce of the scores (strong scaling)")
     return ap.parse_args()
 
 
@@ -370,6 +373,73 @@ def run_qcf(args) -> None:
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------ kv-head shards
+
+def run_head_sharded(args) -> None:
+    """the step of ONE request set split over the ranks by kv-head groups
+    (paper_2606_05875_b200/sharded.py).  Strong scaling: total work is fixed, the only exchange is the all-reduce(sum) of
+    scores[B][n_stride] between a2 and the replicated a3.  Not the default arm (requests are independent: replicas)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_05875_b200 import device, inputs, sharded
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the qcf arm has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    wl = inputs.make_workload(args.workload, ratio=args.ratio)
+    cfg = wl.cfg
+    st = sharded.HeadShardedStep(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, max(cfg.batch, 1),
+                                 max(cfg.n_ctx, 1024), max(cfg.n_query, 1), rank=rank, world=world)
+    dw = device.DeviceWorkload(inputs.shard_heads(wl, rank, world), st.ctx, device=dev)
+    kw = dict(k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused, q_probe=dw.q_probe,
+              scores=dw.scores, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new, out=dw.out,
+              ratio=cfg.ratio)
+    flush_w = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    flush_r = torch.zeros(64 << 20, dtype=torch.int32, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        st.layer_step(dw.batch, **kw)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for i in range(args.steps):
+        flush_w.fill_(i & 0xff)
+        flush_r.max()
+        ev[i][0].record()
+        st.layer_step(dw.batch, **kw)
+        ev[i][1].record()
+    barrier()
+    total_ms = float(sum(a.elapsed_time(b) for a, b in ev))
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms, = max_over_ranks([total_ms], dist if world > 1 else None, dev)
+    if rank == 0:
+        ms = total_ms / args.steps
+        line = {"metric": METRIC, "value": int(dw.batch.total_ctx) / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": dict(config_dict(wl, args, l2="flushed before every timed step"),
+                               parallelism="kv-head shards x%d, all-reduce(sum) of scores (%d B) per step" %
+                                           (world, dw.scores.numel() * 4)),
+                "clocks": clocks, "gpu_launches": KERNELS_PER_STEP * args.steps}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 # ------------------------------------------------------------------------------------------------ config 3 (full stack)
 
 C3_METRIC = "fused context tokens/s through the whole stack at r=0.3 (config 3: stage 1 + 36-layer stage 2)"
@@ -572,6 +642,8 @@ def main():
         run_c3(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.shard == "heads":
+        run_head_sharded(args)
     else:
         run_qcf(args)
 

@@ -148,6 +148,15 @@ QCF_API qcf_status qcf_rope_reposition(qcf_ctx* ctx, const qcf_batch* b, const v
 QCF_API qcf_status qcf_score(qcf_ctx* ctx, const qcf_batch* b, const void* q_probe, const void* k_fused,
                              float* scores, int32_t accumulate, void* stream);
 
+/* KV-head-sharded step: the heads of a layer are independent for a1, a4 and a5, and a2
+ * is a SUM over heads (Eq. 18), so a layer can be split over n_shards ranks, each with a ctx created for Hq/n_shards
+ * query heads and Hkv/n_shards kv-heads and holding those heads' slices of every tensor.  After this call qcf_score on
+ * this ctx divides by (Hq * n_shards) * Lq, i.e. it returns the rank's PARTIAL of Eq. 18 over all heads of the layer:
+ * the element-wise sum of the ranks' score arrays (one all-reduce of [B][n_stride] fp32 — or, on one device,
+ * qcf_score with accumulate != 0 on the same array) is I(t).  qcf_select_topk then runs replicated on the summed
+ * scores, so every rank selects the same P.  n_shards in [1, 64]; 1 (the default) restores the plain behaviour. */
+QCF_API qcf_status qcf_set_head_shards(qcf_ctx* ctx, int32_t n_shards);
+
 /* ------------------------------------------------------------------------------------------------ a3 */
 
 /* Eq. 11: per request, the k_b = qcf_n_select(N_b, ratio) context positions with the

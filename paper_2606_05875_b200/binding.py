@@ -21,7 +21,7 @@ _STATUS = {0: "QCF_OK", 1: "QCF_ERR_INVALID_ARG", 2: "QCF_ERR_UNSUPPORTED", 3: "
 EXPORTS = (
     "qcf_create", "qcf_destroy", "qcf_last_error", "qcf_version", "qcf_batch_create", "qcf_batch_destroy",
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
-    "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms",
+    "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards",
     "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
 )
 
@@ -110,6 +110,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_layer_step": (i32, [vp, vp, C.POINTER(qcf_layer_args), vp]),
         "qcf_layer_step_host": (i32, [vp, vp, C.POINTER(qcf_layer_args), i64, vp]),
         "qcf_set_profiling": (i32, [vp, i32]),
+        "qcf_set_head_shards": (i32, [vp, i32]),
         "qcf_get_stage_ms": (i32, [vp, C.POINTER(C.c_float)]),
         "qcf_anchor_rank": (i32, [vp, vp, vp, i32, f64, vp, i32, i32, vp, vp, vp]),
         "qcf_linear": (i32, [vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]),
@@ -275,6 +276,9 @@ class Context:
 
     def qcf_layer_step_host(self, b: Batch, args: qcf_layer_args, pool_rows: int, stream=None):
         self._check(self.lib.qcf_layer_step_host(self.handle, b.handle, C.byref(args), int(pool_rows), _stream(stream)))
+
+    def qcf_set_head_shards(self, n_shards: int):
+        self._check(self.lib.qcf_set_head_shards(self.handle, int(n_shards)))
 
     def qcf_set_profiling(self, enable: bool):
         self._check(self.lib.qcf_set_profiling(self.handle, int(bool(enable))))

@@ -145,6 +145,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
     const int cl = e3 ? std::atoi(e3) : 0;
     c->attn_cluster = (cl == 1 || cl == 2 || cl == 4) ? cl : 0;
     c->ratio_hint = 0.3;
+    c->head_shards = 1;
   }
   c->profiling = 0; c->ev_valid = false;
   c->ev_ring = nullptr; c->ev_count = 0; c->ev = nullptr;
@@ -446,6 +447,13 @@ qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args
     ctx->ev_count++;
   }
   ctx->ev_valid = false;
+  return QCF_OK;
+}
+
+qcf_status qcf_set_head_shards(qcf_ctx* ctx, int32_t n_shards) {
+  if (!ctx) return QCF_ERR_INVALID_ARG;
+  if (n_shards < 1 || n_shards > 64) return fail(ctx, QCF_ERR_INVALID_ARG, "n_shards must be in [1, 64]");
+  ctx->head_shards = n_shards;
   return QCF_OK;
 }
 

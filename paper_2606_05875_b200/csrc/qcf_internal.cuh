@@ -52,6 +52,7 @@ struct qcf_ctx {
   int pdl;               // 1: chain the step's kernels with programmatic dependent launch (default); 0: QCF_PDL=0
   int gemm_mt;           // GEMM tile height in units of 128 rows: 0 = heuristic, else 1 / 2 (QCF_GEMM_MT)
   int attn_cluster;      // split-KV cluster size of the tcgen05 attention kernel: 0 = heuristic, else 1/2/4 (QCF_ATTN_CLUSTER)
+  int head_shards;       // this ctx holds 1/head_shards of the layer's heads (qcf_set_head_shards); scores divide by Hq*shards
   double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
   // workspace (device)
   float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]

@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(128) score_colsum_kernel(BatchDev bd, int hq, 
                                                            const __nv_bfloat16* __restrict__ k_f,
                                                            const float* __restrict__ stats_m,
                                                            const float* __restrict__ stats_l, int stats_rows,
-                                                           float* __restrict__ part, int part_stride,
+                                                           float* __restrict__ part, int part_stride, int norm_heads,
                                                            unsigned int* __restrict__ counters,
                                                            float* __restrict__ scores, int accumulate) {
   extern __shared__ __align__(128) unsigned char dsmem[];
@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(128) score_colsum_kernel(BatchDev bd, int hq, 
       const int key = key0 + threadIdx.x;
       float sum = 0.f;
       for (int gg = 0; gg < hkv; ++gg) sum += __ldcg(part + (static_cast<size_t>(b) * hkv + gg) * part_stride + key);
-      const float v = rows > 0 ? sum / static_cast<float>(hq * Lq) : 0.f;
+      const float v = rows > 0 ? sum / static_cast<float>(norm_heads * Lq) : 0.f;
       float* dst = scores + static_cast<size_t>(b) * bd.n_stride + key;
       *dst = accumulate ? *dst + v : v;
     }
@@ -299,12 +299,12 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
     auto kern = score_colsum_kernel<128>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     kern<<<g2, 128, smem, stream>>>(b->dev, L.hq, L.hkv, scale_log2, q_probe, k_f, ctx->stats_m, ctx->stats_l,
-                                    stats_rows, ctx->score_part, ctx->max_ctx, ctx->counters, scores, accumulate);
+                                    stats_rows, ctx->score_part, ctx->max_ctx, L.hq * ctx->head_shards, ctx->counters, scores, accumulate);
   } else {
     auto kern = score_colsum_kernel<64>;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     kern<<<g2, 128, smem, stream>>>(b->dev, L.hq, L.hkv, scale_log2, q_probe, k_f, ctx->stats_m, ctx->stats_l,
-                                    stats_rows, ctx->score_part, ctx->max_ctx, ctx->counters, scores, accumulate);
+                                    stats_rows, ctx->score_part, ctx->max_ctx, L.hq * ctx->head_shards, ctx->counters, scores, accumulate);
   }
   return cudaGetLastError();
 }

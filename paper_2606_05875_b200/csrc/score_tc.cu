@@ -53,6 +53,7 @@ enum { kAFull = 0, kBFull = 1, kBEmpty = 3, kSFull = 5, kSEmpty = 7, kAEmpty = 9
 struct ScoreArgs {
   float scale_log2;
   int hq, hkv, n_splits;
+  int norm_heads;                                        // Hq of the WHOLE layer (Hq * head shards): Eq. 18's 1/(Hq Lq)
   int kt_per_cta;                                        // pass 2: key tiles walked by one CTA
   float* stats_m; float* stats_l; int stats_rows;        // [B][n_splits][stats_rows]
   float* part; int part_stride;                          // [B][Hkv][part_stride]
@@ -402,7 +403,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         if (key < N) {
           float sum = 0.f;
           for (int gg = 0; gg < a.hkv; ++gg) sum += __ldcg(a.part + (static_cast<size_t>(b) * a.hkv + gg) * a.part_stride + key);
-          const float v = rows > 0 ? sum / static_cast<float>(a.hq * Lq) : 0.f;
+          const float v = rows > 0 ? sum / static_cast<float>(a.norm_heads * Lq) : 0.f;
           float* dst = a.scores + static_cast<size_t>(b) * bd.n_stride + key;
           *dst = a.accumulate ? *dst + v : v;
         }
@@ -516,7 +517,7 @@ cudaError_t launch_score_tc(const qcf_ctx* ctx, const qcf_batch* b, const __nv_b
     return cudaErrorInvalidValue;
   ScoreArgs a;
   a.scale_log2 = L.scale * kLog2e;
-  a.hq = L.hq; a.hkv = L.hkv; a.n_splits = n_splits; a.kt_per_cta = kt_per_cta;
+  a.hq = L.hq; a.hkv = L.hkv; a.norm_heads = L.hq * ctx->head_shards; a.n_splits = n_splits; a.kt_per_cta = kt_per_cta;
   a.stats_m = ctx->stats_m; a.stats_l = ctx->stats_l; a.stats_rows = L.hq * ctx->max_query;
   a.part = ctx->score_part; a.part_stride = ctx->max_ctx;
   a.counters = ctx->counters;

@@ -15,7 +15,7 @@ rho in 0.1..0.5): the datasets and weights are not in the cont
 """
 from __future__ import annotations
 
-from dataclasses import dataclass, field
+from dataclasses import dataclass, field, replace
 from typing import Dict, List, Optional, Tuple
 
 import numpy as np
@@ -116,6 +116,26 @@ class Workload:
     pool_k: List[np.ndarray] = field(default_factory=list)   # each uint16 [len, Hkv, d]
     pool_v: List[np.ndarray] = field(default_factory=list)
     requests: List[Request] = field(default_factory=list)
+
+
+def shard_heads(wl: Workload, rank: int, world: int) -> Workload:
+    """The slice of `wl` a rank of a KV-head-sharded step holds: kv-heads
+    [rank*Hkv/world, (rank+1)*Hkv/world) of every cache and the q heads that read them.  Slicing only."""
+    cfg = wl.cfg
+    if cfg.n_kv_heads % world:
+        raise ValueError("Hkv = %d is not divisible by %d shards" % (cfg.n_kv_heads, world))
+    per = cfg.n_kv_heads // world
+    g = cfg.n_q_heads // cfg.n_kv_heads
+    kv = slice(rank * per, (rank + 1) * per)
+    qh = slice(rank * per * g, (rank + 1) * per * g)
+    cut = lambda x, sl: np.ascontiguousarray(x[:, sl])
+    out = Workload(replace(cfg, n_q_heads=per * g, n_kv_heads=per))
+    out.pool_k = [cut(k, kv) for k in wl.pool_k]
+    out.pool_v = [cut(v, kv) for v in wl.pool_v]
+    for r in wl.requests:
+        out.requests.append(Request(r.chunk_ids, r.chunk_len, r.n_ctx, r.n_query, cut(r.q_probe, qh), cut(r.q_new, qh),
+                                    cut(r.k_new, kv), cut(r.v_new, kv), r.anchor_idx, r.anchor_ptr))
+    return out
 
 
 # --------------------------------------------------------------------------- synthesis

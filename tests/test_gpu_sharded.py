@@ -1,0 +1,141 @@
+"""GPU parity of the KV-head-sharded step (paper_2606_05875_b200/sharded.py) against
+the fp64 oracle of the UNSHARDED layer.  One GPU: the ranks run one after the other (no kernel waits on another
+rank), and the step's only exchange — the sum of the ranks' partial scores — is formed by qcf_score's own accumulate
+path, which is the arithmetic an all-reduce(sum) performs.  A world-size-1 NCCL group covers the collective call itself.
+Tolerances: BASELINE.json north_star's (see tests/test_gpu_parity.py).
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import qcf_oracle as O
+from paper_2606_05875_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def _mods():
+    from paper_2606_05875_b200 import binding, device, sharded
+    return binding, device, sharded
+
+
+def _f64(t):
+    return O.widen_bf16(t.detach().cpu().view(torch.int16).numpy().view(np.uint16))
+
+
+def _check_selection(sel_g, scores_o, k):
+    want = O.select_topk(scores_o, k)
+    srt = np.sort(scores_o)[::-1]
+    gap = (srt[k - 1] - srt[k]) / max(abs(srt[k - 1]), 1e-300) if 0 < k < len(scores_o) else 1.0
+    if gap > 1e-3:
+        assert np.array_equal(sel_g, want)                               # north_star: exact above the 1e-3 gap
+    else:
+        assert len(np.intersect1d(sel_g, want)) >= 0.99 * k
+
+
+def _ranks(wl, world):
+    _, device, sharded = _mods()
+    cfg = wl.cfg
+    steps, dws = [], []
+    for rank in range(world):
+        st = sharded.HeadShardedStep(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, max(cfg.batch, 1),
+                                     max(cfg.n_ctx, 1024), max(cfg.n_query, 1), rank=rank, world=world)
+        steps.append(st)
+        dws.append(device.DeviceWorkload(inputs.shard_heads(wl, rank, world), st.ctx))
+    return steps, dws
+
+
+@pytest.mark.parametrize("name,world", [("t_mid", 2), ("t_mid", 4), ("t_batch", 2), ("t_ragged", 2), ("c1", 2)])
+def test_head_sharded_step_matches_unsharded_oracle(name, world):
+    wl = inputs.make_workload(name)
+    cfg = wl.cfg
+    steps, dws = _ranks(wl, world)
+    scores = dws[0].scores                       # the array the all-reduce leaves on every rank
+    scores.fill_(7.0)
+    for rank, (st, dw) in enumerate(zip(steps, dws)):
+        st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                       q_probe=dw.q_probe, scores=scores, accumulate=rank > 0)
+    for st, dw in zip(steps, dws):
+        st.fuse_phase(dw.batch, scores=scores, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
+                      k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, lse=dw.lse, ratio=cfg.ratio)
+    torch.cuda.synchronize()
+    g = cfg.n_q_heads // cfg.n_kv_heads
+    sc = scores.cpu().numpy()
+    for b, r in enumerate(wl.requests):
+        k_pic = [O.widen_bf16(wl.pool_k[i]) for i in r.chunk_ids]
+        v_pic = [O.widen_bf16(wl.pool_v[i]) for i in r.chunk_ids]
+        ref = O.layer_step(k_pic, v_pic, cfg.rope_theta, O.widen_bf16(r.q_probe), cfg.ratio, O.widen_bf16(r.q_new),
+                           O.widen_bf16(r.k_new), O.widen_bf16(r.v_new))
+        # a2: the summed partials are Eq. 18 over ALL heads of the layer
+        np.testing.assert_allclose(sc[b, : r.n_ctx].astype(np.float64), ref["scores"], rtol=1e-2, atol=0)
+        # a3: replicated selection, identical on every rank
+        k = int(dws[0].n_sel[b])
+        assert k == len(ref["sel"])
+        sel0 = dws[0].sel[b, :k].cpu().numpy().astype(np.int64)
+        for dw in dws[1:]:
+            assert int(dw.n_sel[b]) == k and np.array_equal(dw.sel[b, :k].cpu().numpy(), sel0)
+        _check_selection(sel0, ref["scores"], k)
+        # a4 + a5: each rank's heads against the oracle run on the GPU's selection
+        ref2 = O.layer_step(k_pic, v_pic, cfg.rope_theta, None, 0.0, O.widen_bf16(r.q_new), O.widen_bf16(r.k_new),
+                            O.widen_bf16(r.v_new), sel=sel0)
+        n_r = k + r.n_query
+        per = cfg.n_kv_heads // world
+        for rank, dw in enumerate(dws):
+            qh = slice(rank * per * g, (rank + 1) * per * g)
+            kv = slice(rank * per, (rank + 1) * per)
+            assert np.max(np.abs(_f64(dw.out[b, :n_r]) - ref2["out"][:, qh]), initial=0.0) <= 2e-2   # max-abs 2e-2
+            t = r.n_ctx + r.n_query
+            assert np.array_equal(_f64(dw.v_fused[b, :t]), ref2["v_fused"][:, kv])
+            kf, want = _f64(dw.k_fused[b, :t]), ref2["k_fused"][:, kv]
+            ulp = np.ldexp(1.0, np.frexp(np.abs(want))[1] - 8)
+            assert np.all(np.abs(kf - want) <= np.maximum(2e-2, ulp))
+
+
+def test_head_shards_restore_and_reject():
+    binding, device, _ = _mods()
+    wl = inputs.make_workload("t_mid")
+    cfg = wl.cfg
+    ctx = binding.Context(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, 1, 1024, cfg.n_query)
+    dw = device.DeviceWorkload(wl, ctx)
+    ctx.qcf_rope_reposition(dw.batch, dw.k_pool, dw.v_pool, dw.k_fused, dw.v_fused)
+    ctx.qcf_score(dw.batch, dw.q_probe, dw.k_fused, dw.scores)
+    s1 = dw.scores.clone()
+    ctx.qcf_set_head_shards(4)
+    ctx.qcf_score(dw.batch, dw.q_probe, dw.k_fused, dw.scores)
+    assert torch.equal(dw.scores * 4, s1)                               # a power-of-two rescale is exact
+    ctx.qcf_set_head_shards(1)
+    ctx.qcf_score(dw.batch, dw.q_probe, dw.k_fused, dw.scores)
+    assert torch.equal(dw.scores, s1)
+    for bad in (0, -1, 65):
+        with pytest.raises(binding.QcfError):
+            ctx.qcf_set_head_shards(bad)
+
+
+def test_layer_step_through_a_nccl_group_of_one():
+    """The collective call itself (NCCL, one rank: the sum is the identity) inside the chained step."""
+    import torch.distributed as dist
+    _, device, sharded = _mods()
+    wl = inputs.make_workload("t_mid")
+    cfg = wl.cfg
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29617")
+    created = not dist.is_initialized()
+    if created:
+        dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        st = sharded.HeadShardedStep(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, 1, 1024, cfg.n_query)
+        dw = device.DeviceWorkload(wl, st.ctx)
+        st.layer_step(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                      q_probe=dw.q_probe, scores=dw.scores, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new,
+                      v_new=dw.v_new, out=dw.out, ratio=cfg.ratio)
+        torch.cuda.synchronize()
+        sel_a, out_a = dw.sel.clone(), dw.out.clone()
+        dw2 = device.DeviceWorkload(wl, st.ctx)
+        st.ctx.qcf_layer_step(dw2.batch, dw2.layer_args())
+        torch.cuda.synchronize()
+        assert torch.equal(sel_a, dw2.sel) and torch.equal(out_a, dw2.out)   # same kernels, same order: bit-identical
+    finally:
+        if created:
+            dist.destroy_process_group()
