@@ -9,6 +9,12 @@
 // MT = 1: 128 x 256 tiles, the two 256-column TMEM accumulators alternate, so the epilogue of tile i overlaps the
 //         main loop of tile i+1 (best wave quantisation: M = 3136 gives 25 row blocks);
 // MT = 2: 256 x 256 tiles, both accumulators belong to one tile (half the W re-reads from L2 per flop).
+// M <= 128 (the 64-row probe GEMMs of stage 1, which only stream weights): 128 x 64 tiles and an 8-stage ring, so 4x as
+//         many SMs pull weights and each UMMA is ~67 cycles instead of 128 (ncu, cold L2, M = 64: QKV 28.3 -> 19.8 us,
+//         O 31.7 -> 24.6, gate/up 41.5 -> 52, down 75.8 -> 56; stage 1 of config 3 4.57 -> 3.95 ms).  These launches are
+//         bound by the UMMA chain (4 MMAs + commit per 64-wide K block = 270-285 cycles, microbenchmarked) plus ~8 us of
+//         fixed prologue / first-load / epilogue time per launch, not by the loads: removing every TMA load after the first
+//         ring fill changes nothing, and an L2 prefetch 32 K blocks ahead of the ring made them slower.
 // Tiles are walked row-block fastest, so the CTAs of one wave share a handful of W tiles: every weight is read from
 // HBM once, A (<= 77 MB) stays in L2.
 // Epilogues: store | + residual (in place allowed) | SwiGLU over interleaved (gate, up) output columns.
@@ -24,14 +30,13 @@ namespace {
 
 using namespace ptx;
 
-constexpr int BN = 256;
 constexpr int BK = 64;
 constexpr int kThreads = 320;           // producer warp, issuer warp, 8 epilogue warps
 constexpr int kTmemCols = 512;
 
-template <int MT>
+template <int MT, int BN>
 struct GemmSmem {
-  static constexpr int kStages = MT == 1 ? 4 : 3;
+  static constexpr int kStages = BN <= 64 ? 8 : (MT == 1 ? 4 : 3);
   static constexpr int kA = 128 * MT * BK * 2;
   static constexpr int kB = BN * BK * 2;
   static constexpr int kStage = kA + kB;
@@ -49,12 +54,12 @@ struct GemmArgs {
 
 __device__ __forceinline__ float silu_f(float x) { return x / (1.f + __expf(-x)); }
 
-template <int MT, int EPI>
+template <int MT, int EPI, int BN>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_w, GemmArgs g) {
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  using S = GemmSmem<MT>;
+  using S = GemmSmem<MT, BN>;
   constexpr int BM = 128 * MT;
   constexpr int kAccBufs = MT == 1 ? 2 : 1;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -92,15 +97,19 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       int it = 0;
       for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         const int m0 = (t % n_mblk) * BM, n0 = (t / n_mblk) * BN;
+        // skinny tiles: every CTA reads the SAME A rows; start each tile at its own K block so that at any moment the
+        // CTAs pull different lines of A instead of queueing on one L2 slice (the K order of the fp32 sum is per tile, fixed)
+        const int rot = BN <= 64 ? (t * 5) % n_kb : 0;
         for (int kb = 0; kb < n_kb; ++kb, ++it) {
           const int st = it % S::kStages;
+          const int kk = (kb + rot >= n_kb ? kb + rot - n_kb : kb + rot) * BK;
           mbar_wait(bar(kEmpty + st), ((it / S::kStages) & 1) ^ 1);
           if (elect_one()) {
             mbar_arrive_expect_tx(bar(kFull + st), S::kStage);
             const uint32_t sa = sbase + st * S::kStage;
 #pragma unroll
-            for (int mt = 0; mt < MT; ++mt) tma_load_2d(sa + mt * (128 * BK * 2), &tm_a, bar(kFull + st), kb * BK, m0 + mt * 128);
-            tma_load_2d(sa + S::kA, &tm_w, bar(kFull + st), kb * BK, n0);
+            for (int mt = 0; mt < MT; ++mt) tma_load_2d(sa + mt * (128 * BK * 2), &tm_a, bar(kFull + st), kk, m0 + mt * 128);
+            tma_load_2d(sa + S::kA, &tm_w, bar(kFull + st), kk, n0);
           }
           __syncwarp();
         }
@@ -150,8 +159,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__
       mbar_wait(bar(kAccFull + buf), (tile_i / kAccBufs) & 1);
       tc_fence_after();
       const int row = m0 + (MT == 2 ? half * 128 : 0) + quarter * 32 + lane;
-      const int col_begin = MT == 1 ? half * 128 : 0;
-      constexpr int kCols = MT == 1 ? 128 : 256;
+      // MT = 1: the two warps of a lane quarter split the columns (BN = 32: the second one has none and only hands back)
+      constexpr int kCols = MT == 1 ? (BN >= 64 ? BN / 2 : BN) : BN;
+      const int col_begin = MT == 1 ? half * kCols : 0;
+      if (MT == 1 && BN < 64 && half == 1) {
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(kAccEmpty + buf));
+        continue;
+      }
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) +
                              (buf * MT + (MT == 2 ? half : 0)) * BN + col_begin;
       const bool row_ok = row < g.M;
@@ -240,14 +256,14 @@ bool make_map_2d(CUtensorMap* m, const void* base, int rows, int cols, int box_r
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int MT, int EPI>
+template <int MT, int EPI, int BN>
 cudaError_t launch_one(const qcf_ctx* ctx, const CUtensorMap& tm_a, const CUtensorMap& tm_w, const GemmArgs& g,
                        cudaStream_t stream) {
   constexpr int BM = 128 * MT;
   const int n_tiles = ((g.M + BM - 1) / BM) * ((g.N + BN - 1) / BN);
   const int grid = n_tiles < ctx->n_sm ? n_tiles : ctx->n_sm;
-  const int smem = GemmSmem<MT>::kBytes + 1024;
-  auto kern = gemm_tc_kernel<MT, EPI>;
+  const int smem = GemmSmem<MT, BN>::kBytes + 1024;
+  auto kern = gemm_tc_kernel<MT, EPI, BN>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   kern<<<grid, kThreads, smem, stream>>>(tm_a, tm_w, g);
   return cudaGetLastError();
@@ -259,25 +275,40 @@ cudaError_t launch_gemm(const qcf_ctx* ctx, const __nv_bfloat16* a, const __nv_b
                         const __nv_bfloat16* residual, __nv_bfloat16* c, int M, int N, int K, int epilogue,
                         cudaStream_t stream) {
   if (M <= 0 || N <= 0) return cudaSuccess;
+  // Skinny problems (one row block: the 64-row probe GEMMs of stage 1) stream 34-200 MB of weights and are bound by how
+  // many SMs pull them: 128 x 64 tiles give 4x the CTAs of 128 x 256 tiles and an 8-deep ring keeps ~100 KB in flight per SM.
+  const bool skinny = M <= 128 && ctx->gemm_mt == 0;
+  // 64-wide tiles, or 32-wide when that still leaves a single wave (N = 4096: 64 -> 128 CTAs; O 24.6 -> 20.8 us, down 56 -> 51)
+  const int bn = skinny ? ((N + 31) / 32 <= ctx->n_sm ? 32 : 64) : 256;
   // tile height: 256-row tiles halve the W traffic per flop but quantise worse; take them when they cost no extra wave
   int mt = ctx->gemm_mt;
   if (mt == 0) {
-    const int n_nblk = (N + BN - 1) / BN;
+    const int n_nblk = (N + bn - 1) / bn;
     const int w1 = (((M + 127) / 128) * n_nblk + ctx->n_sm - 1) / ctx->n_sm;       // waves of 128-row tiles
     const int w2 = (((M + 255) / 256) * n_nblk + ctx->n_sm - 1) / ctx->n_sm;       // waves of 256-row tiles (2x work)
-    mt = (2 * w2 <= w1) ? 2 : 1;
+    mt = (!skinny && 2 * w2 <= w1) ? 2 : 1;
   }
   CUtensorMap tm_a, tm_w;
-  if (!make_map_2d(&tm_a, a, M, K, 128) || !make_map_2d(&tm_w, w, N, K, BN)) return cudaErrorInvalidValue;
+  if (!make_map_2d(&tm_a, a, M, K, 128) || !make_map_2d(&tm_w, w, N, K, bn)) return cudaErrorInvalidValue;
   GemmArgs g{M, N, K, residual, c};
-  if (mt == 1) {
-    if (epilogue == 0) return launch_one<1, 0>(ctx, tm_a, tm_w, g, stream);
-    if (epilogue == 1) return launch_one<1, 1>(ctx, tm_a, tm_w, g, stream);
-    return launch_one<1, 2>(ctx, tm_a, tm_w, g, stream);
+  if (skinny) {
+    if (bn == 32) {
+      if (epilogue == 0) return launch_one<1, 0, 32>(ctx, tm_a, tm_w, g, stream);
+      if (epilogue == 1) return launch_one<1, 1, 32>(ctx, tm_a, tm_w, g, stream);
+      return launch_one<1, 2, 32>(ctx, tm_a, tm_w, g, stream);
+    }
+    if (epilogue == 0) return launch_one<1, 0, 64>(ctx, tm_a, tm_w, g, stream);
+    if (epilogue == 1) return launch_one<1, 1, 64>(ctx, tm_a, tm_w, g, stream);
+    return launch_one<1, 2, 64>(ctx, tm_a, tm_w, g, stream);
   }
-  if (epilogue == 0) return launch_one<2, 0>(ctx, tm_a, tm_w, g, stream);
-  if (epilogue == 1) return launch_one<2, 1>(ctx, tm_a, tm_w, g, stream);
-  return launch_one<2, 2>(ctx, tm_a, tm_w, g, stream);
+  if (mt == 1) {
+    if (epilogue == 0) return launch_one<1, 0, 256>(ctx, tm_a, tm_w, g, stream);
+    if (epilogue == 1) return launch_one<1, 1, 256>(ctx, tm_a, tm_w, g, stream);
+    return launch_one<1, 2, 256>(ctx, tm_a, tm_w, g, stream);
+  }
+  if (epilogue == 0) return launch_one<2, 0, 256>(ctx, tm_a, tm_w, g, stream);
+  if (epilogue == 1) return launch_one<2, 1, 256>(ctx, tm_a, tm_w, g, stream);
+  return launch_one<2, 2, 256>(ctx, tm_a, tm_w, g, stream);
 }
 
 }  // namespace qcf

@@ -124,6 +124,34 @@ def test_linear_swiglu(mt, monkeypatch):
     assert np.all(np.abs(_f64(c) - want) <= 0.5 * _ulp(want) + 1e-4 * (1 + np.abs(want)))
 
 
+@pytest.mark.parametrize("M,N,K", [(1, 528, 1536), (64, 4096, 512), (100, 6160, 200), (128, 9472, 1536)])
+def test_linear_skinny_tiles(M, N, K):
+    """M <= 128 takes the 128 x 32 / 128 x 64 tile variants (32-wide while N / 32 <= the SM count) with a per-tile
+    rotated K order; every epilogue, N and K tails."""
+    binding = _binding()
+    ctx = binding.Context(8, 2, 64, 1e6, 1, 1024, 8)
+    rng = np.random.default_rng(M * 11 + N)
+    a = inputs.f32_to_bf16_bits(rng.standard_normal((M, K), dtype=np.float32))
+    w = inputs.f32_to_bf16_bits(rng.standard_normal((N, K), dtype=np.float32) * np.float32(K ** -0.5))
+    r = inputs.f32_to_bf16_bits(rng.standard_normal((M, N), dtype=np.float32))
+    A, W = O.widen_bf16(a), O.widen_bf16(w)
+    exact = A @ W.T
+    da, dw = _dev(a), _dev(w)
+    c = torch.full((M + 1, N), 7.0, dtype=torch.bfloat16, device="cuda")
+    ctx.qcf_linear(da, dw, None, c, M, N, K, binding.QCF_EPI_STORE)
+    x = _dev(r)
+    ctx.qcf_linear(da, dw, x, x, M, N, K, binding.QCF_EPI_ADD_RESIDUAL)
+    g = torch.zeros((M, N // 2), dtype=torch.bfloat16, device="cuda")
+    ctx.qcf_linear(da, dw, None, g, M, N, K, binding.QCF_EPI_SWIGLU)             # rows 2j / 2j+1 of w as (gate_j, up_j)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(_f64(c[:M]) - exact) <= 0.5 * _ulp(exact) + 2e-5 * np.sqrt(K))
+    assert torch.all(c[M] == 7.0), "rows past M are untouched"
+    want = O.widen_bf16(r) + exact
+    assert np.all(np.abs(_f64(x) - want) <= 0.5 * _ulp(want) + 2e-5 * np.sqrt(K))
+    want = S.silu(exact[:, 0::2]) * exact[:, 1::2]
+    assert np.all(np.abs(_f64(g) - want) <= 0.5 * _ulp(want) + 1e-4 * (1 + np.abs(want)))
+
+
 # ----------------------------------------------------------------------------------------------- a1' anchor stitch
 
 def test_anchor_stitch_parity():
