@@ -276,6 +276,32 @@ def _to_bits(x):
 
 
 @pytest.mark.parametrize("name", ["s_small", "s_d128"])
+def test_stack_prefill_is_bit_identical_with_and_without_pdl(name, monkeypatch):
+    """The layer's kernels are chained with programmatic dependent launch (each one's prologue overlaps its
+    predecessor's tail).  A stale or early read would change bits: the chained run must equal the serialised one
+    (QCF_PDL=0) exactly, every time."""
+    results = []
+    for pdl in ("1", "0"):
+        monkeypatch.setenv("QCF_PDL", pdl)
+        wl, ctx, stack = _make(name)
+        sp = wl.spec
+        t = sp.n_ctx + sp.n_query
+        b = ctx.batch([[sp.chunk_len] * sp.n_chunks], [[i * sp.chunk_len for i in range(sp.n_chunks)]], [sp.n_query])
+        toks = torch.from_numpy(np.concatenate(wl.chunk_tokens + [wl.query_tokens]).astype(np.int32)).cuda()
+        for rep in range(3 if pdl == "1" else 1):
+            kc = [torch.zeros((t, sp.n_kv_heads, sp.head_dim), dtype=torch.bfloat16, device="cuda") for _ in range(sp.n_layers)]
+            vc = [torch.zeros_like(k) for k in kc]
+            hid = torch.full((t, sp.hidden), 3.0, dtype=torch.bfloat16, device="cuda")
+            stack.qcf_stack_prefill(b, toks, kc, vc, hid)
+            torch.cuda.synchronize()
+            results.append((hid, kc, vc))
+    ref = results[-1]
+    for hid, kc, vc in results[:-1]:
+        assert torch.equal(hid, ref[0])
+        assert all(torch.equal(x, y) for x, y in zip(kc, ref[1])) and all(torch.equal(x, y) for x, y in zip(vc, ref[2]))
+
+
+@pytest.mark.parametrize("name", ["s_small", "s_d128"])
 def test_stack_fuse_pipeline_free_running(name):
     """Fig. 9 end to end (stage 1 probe over the anchor cache, Eq. 20 scores, top-k, stage 2 with layer-ahead loading
     from pinned host pools) against the oracle on the same PIC caches (built by the oracle, so both sides start from
