@@ -128,7 +128,9 @@ QCF_API int32_t qcf_n_select(int32_t n_ctx, double ratio);
  * fp32 arithmetic, one bf16 rounding (RNE) on store.  A chunk at off_i = 0 is copied bit-exactly.
  *   k_pool, v_pool : dev, [pool_rows][Hkv][d] bf16, read-only (the layer's PIC pool)
  *   k_fused,v_fused: dev, [B][t_stride][Hkv][d] bf16; rows 0..N_b-1 of each request are written, the rest
- *                    (the Lq query rows and padding) are left untouched. */
+ *                    (the Lq query rows and padding) are left untouched.
+ * Either half may be omitted: v_pool == v_fused == NULL re-positions K only (the scoring prefetch of a critical layer
+ * reads no V), k_pool == k_fused == NULL stitches V only (its V, loaded later).  QCF_ERR_INVALID_ARG if both are. */
 QCF_API qcf_status qcf_rope_reposition(qcf_ctx* ctx, const qcf_batch* b, const void* k_pool, const void* v_pool,
                                        void* k_fused, void* v_fused, void* stream);
 

@@ -329,8 +329,9 @@ qcf_status qcf_rope_reposition(qcf_ctx* ctx, const qcf_batch* b, const void* k_p
                                void* v_fused, void* stream) {
   if (qcf_status st = check_ctx_batch(ctx, b)) return st;
   if (b->total_ctx == 0) return QCF_OK;
-  QCF_REQUIRE(ctx, k_pool && k_fused, "qcf_rope_reposition: NULL tensor pointer");
-  QCF_REQUIRE(ctx, (v_pool == nullptr) == (v_fused == nullptr), "qcf_rope_reposition: v_pool and v_fused must both be given or both be NULL");
+  QCF_REQUIRE(ctx, (k_pool && k_fused) || (v_pool && v_fused), "qcf_rope_reposition: NULL tensor pointer");
+  QCF_REQUIRE(ctx, (v_pool == nullptr) == (v_fused == nullptr) && (k_pool == nullptr) == (k_fused == nullptr),
+              "qcf_rope_reposition: a pool and its cache must both be given or both be NULL");
   QCF_REQUIRE(ctx, aligned16(k_pool) && aligned16(v_pool) && aligned16(k_fused) && aligned16(v_fused),
               "qcf_rope_reposition: pointers must be 16-byte aligned");
   QCF_CUDA(ctx, launch_reposition(ctx, b, static_cast<const __nv_bfloat16*>(k_pool),

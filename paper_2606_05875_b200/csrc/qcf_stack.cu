@@ -28,6 +28,8 @@ struct qcf_stack {
   __nv_bfloat16* probe_v[2];
   size_t probe_rows;
   cudaStream_t loader;
+  cudaStream_t loader2;                            // stage 1: K of the critical layers, issued at t = 0
+  __nv_bfloat16* stage_k2[2];                      // its staging ring
   std::vector<cudaEvent_t> ev_ready, ev_done;      // per pipeline slot
   cudaEvent_t ev_fork, ev_join;
   unsigned long long* load_t0;                     // device stamp of the bandwidth emulation (load_gbps)
@@ -148,7 +150,8 @@ qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_
   s->rope_table = nullptr;
   for (int i = 0; i < qcf_stack::kRing; ++i) s->stage_k[i] = s->stage_v[i] = nullptr;
   s->probe_k[0] = s->probe_k[1] = s->probe_v[0] = s->probe_v[1] = nullptr;
-  s->loader = nullptr; s->ev_fork = s->ev_join = nullptr; s->zero_i32 = nullptr;
+  s->loader = s->loader2 = nullptr; s->ev_fork = s->ev_join = nullptr; s->zero_i32 = nullptr;
+  s->stage_k2[0] = s->stage_k2[1] = nullptr;
   s->probe_rows = static_cast<size_t>(max_pool_rows) + ctx->max_query;
   bool ok = dalloc(&s->x, R * dims->hidden) == cudaSuccess && dalloc(&s->h, R * dims->hidden) == cudaSuccess &&
             dalloc(&s->qkv, R * (qd + 2 * kv)) == cudaSuccess && dalloc(&s->q_new, R * qd) == cudaSuccess &&
@@ -160,12 +163,14 @@ qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_
       ok = dalloc(&s->stage_k[i], static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess &&
            dalloc(&s->stage_v[i], static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess;
     for (int i = 0; i < 2 && ok; ++i)
-      ok = dalloc(&s->probe_k[i], s->probe_rows * kv) == cudaSuccess && dalloc(&s->probe_v[i], s->probe_rows * kv) == cudaSuccess;
+      ok = dalloc(&s->probe_k[i], s->probe_rows * kv) == cudaSuccess && dalloc(&s->probe_v[i], s->probe_rows * kv) == cudaSuccess &&
+           dalloc(&s->stage_k2[i], static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess;
   }
   s->load_t0 = nullptr;
   ok = ok && dalloc(&s->load_t0, 2) == cudaSuccess;
   ok = ok && dalloc(&s->zero_i32, 4) == cudaSuccess && cudaMemset(s->zero_i32, 0, 16) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&s->loader, cudaStreamNonBlocking) == cudaSuccess &&
+       cudaStreamCreateWithFlags(&s->loader2, cudaStreamNonBlocking) == cudaSuccess &&
        cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
        cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming) == cudaSuccess;
   const int n_slots = 2 * dims->n_layers + 4;
@@ -192,7 +197,7 @@ void qcf_stack_destroy(qcf_stack* s) {
                   static_cast<void*>(s->act), static_cast<void*>(s->rope_table)})
     if (p) cudaFree(p);
   for (int i = 0; i < qcf_stack::kRing; ++i) { if (s->stage_k[i]) cudaFree(s->stage_k[i]); if (s->stage_v[i]) cudaFree(s->stage_v[i]); }
-  for (int i = 0; i < 2; ++i) { if (s->probe_k[i]) cudaFree(s->probe_k[i]); if (s->probe_v[i]) cudaFree(s->probe_v[i]); }
+  for (int i = 0; i < 2; ++i) { if (s->probe_k[i]) cudaFree(s->probe_k[i]); if (s->probe_v[i]) cudaFree(s->probe_v[i]); if (s->stage_k2[i]) cudaFree(s->stage_k2[i]); }
   for (cudaEvent_t e : s->ev_ready) if (e) cudaEventDestroy(e);
   for (cudaEvent_t e : s->ev_done) if (e) cudaEventDestroy(e);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
@@ -200,6 +205,7 @@ void qcf_stack_destroy(qcf_stack* s) {
   if (s->load_t0) cudaFree(s->load_t0);
   if (s->zero_i32) cudaFree(s->zero_i32);
   if (s->loader) cudaStreamDestroy(s->loader);
+  if (s->loader2) cudaStreamDestroy(s->loader2);
   delete s;
 }
 
@@ -283,6 +289,10 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
   const bool do1 = a->stages == 0 || (a->stages & 1), do2 = a->stages == 0 || (a->stages & 2);
   cudaStream_t cs = static_cast<cudaStream_t>(stream);
   cudaStream_t ls = a->overlap ? s->loader : cs;
+  // K of the critical layers (the only FULL-context tensors stage 1 needs, Eq. 18) travels on its own stream from t = 0:
+  // on the main loader it would queue behind anchor jobs that are gated on the probe's progress and arrive at the very
+  // end of stage 1 with nothing left to hide it.  (With the bandwidth emulation the link is one serial resource.)
+  cudaStream_t ls2 = (a->overlap && !(a->load_gbps > 0.0)) ? s->loader2 : ls;
   const size_t kv_row = static_cast<size_t>(L.hkv) * L.d * 2;
   auto is_crit = [&](int l) { return std::find(a->crit_layers, a->crit_layers + a->n_crit, l) != a->crit_layers + a->n_crit; };
   const int slot_pic0 = l_max + 1;                       // event slot of PIC layer l = slot_pic0 + l; anchor layer l = l
@@ -290,6 +300,7 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
 
   STK_CUDA(ctx, cudaEventRecord(s->ev_fork, cs));
   if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(ls, s->ev_fork, 0));
+  if (ls2 != ls) STK_CUDA(ctx, cudaStreamWaitEvent(ls2, s->ev_fork, 0));
 
   // Loader jobs, in the order the pipeline consumes them.  The staging buffer of a job is read by the stitch kernel
   // issued right behind it on the same stream, so ring reuse needs no cross-stream wait; destinations are per layer.
@@ -312,6 +323,30 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
     STK_CUDA(ctx, cudaEventRecord(s->ev_ready[slot_pic0 + l], ls));
     return QCF_OK;
   };
+  // Critical layers: K alone in stage 1 (scoring reads no V), V stitched later by the stage-2 loader
+  int ring2 = 0;
+  auto load_pic_k = [&](int l, cudaStream_t st) -> qcf_status {
+    STK_REQUIRE(ctx, a->k_pic[l] && a->k_fused[l], "qcf_stack_fuse: NULL pool / cache pointer");
+    __nv_bfloat16* sk = st == ls ? s->stage_k[ring] : s->stage_k2[ring2];
+    if (st == ls) ring = (ring + 1) % qcf_stack::kRing; else ring2 ^= 1;
+    if (st == ls) STK_CUDA(ctx, throttle_begin());
+    STK_CUDA(ctx, cudaMemcpyAsync(sk, a->k_pic[l], a->pool_rows * kv_row, cudaMemcpyDefault, st));
+    if (st == ls) STK_CUDA(ctx, throttle_end(a->pool_rows * kv_row));
+    if (qcf_status e = qcf_rope_reposition(ctx, mb, sk, nullptr, a->k_fused[l], nullptr, st)) return e;         // a1, K only
+    STK_CUDA(ctx, cudaEventRecord(s->ev_ready[slot_pic0 + l], st));
+    return QCF_OK;
+  };
+  auto load_pic_v = [&](int l) -> qcf_status {
+    STK_REQUIRE(ctx, a->v_pic[l] && a->v_fused[l], "qcf_stack_fuse: NULL pool / cache pointer");
+    __nv_bfloat16* sv = s->stage_v[ring];
+    ring = (ring + 1) % qcf_stack::kRing;
+    STK_CUDA(ctx, throttle_begin());
+    STK_CUDA(ctx, cudaMemcpyAsync(sv, a->v_pic[l], a->pool_rows * kv_row, cudaMemcpyDefault, ls));
+    STK_CUDA(ctx, throttle_end(a->pool_rows * kv_row));
+    if (qcf_status e = qcf_rope_reposition(ctx, mb, nullptr, sv, nullptr, a->v_fused[l], ls)) return e;         // V stitch
+    STK_CUDA(ctx, cudaEventRecord(s->ev_ready[slot_pic0 + l], ls));      // re-recorded: stage 2 waits for K (earlier) and V
+    return QCF_OK;
+  };
   auto load_anchor = [&](int l) -> qcf_status {
     STK_REQUIRE(ctx, a->k_anchor[l] && a->v_anchor[l], "qcf_stack_fuse: NULL anchor pool pointer");
     __nv_bfloat16 *sk = s->stage_k[ring], *sv = s->stage_v[ring];
@@ -329,10 +364,14 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
   // ---- stage 1: selective token localization.  Loads are issued one layer ahead of their consumer.
   auto issue_stage1_loads = [&](int l) -> qcf_status {
     if (qcf_status e = load_anchor(l)) return e;
-    if (is_crit(l)) if (qcf_status e = load_pic(l)) return e;
+    if (is_crit(l) && ls2 == ls) if (qcf_status e = load_pic_k(l, ls)) return e;
     return QCF_OK;
   };
   if (do1) {
+  // two-stream mode: every critical layer's K goes out at t = 0 (slicing these transfers between the anchor jobs was
+  // measured and changes nothing: with both on the link stage 1 is bound by the ~30-40 GB/s that 2-4 MB copies reach)
+  if (ls2 != ls)
+    for (int i = 0; i < a->n_crit; ++i) if (qcf_status e = load_pic_k(a->crit_layers[i], ls2)) return e;
   if (qcf_status e = issue_stage1_loads(0)) return e;
   STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, nullptr, nullptr, 0, N, Lq, s->dims.hidden, s->x, cs));
   bool first = true;
@@ -355,7 +394,7 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
   // ---- stage 2: pipeline cache fusion.  The loader runs ahead through all remaining layers
   // (every layer has its own destination cache); the compute stream consumes them in order.
   for (int l = 0; l < n_l; ++l)
-    if (!do1 || !is_crit(l)) { if (qcf_status e = load_pic(l)) return e; }       // critical layers were stitched in stage 1
+    if (qcf_status e = (!do1 || !is_crit(l)) ? load_pic(l) : load_pic_v(l)) return e;   // critical layers: K is in place since stage 1
   STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, a->sel, a->n_sel, N, 0, n_rows, s->dims.hidden, s->x, cs));
   for (int l = 0; l < n_l; ++l) {
     if (ls != cs) STK_CUDA(ctx, cudaStreamWaitEvent(cs, s->ev_ready[slot_pic0 + l], 0));

@@ -79,7 +79,9 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
 #pragma unroll
   for (int u = 0; u < 4; ++u)
     if (static_cast<int>(threadIdx.x + u * blockDim.x) < n_vec) tv[u] = ld_nc_v4(vs + threadIdx.x + u * blockDim.x);
-  if (identity) {
+  if (k_pool == nullptr) {
+    // V-only stitch (the K of a critical layer was re-positioned ahead of time for scoring)
+  } else if (identity) {
     for (int r = rsub; r < rows; r += rows_per_pass) {
       const uint4 a = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0);
       const uint4 b = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0 + D / 2);

@@ -96,6 +96,27 @@ def test_reposition_leaves_query_rows_untouched():
     assert torch.all(dw.k_fused[0, n:] == 7.0) and torch.all(dw.v_fused[0, n:] == -3.0)
 
 
+@pytest.mark.parametrize("name", ["t_ragged", "t_batch"])
+def test_reposition_halves_compose(name):
+    """K-only followed by V-only writes exactly what one full call writes (include/qcf.h, a1)."""
+    binding, _ = _binding()
+    wl, ctx, dw = _setup(name)
+    ctx.qcf_rope_reposition(dw.batch, dw.k_pool, dw.v_pool, dw.k_fused, dw.v_fused)
+    torch.cuda.synchronize()
+    k_all, v_all = dw.k_fused.clone(), dw.v_fused.clone()
+    dw.k_fused.zero_(); dw.v_fused.zero_()
+    ctx.qcf_rope_reposition(dw.batch, dw.k_pool, None, dw.k_fused, None)
+    torch.cuda.synchronize()
+    assert torch.equal(dw.k_fused, k_all) and not dw.v_fused.any()
+    ctx.qcf_rope_reposition(dw.batch, None, dw.v_pool, None, dw.v_fused)
+    torch.cuda.synchronize()
+    assert torch.equal(dw.k_fused, k_all) and torch.equal(dw.v_fused, v_all)
+    with pytest.raises(binding.QcfError):
+        ctx.qcf_rope_reposition(dw.batch, None, None, None, None)
+    with pytest.raises(binding.QcfError):
+        ctx.qcf_rope_reposition(dw.batch, dw.k_pool, None, None, None)
+
+
 # --------------------------------------------------------------------------------------------- a2
 
 def _gpu_scores(ctx, dw, accumulate=False):
