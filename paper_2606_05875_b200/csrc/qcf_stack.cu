@@ -30,6 +30,9 @@ struct qcf_stack {
   cudaStream_t loader;
   cudaStream_t loader2;                            // stage 1: K of the critical layers, issued at t = 0
   __nv_bfloat16* stage_k2[2];                      // its staging ring
+  static constexpr int kArena = 2;                 // anchor arena: kArena x max_pool_rows rows of K and of V
+  __nv_bfloat16 *arena_k, *arena_v;                // stage 1, two-stream mode: anchor pools copied ahead of their stitch
+  std::vector<cudaEvent_t> ev_copy;                // per probe layer: its anchor rows are in the arena
   std::vector<cudaEvent_t> ev_ready, ev_done;      // per pipeline slot
   cudaEvent_t ev_fork, ev_join;
   unsigned long long* load_t0;                     // device stamp of the bandwidth emulation (load_gbps)
@@ -152,6 +155,7 @@ qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_
   s->probe_k[0] = s->probe_k[1] = s->probe_v[0] = s->probe_v[1] = nullptr;
   s->loader = s->loader2 = nullptr; s->ev_fork = s->ev_join = nullptr; s->zero_i32 = nullptr;
   s->stage_k2[0] = s->stage_k2[1] = nullptr;
+  s->arena_k = s->arena_v = nullptr;
   s->probe_rows = static_cast<size_t>(max_pool_rows) + ctx->max_query;
   bool ok = dalloc(&s->x, R * dims->hidden) == cudaSuccess && dalloc(&s->h, R * dims->hidden) == cudaSuccess &&
             dalloc(&s->qkv, R * (qd + 2 * kv)) == cudaSuccess && dalloc(&s->q_new, R * qd) == cudaSuccess &&
@@ -165,6 +169,8 @@ qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_
     for (int i = 0; i < 2 && ok; ++i)
       ok = dalloc(&s->probe_k[i], s->probe_rows * kv) == cudaSuccess && dalloc(&s->probe_v[i], s->probe_rows * kv) == cudaSuccess &&
            dalloc(&s->stage_k2[i], static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess;
+    ok = ok && dalloc(&s->arena_k, qcf_stack::kArena * static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess &&
+         dalloc(&s->arena_v, qcf_stack::kArena * static_cast<size_t>(max_pool_rows) * kv) == cudaSuccess;
   }
   s->load_t0 = nullptr;
   ok = ok && dalloc(&s->load_t0, 2) == cudaSuccess;
@@ -176,8 +182,10 @@ qcf_status qcf_stack_create(qcf_ctx* ctx, const qcf_stack_dims* dims, const qcf_
   const int n_slots = 2 * dims->n_layers + 4;
   s->ev_ready.assign(n_slots, nullptr);
   s->ev_done.assign(n_slots, nullptr);
+  s->ev_copy.assign(n_slots, nullptr);
   for (int i = 0; i < n_slots && ok; ++i)
-    ok = cudaEventCreateWithFlags(&s->ev_ready[i], cudaEventDisableTiming) == cudaSuccess &&
+    ok = cudaEventCreateWithFlags(&s->ev_copy[i], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&s->ev_ready[i], cudaEventDisableTiming) == cudaSuccess &&
          cudaEventCreateWithFlags(&s->ev_done[i], cudaEventDisableTiming) == cudaSuccess;
   ok = ok && launch_rope_table(s->rope_table, max_pos, L.d, static_cast<double>(L.theta), nullptr) == cudaSuccess &&
        cudaDeviceSynchronize() == cudaSuccess;
@@ -200,6 +208,9 @@ void qcf_stack_destroy(qcf_stack* s) {
   for (int i = 0; i < 2; ++i) { if (s->probe_k[i]) cudaFree(s->probe_k[i]); if (s->probe_v[i]) cudaFree(s->probe_v[i]); if (s->stage_k2[i]) cudaFree(s->stage_k2[i]); }
   for (cudaEvent_t e : s->ev_ready) if (e) cudaEventDestroy(e);
   for (cudaEvent_t e : s->ev_done) if (e) cudaEventDestroy(e);
+  for (cudaEvent_t e : s->ev_copy) if (e) cudaEventDestroy(e);
+  if (s->arena_k) cudaFree(s->arena_k);
+  if (s->arena_v) cudaFree(s->arena_v);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
   if (s->ev_join) cudaEventDestroy(s->ev_join);
   if (s->load_t0) cudaFree(s->load_t0);
@@ -347,8 +358,42 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
     STK_CUDA(ctx, cudaEventRecord(s->ev_ready[slot_pic0 + l], ls));      // re-recorded: stage 2 waits for K (earlier) and V
     return QCF_OK;
   };
+  // Two-stream mode: the transfer stream ls2 carries pure copies, in the order stage 1 consumes them and never gated by
+  // the probe's progress except through arena space: anchor rows of layer j land in arena slot j % n_aslots (its previous
+  // tenant, layer j - n_aslots, must have been stitched), K of a critical layer follows its anchors.  The stitches stay
+  // on ls, gated by the copy and by the probe cache they write.
+  const int n_aslots = a->anchor_rows > 0
+                           ? static_cast<int>(std::min<int64_t>(l_max + 1, qcf_stack::kArena * s->max_pool_rows / a->anchor_rows))
+                           : l_max + 1;
+  int next_copy = 0;
+  auto issue_copies = [&](int upto) -> qcf_status {          // anchor (and critical-K) transfers of layers < = upto
+    for (; ls2 != ls && next_copy <= std::min(upto, l_max); ++next_copy) {
+      const int j = next_copy;
+      STK_REQUIRE(ctx, a->k_anchor[j] && a->v_anchor[j], "qcf_stack_fuse: NULL anchor pool pointer");
+      if (j >= n_aslots) STK_CUDA(ctx, cudaStreamWaitEvent(ls2, s->ev_ready[j - n_aslots], 0));   // that stitch was enqueued earlier
+      const size_t off = static_cast<size_t>(j % n_aslots) * a->anchor_rows * kv_row;
+      if (a->anchor_rows > 0) {
+        STK_CUDA(ctx, cudaMemcpyAsync(reinterpret_cast<char*>(s->arena_k) + off, a->k_anchor[j], a->anchor_rows * kv_row, cudaMemcpyDefault, ls2));
+        STK_CUDA(ctx, cudaMemcpyAsync(reinterpret_cast<char*>(s->arena_v) + off, a->v_anchor[j], a->anchor_rows * kv_row, cudaMemcpyDefault, ls2));
+      }
+      STK_CUDA(ctx, cudaEventRecord(s->ev_copy[j], ls2));
+      if (is_crit(j)) if (qcf_status e = load_pic_k(j, ls2)) return e;
+    }
+    return QCF_OK;
+  };
   auto load_anchor = [&](int l) -> qcf_status {
     STK_REQUIRE(ctx, a->k_anchor[l] && a->v_anchor[l], "qcf_stack_fuse: NULL anchor pool pointer");
+    if (ls2 != ls) {
+      // stitch(l) is enqueued here, so the copies that may overwrite slots stitched up to l can go out now
+      const size_t off = static_cast<size_t>(l % n_aslots) * a->anchor_rows * kv_row;
+      STK_CUDA(ctx, cudaStreamWaitEvent(ls, s->ev_copy[l], 0));
+      if (l >= 2) STK_CUDA(ctx, cudaStreamWaitEvent(ls, s->ev_done[l - 2], 0));                    // probe cache l&1 is free again
+      if (qcf_status e = qcf_rope_reposition(ctx, pb, reinterpret_cast<char*>(s->arena_k) + off, reinterpret_cast<char*>(s->arena_v) + off,
+                                             s->probe_k[l & 1], s->probe_v[l & 1], ls))
+        return e;                                                                                  // a1'
+      STK_CUDA(ctx, cudaEventRecord(s->ev_ready[l], ls));
+      return issue_copies(l + n_aslots);
+    }
     __nv_bfloat16 *sk = s->stage_k[ring], *sv = s->stage_v[ring];
     ring = (ring + 1) % qcf_stack::kRing;
     STK_CUDA(ctx, throttle_begin());
@@ -368,10 +413,7 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
     return QCF_OK;
   };
   if (do1) {
-  // two-stream mode: every critical layer's K goes out at t = 0 (slicing these transfers between the anchor jobs was
-  // measured and changes nothing: with both on the link stage 1 is bound by the ~30-40 GB/s that 2-4 MB copies reach)
-  if (ls2 != ls)
-    for (int i = 0; i < a->n_crit; ++i) if (qcf_status e = load_pic_k(a->crit_layers[i], ls2)) return e;
+  if (qcf_status e = issue_copies(n_aslots - 1)) return e;
   if (qcf_status e = issue_stage1_loads(0)) return e;
   STK_CUDA(ctx, launch_embed_gather(s->embed, a->tokens, nullptr, nullptr, 0, N, Lq, s->dims.hidden, s->x, cs));
   bool first = true;
