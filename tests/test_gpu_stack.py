@@ -78,7 +78,7 @@ def _make(name, max_rows=None):
 
 # ----------------------------------------------------------------------------------------------- qcf_linear
 
-@pytest.mark.parametrize("mt", ["1", "2"])
+@pytest.mark.parametrize("mt", ["0", "1", "2"])
 @pytest.mark.parametrize("M,N,K", [(200, 768, 512), (131, 1536, 384), (1, 512, 1536), (300, 264, 64), (515, 1032, 4096)])
 def test_linear_store_and_residual(M, N, K, mt, monkeypatch):
     monkeypatch.setenv("QCF_GEMM_MT", mt)
@@ -104,7 +104,7 @@ def test_linear_store_and_residual(M, N, K, mt, monkeypatch):
     assert np.all(np.abs(_f64(x) - want) <= 0.5 * _ulp(want) + 2e-5 * np.sqrt(K))
 
 
-@pytest.mark.parametrize("mt", ["1", "2"])
+@pytest.mark.parametrize("mt", ["0", "1", "2"])
 def test_linear_swiglu(mt, monkeypatch):
     monkeypatch.setenv("QCF_GEMM_MT", mt)
     binding = _binding()
