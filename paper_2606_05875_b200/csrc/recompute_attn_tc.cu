@@ -57,7 +57,9 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 //   * S = Q K^T for PAIRS of key tiles as one 128 x 128 x 16 chain into a single 128-column S buffer (the TMEM budget of two
 //     CTAs per SM leaves no room to double-buffer it): c2 75.8 -> 90.1 us, c5 2.51 -> 2.90 ms — the serialised
 //     QK -> softmax -> PV chain costs more than the cheaper MMA saves;
-//   * pairing the heaviest tile of the first block round with the lightest of the second (equal pair sums): 75.8 -> 74.9 us.
+//   * pairing the heaviest tile of the first block round with the lightest of the second (equal pair sums): 75.8 -> 74.9 us;
+//   * one launch of 2-CTA clusters in which the heaviest 10-100 % of the items have their keys split over the pair and every
+//     other cluster carries two independent items: 75.8 -> 80.1 (10 %) ... 95.0 us (100 %).
 // What bounds it (microbenchmarks + knock-outs): a 128 x 64 x 16 SS MMA takes ~57 cycles, not the 32
 // its flops need (the 4 KB A read from shared memory; N = 128: 67, N = 256: 128, TS N = 128: 64), so one 64-key step is
 // 624 cycles of tensor pipe (8 SS + 4 TS), 82 % of peak at best.  A skeleton of this loop (MMAs and barrier handshakes
