@@ -90,6 +90,7 @@ struct Smem {
   static constexpr int kBytes = oStat + 2 * BM * 4;
   static_assert(2 * kStages * kTile >= BM * D * 4, "the K/V rings must hold one fp32 O tile for the split-KV merge");
 };
+// (the kEmptyK / kEmptyV slots are unused: a K stage is free when S of its tile is signalled, a V stage when its P V is)
 enum { kFullK = 0, kEmptyK = kStages, kFullV = 2 * kStages, kEmptyV = 3 * kStages, kSFull = 4 * kStages,
        kPReady = 4 * kStages + 2, kODone = 4 * kStages + 4, kQFull = 4 * kStages + 6 };
 
@@ -227,14 +228,15 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     for (int j = 0; j < n_kt; ++j) {
       const int st = j % kStages;
       const uint32_t ph = (j / kStages) & 1;
-      mbar_wait(bar(kEmptyK + st), ph ^ 1);
+      // stage st is free once Q K_{j-2}^T has completed: that is the phase S_{j-2} was signalled on (no separate commit)
+      if (j >= kStages) mbar_wait(bar(kSFull + st), ph ^ 1);
       if (elect_one()) {
         mbar_arrive_expect_tx(bar(kFullK + st), S::kTile);
 #pragma unroll
         for (int kb = 0; kb < D / 64; ++kb)
           tma_load_4d(sK + st * S::kTile + kb * S::kBlk, &tm_k, bar(kFullK + st), kb * 64, g, (jt0 + j) * BN, b);
       }
-      mbar_wait(bar(kEmptyV + st), ph ^ 1);
+      if (j >= kStages) mbar_wait(bar(kODone + st), ph ^ 1);     // P_{j-2} V_{j-2} has completed
       if (elect_one()) {
         mbar_arrive_expect_tx(bar(kFullV + st), S::kTile);
 #pragma unroll
@@ -266,7 +268,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
           for (int ks = 0; ks < D / 16; ++ks)
             umma_ss(d_tmem, dq + static_cast<uint64_t>(((ks >> 2) * S::kQBlk + (ks & 3) * 32) >> 4),
                     dk_st + static_cast<uint64_t>(((ks >> 2) * S::kBlk + (ks & 3) * 32) >> 4), idesc_qk, ks > 0 ? 1u : 0u);
-          umma_commit(bar(kEmptyK + st));
           umma_commit(bar(kSFull + (j & 1)));
         }
         __syncwarp();
@@ -286,7 +287,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
           for (int ks = 0; ks < BN / 16; ++ks)
             umma_ts(tmem_o, tmem_base + (j & 1) * BN + ks * 8, dv_st + static_cast<uint64_t>((ks * 2048) >> 4), idesc_pv,
                     (j > 0 || ks > 0) ? 1u : 0u);
-          umma_commit(bar(kEmptyV + st));
           umma_commit(bar(kODone + (j & 1)));
         }
         __syncwarp();
