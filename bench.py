@@ -35,7 +35,7 @@ KERNELS_PER_STEP = 6           # reposition, score_stats, score_colsum, topk, sc
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one attn_kernel launch on c2, from the ncu --set full capture
 # summarised in profiles/ (None until a capture of the current kernel is committed)
-A5_DRAM_TRAFFIC_BYTES = 34478080   # profiles/r01_c2_attn_tc_ncu.csv (34 425 856 read + 52 224 written)
+A5_DRAM_TRAFFIC_BYTES = 34467840   # profiles/r01_c2_attn_tc_ncu.csv (34 426 368 read + 41 472 written)
 
 
 def parse_args():
