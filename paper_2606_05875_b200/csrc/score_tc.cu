@@ -148,7 +148,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         __syncwarp();
         for (int j = 0; j < n_j; ++j, ++it) {
           const int st = it & 1;
-          mbar_wait(bar(kBEmpty + st), ((it >> 1) & 1) ^ 1);
+          // stage st is free once the MMAs of step it - 2 have completed: the phase S of that step was signalled on
+          if (it >= 2) mbar_wait(bar(kSFull + st), ((it >> 1) & 1) ^ 1);
           if (elect_one()) {
             mbar_arrive_expect_tx(bar(kBFull + st), S::kTile);
             if (PASS == 1) load_k_tile(sB + st * S::kTile, bar(kBFull + st), k_begin + j * BT);
@@ -179,7 +180,6 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
               const uint64_t koff = static_cast<uint64_t>(((ks >> 2) * S::kBlk + (ks & 3) * 32) >> 4);
               umma_ss(tmem_base + st * BT, da0 + koff, db + koff, idesc, ks > 0 ? 1u : 0u);
             }
-            umma_commit(bar(kBEmpty + st));
             umma_commit(bar(kSFull + st));
             if (j == n_j - 1) umma_commit(bar(kAEmpty));
           }
