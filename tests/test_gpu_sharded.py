@@ -93,6 +93,43 @@ def test_head_sharded_step_matches_unsharded_oracle(name, world):
             assert np.all(np.abs(kf - want) <= np.maximum(2e-2, ulp))
 
 
+def test_head_sharded_full_size_c2_matches_the_unsharded_step():
+    """BASELINE configs[1] at full size, two shards, against the UNSHARDED CUDA step on the same inputs (itself checked
+    against the oracle in tests/test_gpu_parity.py): the summed partial scores agree to fp32 rounding, the selection is
+    the same up to near-ties (north_star: >= 99 % overlap), and with the same selection forced on both sides every
+    head's attention output and fused cache is bit-identical (same kernels, same per-kv-head tiles)."""
+    binding, device, _ = _mods()
+    wl = inputs.make_workload("c2")
+    cfg = wl.cfg
+    ctx = binding.Context(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, 1, cfg.n_ctx, cfg.n_query)
+    ref = device.DeviceWorkload(wl, ctx)
+    ctx.qcf_layer_step(ref.batch, ref.layer_args())
+    torch.cuda.synchronize()
+    steps, dws = _ranks(wl, 2)
+    scores = dws[0].scores
+    for rank, (st, dw) in enumerate(zip(steps, dws)):
+        st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                       q_probe=dw.q_probe, scores=scores, accumulate=rank > 0)
+    torch.cuda.synchronize()
+    n = cfg.n_ctx
+    np.testing.assert_allclose(scores[0, :n].cpu().numpy(), ref.scores[0, :n].cpu().numpy(), rtol=1e-5, atol=1e-12)
+    k = int(ref.n_sel[0])
+    steps[0].ctx.qcf_select_topk(dws[0].batch, scores, cfg.ratio, dws[0].sel, dws[0].n_sel)
+    torch.cuda.synchronize()
+    assert int(dws[0].n_sel[0]) == k
+    assert len(np.intersect1d(dws[0].sel[0, :k].cpu().numpy(), ref.sel[0, :k].cpu().numpy())) >= 0.99 * k
+    g = cfg.n_q_heads // cfg.n_kv_heads
+    per = cfg.n_kv_heads // 2
+    for rank, (st, dw) in enumerate(zip(steps, dws)):
+        st.fuse_phase(dw.batch, scores=scores, sel=ref.sel, n_sel=ref.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
+                      k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, ratio=cfg.ratio, select_now=False)
+        torch.cuda.synchronize()
+        n_r = k + cfg.n_query
+        assert torch.equal(dw.out[0, :n_r], ref.out[0, :n_r, rank * per * g:(rank + 1) * per * g])
+        assert torch.equal(dw.k_fused[0], ref.k_fused[0][:, rank * per:(rank + 1) * per])
+        assert torch.equal(dw.v_fused[0], ref.v_fused[0][:, rank * per:(rank + 1) * per])
+
+
 def test_head_shards_restore_and_reject():
     binding, device, _ = _mods()
     wl = inputs.make_workload("t_mid")
