@@ -22,9 +22,9 @@ __device__ __forceinline__ uint32_t order_key(float f) {
 __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float* __restrict__ scores, double ratio,
                                                         int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached, int ceil_mode) {
   extern __shared__ uint32_t s_keys[];                           // order keys of the first n_cached scores
-  __shared__ unsigned int hist[256];
+  __shared__ unsigned int hist[2][256];        // double-buffered: pass p + 1's bins are zeroed while pass p's are scanned
   __shared__ unsigned int s_prefix, s_remaining;
-  __shared__ unsigned int warp_cnt[32];                          // packed (gt << 16) | eq per warp
+  __shared__ unsigned int warp_cnt[32], warp_cnt2[32];           // per-warp counts of keys > T and == T
   pdl_trigger();
   const int b = blockIdx.x;
   const int N = bd.n_ctx[b];
@@ -46,29 +46,30 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   const int n_sm_keys = min(N, n_cached);
   for (int i = tid; i < n_sm_keys; i += kThreads) s_keys[i] = order_key(__ldcg(s + i));
   auto key_of = [&](int i) -> uint32_t { return i < n_sm_keys ? s_keys[i] : order_key(__ldcg(s + i)); };
+  if (tid < 256) hist[0][tid] = 0u;
+  if (tid == 0) { s_prefix = 0u; s_remaining = static_cast<unsigned int>(k); }
   __syncthreads();
 
   // ---- radix select: after pass p the top 8(p+1) bits of the k-th largest key are known
-  if (tid == 0) { s_prefix = 0u; s_remaining = static_cast<unsigned int>(k); }
 #pragma unroll 1
   for (int pass = 0; pass < 4; ++pass) {
     const int shift = 24 - 8 * pass;
-    if (tid < 256) hist[tid] = 0u;
-    __syncthreads();
+    unsigned int* h = hist[pass & 1];
     const uint32_t prefix = s_prefix;
     const uint32_t mask = pass == 0 ? 0u : (0xffffffffu << (shift + 8));
     for (int i = tid; i < N; i += kThreads) {
       const uint32_t key = key_of(i);
       // (warp-aggregating these atomics with match.any was measured: 12.6 -> 16.7 us on c2, 41 -> 63 us on c5)
-      if ((key & mask) == prefix) atomicAdd(&hist[(key >> shift) & 0xffu], 1u);
+      if ((key & mask) == prefix) atomicAdd(&h[(key >> shift) & 0xffu], 1u);
     }
     __syncthreads();
+    if (warp >= 1 && warp <= 8) hist[(pass + 1) & 1][tid - 32] = 0u;        // the next pass's bins
     if (warp == 0) {
       // bins from the top: find the digit where the cumulative count reaches `remaining`
       const unsigned int remaining = s_remaining;
       unsigned int cnt[8], tot = 0;
 #pragma unroll
-      for (int j = 0; j < 8; ++j) { cnt[j] = hist[255 - (lane * 8 + j)]; tot += cnt[j]; }
+      for (int j = 0; j < 8; ++j) { cnt[j] = h[255 - (lane * 8 + j)]; tot += cnt[j]; }
       unsigned int incl = tot;
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
@@ -93,37 +94,43 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   const uint32_t T = s_prefix;
   const unsigned int need = s_remaining;                         // elements equal to T that are selected (>= 1)
 
-  // ---- ordered emission: position of element i = #(key > T before i) + min(#(key == T before i), need)
-  unsigned int run_gt = 0, run_eq = 0;
-  for (int base = 0; base < N; base += kThreads) {
-    const int i = base + tid;
-    uint32_t key = 0u;
-    const bool valid = i < N;
-    if (valid) key = key_of(i);
-    const bool gt = valid && key > T, eq = valid && key == T;
-    const unsigned int bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
-    if (lane == 0) warp_cnt[warp] = (static_cast<unsigned int>(__popc(bg)) << 16) | static_cast<unsigned int>(__popc(be));
-    __syncthreads();
-    unsigned int before = 0, total = 0;
-    {
-      const unsigned int v = warp_cnt[lane];
-      unsigned int incl = v;
+  // ---- ordered emission: position of element i = #(key > T before i) + min(#(key == T before i), need).
+  // Warp w owns the contiguous block [w * rows * 32, (w + 1) * rows * 32) and walks it in rows of 32 (lane = element, so
+  // shared-memory and global accesses stay conflict-free / coalesced): a counting sweep, ONE block-level exchange of the
+  // 32 warp totals, then an emitting sweep with running offsets.
+  const int rows = ((N + 31) / 32 + 31) / 32;                    // rows of 32 elements per warp
+  const int base = warp * rows * 32;
+  unsigned int wg = 0, we = 0;
+  for (int j = 0; j < rows; ++j) {
+    const int i = base + j * 32 + lane;
+    const uint32_t key = i < N ? key_of(i) : 0u;
+    wg += __popc(__ballot_sync(0xffffffffu, i < N && key > T));
+    we += __popc(__ballot_sync(0xffffffffu, i < N && key == T));
+  }
+  if (lane == 0) { warp_cnt[warp] = wg; warp_cnt2[warp] = we; }
+  __syncthreads();
+  unsigned int run_gt, run_eq;
+  {
+    const unsigned int vg = warp_cnt[lane], ve = warp_cnt2[lane];
+    unsigned int ig = vg, ie = ve;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned int u = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += u;
-      }
-      const unsigned int excl = incl - v;
-      before = __shfl_sync(0xffffffffu, excl, warp);
-      total = __shfl_sync(0xffffffffu, incl, 31);
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned int ug = __shfl_up_sync(0xffffffffu, ig, o), ue = __shfl_up_sync(0xffffffffu, ie, o);
+      if (lane >= o) { ig += ug; ie += ue; }
     }
-    const unsigned int lt_mask = (1u << lane) - 1u;
-    const unsigned int gt_before = run_gt + (before >> 16) + __popc(bg & lt_mask);
-    const unsigned int eq_before = run_eq + (before & 0xffffu) + __popc(be & lt_mask);
+    run_gt = __shfl_sync(0xffffffffu, ig - vg, warp);
+    run_eq = __shfl_sync(0xffffffffu, ie - ve, warp);
+  }
+  const unsigned int lt_mask = (1u << lane) - 1u;
+  for (int j = 0; j < rows; ++j) {
+    const int i = base + j * 32 + lane;
+    const uint32_t key = i < N ? key_of(i) : 0u;
+    const bool gt = i < N && key > T, eq = i < N && key == T;
+    const unsigned int bg = __ballot_sync(0xffffffffu, gt), be = __ballot_sync(0xffffffffu, eq);
+    const unsigned int gt_before = run_gt + __popc(bg & lt_mask), eq_before = run_eq + __popc(be & lt_mask);
     if (gt || (eq && eq_before < need)) out[gt_before + min(eq_before, need)] = i;
-    run_gt += total >> 16;
-    run_eq += total & 0xffffu;
-    __syncthreads();
+    run_gt += __popc(bg);
+    run_eq += __popc(be);
   }
 }
 
