@@ -270,7 +270,14 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
   size_t o_len = up(o_off + sizeof(int32_t) * n_chunks, 16), o_blk = up(o_len + sizeof(int32_t) * n_chunks, 16);
   size_t o_row = up(o_blk + sizeof(int32_t) * (n_chunks + 1), 16), o_rot = up(o_row + sizeof(int64_t) * n_chunks, 16);
   size_t o_crot = up(o_rot + sizeof(float) * rot.size(), 16);
-  size_t total = up(o_crot + sizeof(int32_t) * n_chunks, 16) + 16;
+  size_t o_item = up(o_crot + sizeof(int32_t) * n_chunks, 32);
+  std::vector<RepoItem> items;
+  items.reserve(c_blk.back());
+  for (int c = 0; c < n_chunks; ++c)
+    for (int r0 = 0; r0 < c_len[c]; r0 += kRepoRows)
+      items.push_back(RepoItem{c_row[c] + r0, static_cast<int64_t>(c_req[c]) * t_stride + c_off[c] + r0,
+                               std::min<int32_t>(kRepoRows, c_len[c] - r0), c, c_rot[c] == 0 ? 1 : 0, 0});
+  size_t total = up(o_item + sizeof(RepoItem) * items.size(), 16) + 16;
   std::vector<unsigned char> host(total, 0);
   if (batch > 0) {
     std::memcpy(host.data() + o_nctx, n_ctx.data(), sizeof(int32_t) * batch);
@@ -285,6 +292,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
     std::memcpy(host.data() + o_crot, c_rot.data(), sizeof(int32_t) * n_chunks);
   }
   std::memcpy(host.data() + o_blk, c_blk.data(), sizeof(int32_t) * (n_chunks + 1));
+  if (!items.empty()) std::memcpy(host.data() + o_item, items.data(), sizeof(RepoItem) * items.size());
   cudaError_t e = cudaMalloc(&qb->blob, total);
   if (e == cudaSuccess) e = cudaMemcpy(qb->blob, host.data(), total, cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
@@ -304,6 +312,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
   bd.chunk_row = reinterpret_cast<const int64_t*>(d + o_row);
   bd.rot = reinterpret_cast<const float2*>(d + o_rot);
   bd.chunk_rot = reinterpret_cast<const int32_t*>(d + o_crot);
+  bd.repo_items = reinterpret_cast<const int4*>(d + o_item);
   *out = qb;
   return QCF_OK;
 }

@@ -29,6 +29,18 @@ struct BatchDev {
   const int64_t* chunk_row;    // first row in the PIC pool
   const int32_t* chunk_blk;    // [n_chunks+1] exclusive prefix of ceil(len / kRepoRows): reposition work list
   const float2* rot;           // [n_chunks][d/2] (cos, sin)(off_i * theta^(-2j/d))
+  const int4* repo_items;      // [repo_blocks][2]: one flat record per reposition work item (RepoItem)
+};
+
+// One reposition work item (kRepoRows rows of one chunk), 32 bytes: everything a CTA needs in ONE load, so that its pool
+// reads are one dependent round trip behind the launch instead of five (binary search over chunk_blk, then the fields).
+struct RepoItem {
+  int64_t src_row;   // first pool row
+  int64_t dst_row;   // first row in the fused cache (request * t_stride + off + row0)
+  int32_t rows;      // <= kRepoRows
+  int32_t chunk;     // index into rot
+  int32_t identity;  // != 0: rotation position 0, K is copied bit-exactly
+  int32_t pad;
 };
 
 struct Layout {

@@ -41,21 +41,12 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   constexpr int kSlotsPerHead = D / 16;
   const int slots = hkv * kSlotsPerHead;
   const int row_elems = hkv * D;
-  // locate the chunk of this work item (chunk_blk is an exclusive prefix sum; a handful of chunks per batch)
-  const int item = blockIdx.x;
-  int lo = 0, hi = bd.n_chunks;
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (bd.chunk_blk[mid] <= item) lo = mid; else hi = mid;
-  }
-  const int c = lo;
-  const int row0 = (item - bd.chunk_blk[c]) * kRepoRows;
-  const int len = bd.chunk_len[c];
-  const int rows = min(kRepoRows, len - row0);
-  const int off = bd.chunk_off[c];
-  const int req = bd.chunk_req[c];
-  const size_t src_row = static_cast<size_t>(bd.chunk_row[c]) + row0;
-  const size_t dst_row = static_cast<size_t>(req) * bd.t_stride + off + row0;
+  // this work item's flat record (RepoItem, qcf_internal.cuh): two 16-byte loads, no search
+  const int4 w0 = __ldg(bd.repo_items + 2 * blockIdx.x), w1 = __ldg(bd.repo_items + 2 * blockIdx.x + 1);
+  const size_t src_row = (static_cast<size_t>(static_cast<uint32_t>(w0.y)) << 32) | static_cast<uint32_t>(w0.x);
+  const size_t dst_row = (static_cast<size_t>(static_cast<uint32_t>(w0.w)) << 32) | static_cast<uint32_t>(w0.z);
+  const int rows = w1.x;
+  const int c = w1.y;
 
   pdl_trigger();
   const int slot = threadIdx.x % slots;
@@ -68,7 +59,7 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   // ---- K: rotate by the chunk's offset angle.  A rotation position of 0 is the identity and is copied bit-exactly.
   const __nv_bfloat16* ks = k_pool + src_row * row_elems;
   __nv_bfloat16* kd = k_f + dst_row * row_elems;
-  const bool identity = bd.chunk_rot[c] == 0;
+  const bool identity = w1.z != 0;
   pdl_wait();                          // before the first pool read / cache write (descriptor reads above are constant)
   // V rows of this work item (byte copy): the first sweep's loads are issued BEFORE the K section so that a thread has
   // all of its bytes (K pairs + V vectors, 128 B at 8 x 128) in flight at once — at c2 the whole 21 MB input is then
