@@ -250,7 +250,8 @@ typedef struct {
  * chained on `stream` with no host synchronisation. */
 QCF_API qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* args, void* stream);
 
-/* Same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe
+/* pool_rows: rows of host->k_pool / v_pool; every chunk of the batch must lie inside them (QCF_ERR_INVALID_ARG otherwise).
+ * Same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe
  * and fresh rows, runs qcf_layer_step on the context's internal device buffers, downloads the |R_b| written rows of `out`, `sel`,
  * `n_sel` (and the fused cache if k_fused / v_fused are non-NULL), and synchronises `stream` before
  * returning.  Pointer fields of `host` are host pointers with the same shapes; `pool_rows` is the number of
@@ -264,6 +265,17 @@ QCF_API qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const q
  * over the profiled steps issued since the previous call (or since profiling was enabled), then forgets them. */
 QCF_API qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable);
 QCF_API qcf_status qcf_get_stage_ms(qcf_ctx* ctx, float* ms5);
+
+/* Test-only launch knobs (the one debug entry point; nothing is read from the environment).  They change HOW the same
+ * kernels are launched, never WHAT is computed — the parity tests use them to force launch shapes the host heuristics
+ * would only pick at other problem sizes:
+ *   QCF_DEBUG_PDL          value 0: plain stream-ordered launches; 1 (default): programmatic dependent launch between the
+ *                          kernels of a step
+ *   QCF_DEBUG_ATTN_CLUSTER value 1 / 2 / 4: split-KV cluster size of the a5 kernel; 0 (default): host heuristic
+ *   QCF_DEBUG_GEMM_MT      value 1 / 2: GEMM tile height in units of 128 rows; 0 (default): host heuristic
+ * QCF_ERR_INVALID_ARG for an unknown knob or value. */
+typedef enum { QCF_DEBUG_PDL = 0, QCF_DEBUG_ATTN_CLUSTER = 1, QCF_DEBUG_GEMM_MT = 2 } qcf_debug_knob;
+QCF_API qcf_status qcf_debug_set(qcf_ctx* ctx, int32_t knob, int32_t value);
 
 /* ---------------------------------------------------------------------------------------- a7 / a8 (config 3) */
 
@@ -351,10 +363,10 @@ QCF_API qcf_status qcf_stack_first_token(qcf_stack* s, const void* hidden, int32
 typedef struct {
   const void* const* k_pic;      /* host array [L] of pointers to [pool_rows][Hkv][d] bf16 PIC pools              */
   const void* const* v_pic;
-  int64_t pool_rows;
+  int64_t pool_rows;             /* rows of each PIC pool; every chunk of main_batch must lie inside (else INVALID_ARG)  */
   const void* const* k_anchor;   /* host array [L] (entries l <= max(L*) are read) of compact anchor pools         */
   const void* const* v_anchor;
-  int64_t anchor_rows;
+  int64_t anchor_rows;           /* rows of each anchor pool; every chunk of probe_batch must lie inside                  */
   const int32_t* crit_layers;    /* host [n_crit], ascending 0-based layer indices of L*                           */
   int32_t n_crit;
   double ratio;                  /* rho                                                                             */
@@ -367,7 +379,11 @@ typedef struct {
   void* hidden_out;              /* dev [n_R][hidden] out: final hidden states of the rows R (P ascending, then U)  */
   int32_t overlap;               /* != 0: layer-ahead loading on a second stream (a8); 0: serial, for the ablation  */
   int32_t stages;                /* 0 or 3: both stages; 1: stage 1 only (scores, sel, n_sel are produced, no layer is
-                                    recomputed); 2: stage 2 only (sel / n_sel are INPUTS, e.g. from another selector)   */
+                                    recomputed); 2: stage 2 only (sel / n_sel are INPUTS, e.g. from another selector: they
+                                    must hold EXACTLY qcf_n_select(N, ratio) positions — every stage-2 row count is derived
+                                    on the host from `ratio`; pass ratio = |P| / N for an external selection of another size.
+                                    This mode reads n_sel[0] back once (one stream synchronisation before the first launch)
+                                    and returns QCF_ERR_INVALID_ARG on a mismatch)                                        */
   double load_gbps;              /* > 0: emulate a KV store of this bandwidth (GB/s): every pool load on the loader stream
                                     is held until bytes / load_gbps have elapsed since it started (the
                                     bandwidth-constrained loading experiment); 0: unthrottled                            */

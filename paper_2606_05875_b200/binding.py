@@ -21,12 +21,13 @@ _STATUS = {0: "QCF_OK", 1: "QCF_ERR_INVALID_ARG", 2: "QCF_ERR_UNSUPPORTED", 3: "
 EXPORTS = (
     "qcf_create", "qcf_destroy", "qcf_last_error", "qcf_version", "qcf_batch_create", "qcf_batch_destroy",
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
-    "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards",
+    "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards", "qcf_debug_set",
     "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
 )
 
 QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
 QCF_ANCHOR_SINK, QCF_ANCHOR_KNORM = 0, 1
+QCF_DEBUG_PDL, QCF_DEBUG_ATTN_CLUSTER, QCF_DEBUG_GEMM_MT = 0, 1, 2
 
 
 class QcfError(RuntimeError):
@@ -111,6 +112,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_layer_step_host": (i32, [vp, vp, C.POINTER(qcf_layer_args), i64, vp]),
         "qcf_set_profiling": (i32, [vp, i32]),
         "qcf_set_head_shards": (i32, [vp, i32]),
+        "qcf_debug_set": (i32, [vp, i32, i32]),
         "qcf_get_stage_ms": (i32, [vp, C.POINTER(C.c_float)]),
         "qcf_anchor_rank": (i32, [vp, vp, vp, i32, f64, vp, i32, i32, vp, vp, vp]),
         "qcf_linear": (i32, [vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]),
@@ -279,6 +281,9 @@ class Context:
 
     def qcf_set_head_shards(self, n_shards: int):
         self._check(self.lib.qcf_set_head_shards(self.handle, int(n_shards)))
+
+    def qcf_debug_set(self, knob: int, value: int):
+        self._check(self.lib.qcf_debug_set(self.handle, int(knob), int(value)))
 
     def qcf_set_profiling(self, enable: bool):
         self._check(self.lib.qcf_set_profiling(self.handle, int(bool(enable))))

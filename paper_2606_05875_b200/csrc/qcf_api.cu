@@ -130,23 +130,9 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->score_row_ctr = nullptr;
   c->counters = nullptr;
   c->stage = nullptr;
-  c->ptc_units = nullptr; c->ptc_n_units = nullptr; c->ptc_part_o = c->ptc_part_ml = nullptr; c->ptc_item_ctr = nullptr;
-  {
-    const char* e = std::getenv("QCF_ATTN_IMPL");
-    c->attn_impl = (e && std::strcmp(e, "mma") == 0) ? 0 : ((e && std::strcmp(e, "ptc") == 0) ? 2 : 1);
-    const char* e2 = std::getenv("QCF_SCORE_IMPL");
-    c->score_impl = (e2 && std::strcmp(e2, "mma") == 0) ? 0 : 1;
-    const char* e3 = std::getenv("QCF_ATTN_CLUSTER");
-    const char* e5 = std::getenv("QCF_PDL");
-    c->pdl = (e5 && std::strcmp(e5, "0") == 0) ? 0 : 1;
-    const char* e4 = std::getenv("QCF_GEMM_MT");
-    const int mt = e4 ? std::atoi(e4) : 0;
-    c->gemm_mt = (mt == 1 || mt == 2) ? mt : 0;
-    const int cl = e3 ? std::atoi(e3) : 0;
-    c->attn_cluster = (cl == 1 || cl == 2 || cl == 4) ? cl : 0;
-    c->ratio_hint = 0.3;
-    c->head_shards = 1;
-  }
+  c->pdl = 1; c->gemm_mt = 0; c->attn_cluster = 0;
+  c->ratio_hint = 0.3;
+  c->head_shards = 1;
   c->profiling = 0; c->ev_valid = false;
   c->ev_ring = nullptr; c->ev_count = 0; c->ev = nullptr;
 
@@ -162,16 +148,6 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
             cudaMemset(c->score_row_ctr, 0, row_ctr_n * sizeof(unsigned int)) == cudaSuccess &&
             cudaMalloc(&c->counters, c->n_counters * sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(c->counters, 0, c->n_counters * sizeof(unsigned int)) == cudaSuccess;
-  if (c->attn_impl == 2) {     // experimental persistent attention kernel (opt-in): work list, split-KV partials, counters
-    const size_t slots = static_cast<size_t>(attn_ptc_slots(c));
-    const size_t o_bytes = slots * static_cast<size_t>(128) * lay->head_dim * 4, ml_bytes = slots * 2 * 128 * 4;
-    const size_t items = attn_ptc_items(c);
-    ok = ok && cudaMalloc(&c->ptc_units, attn_ptc_units_bytes(c)) == cudaSuccess &&
-         cudaMalloc(&c->ptc_n_units, 16) == cudaSuccess && cudaMemset(c->ptc_n_units, 0, 16) == cudaSuccess &&
-         cudaMalloc(&c->ptc_part_o, o_bytes + 16) == cudaSuccess && cudaMalloc(&c->ptc_part_ml, ml_bytes + 16) == cudaSuccess &&
-         cudaMalloc(&c->ptc_item_ctr, items * sizeof(unsigned int) + 16) == cudaSuccess &&
-         cudaMemset(c->ptc_item_ctr, 0, items * sizeof(unsigned int) + 16) == cudaSuccess;
-  }
   if (!ok) {
     const cudaError_t le = cudaGetLastError();
     qcf_destroy(c);
@@ -185,7 +161,6 @@ void qcf_destroy(qcf_ctx* c) {
   if (!c) return;
   cudaFree(c->stats_m); cudaFree(c->stats_l); cudaFree(c->score_part); cudaFree(c->counters);
   cudaFree(c->score_lse); cudaFree(c->score_row_ctr);
-  cudaFree(c->ptc_units); cudaFree(c->ptc_n_units); cudaFree(c->ptc_part_o); cudaFree(c->ptc_part_ml); cudaFree(c->ptc_item_ctr);
   if (c->ev_ring) {
     for (int i = 0; i < qcf_ctx::kEvRing; ++i)
       for (int j = 0; j < 6; ++j) if (c->ev_ring[i][j]) cudaEventDestroy(c->ev_ring[i][j]);
@@ -207,7 +182,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
   std::vector<int32_t> n_ctx(batch), n_query(batch), c_req, c_off, c_rot, c_len, c_blk;
   std::vector<int64_t> c_row;
   std::vector<float> rot;      // (cos, sin) interleaved
-  int64_t total_ctx = 0;
+  int64_t total_ctx = 0, pool_row_end = 0;
   int32_t t_stride = 0, n_stride = 0, q_stride = 0;
   // inv_freq_j = theta^(-2j/d) in double (reading (a))
   std::vector<double> inv_freq(half);
@@ -231,6 +206,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
       c_rot.push_back(static_cast<int32_t>(rot_pos));
       c_len.push_back(r.chunk_len[i]);
       c_row.push_back(r.chunk_row[i]);
+      pool_row_end = std::max<int64_t>(pool_row_end, r.chunk_row[i] + r.chunk_len[i]);
       c_blk.push_back(c_blk.back() + (r.chunk_len[i] + kRepoRows - 1) / kRepoRows);
       for (int j = 0; j < half; ++j) {
         const double phi = static_cast<double>(rot_pos) * inv_freq[j];
@@ -256,6 +232,7 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
   qb->t_stride = t_stride; qb->n_stride = n_stride; qb->q_stride = q_stride;
   qb->max_ctx = n_stride; qb->max_query = q_stride; qb->total_ctx = total_ctx;
   qb->repo_blocks = c_blk.back();
+  qb->pool_row_end = pool_row_end;
   qb->h_n_ctx = static_cast<int32_t*>(std::malloc(sizeof(int32_t) * (batch > 0 ? batch : 1)));
   qb->h_n_query = static_cast<int32_t*>(std::malloc(sizeof(int32_t) * (batch > 0 ? batch : 1)));
   if (batch > 0) {
@@ -467,6 +444,25 @@ qcf_status qcf_set_head_shards(qcf_ctx* ctx, int32_t n_shards) {
   return QCF_OK;
 }
 
+qcf_status qcf_debug_set(qcf_ctx* ctx, int32_t knob, int32_t value) {
+  if (!ctx) return QCF_ERR_INVALID_ARG;
+  switch (knob) {
+    case QCF_DEBUG_PDL:
+      ctx->pdl = value != 0;
+      return QCF_OK;
+    case QCF_DEBUG_ATTN_CLUSTER:
+      if (!(value == 0 || value == 1 || value == 2 || value == 4)) return fail(ctx, QCF_ERR_INVALID_ARG, "attention cluster size must be 0, 1, 2 or 4");
+      ctx->attn_cluster = value;
+      return QCF_OK;
+    case QCF_DEBUG_GEMM_MT:
+      if (value < 0 || value > 2) return fail(ctx, QCF_ERR_INVALID_ARG, "GEMM tile height must be 0, 1 or 2");
+      ctx->gemm_mt = value;
+      return QCF_OK;
+    default:
+      return fail(ctx, QCF_ERR_INVALID_ARG, "qcf_debug_set: unknown knob");
+  }
+}
+
 qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable) {
   if (!ctx) return QCF_ERR_INVALID_ARG;
   if (enable && !ctx->ev_ring) {
@@ -504,6 +500,7 @@ qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer
   if (qcf_status st = check_ctx_batch(ctx, b)) return st;
   QCF_REQUIRE(ctx, h != nullptr, "qcf_layer_step_host: args is NULL");
   QCF_REQUIRE(ctx, pool_rows >= 0, "qcf_layer_step_host: pool_rows must be >= 0");
+  QCF_REQUIRE(ctx, b->pool_row_end <= pool_rows, "qcf_layer_step_host: a chunk of the batch lies outside the pool_rows rows of k_pool / v_pool");
   QCF_REQUIRE(ctx, h->k_pool && h->v_pool && h->q_new && h->k_new && h->v_new && h->out && h->sel && h->n_sel,
               "qcf_layer_step_host: NULL tensor pointer");
   QCF_REQUIRE(ctx, !h->is_critical_layer || h->q_probe, "qcf_layer_step_host: q_probe is NULL on a critical layer");

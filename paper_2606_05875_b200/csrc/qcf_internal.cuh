@@ -58,12 +58,10 @@ struct qcf_ctx {
   int device;
   int n_sm;
   int max_batch, max_ctx, max_query;
-  int score_impl;        // 1: tcgen05 kernels (default); 0: legacy mma.sync kernels (QCF_SCORE_IMPL=mma)
-  int attn_impl;         // 2: persistent tcgen05 kernel with a device work list (QCF_ATTN_IMPL=ptc); 1: one CTA per tile (tc);
-                         // 0: legacy mma.sync kernel (mma, for A/B timing)
-  int pdl;               // 1: chain the step's kernels with programmatic dependent launch (default); 0: QCF_PDL=0
-  int gemm_mt;           // GEMM tile height in units of 128 rows: 0 = heuristic, else 1 / 2 (QCF_GEMM_MT)
-  int attn_cluster;      // split-KV cluster size of the tcgen05 attention kernel: 0 = heuristic, else 1/2/4 (QCF_ATTN_CLUSTER)
+  // test-only knobs, set through qcf_debug_set (never read from the environment)
+  int pdl;               // 1: chain the step's kernels with programmatic dependent launch (default); 0: plain launches
+  int gemm_mt;           // GEMM tile height in units of 128 rows: 0 = heuristic, else 1 / 2
+  int attn_cluster;      // split-KV cluster size of the attention kernel: 0 = heuristic, else 1 / 2 / 4
   int head_shards;       // this ctx holds 1/head_shards of the layer's heads (qcf_set_head_shards); scores divide by Hq*shards
   double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
   // workspace (device)
@@ -73,12 +71,6 @@ struct qcf_ctx {
   unsigned int* score_row_ctr;   // pass-1 arrival counters per (request, kv-head, row tile), self-resetting
   float* score_part;     // score pass-2 per-kv-head partial column sums [max_batch][Hkv][max_ctx]
   unsigned int* counters;  // tile counters (zeroed, self-resetting)
-  // persistent attention kernel: work list, split-KV partials, per-item arrival counters (zeroed, self-resetting)
-  void* ptc_units;
-  int32_t* ptc_n_units;
-  float* ptc_part_o;
-  float* ptc_part_ml;
-  unsigned int* ptc_item_ctr;
   size_t n_counters;
   // host staging for qcf_layer_step_host
   struct HostStage* stage;
@@ -103,13 +95,13 @@ struct qcf_batch {
   int32_t max_ctx, max_query;
   int64_t total_ctx;
   int32_t repo_blocks;     // total reposition work items
+  int64_t pool_row_end;    // max over chunks of chunk_row + chunk_len: rows of the pool the batch reads (host-side validation)
   int32_t* h_n_ctx;        // [batch]
   int32_t* h_n_query;      // [batch]
 };
 
 namespace qcf {
 
-constexpr int kScoreSplits = 8;     // key-range splits of the legacy (mma.sync) score statistics pass
 constexpr int kScoreSplitsMax = 32; // upper bound of the tcgen05 pass-1 key splits (sizes the statistics workspace)
 
 // Records `msg` as the last error of ctx (or of this thread's failed qcf_create when ctx == nullptr); returns st.
@@ -133,13 +125,6 @@ cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, co
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
 
-cudaError_t launch_attn_ptc(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
-                            const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
-                            const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
-size_t attn_ptc_units_bytes(const qcf_ctx*);
-size_t attn_ptc_items(const qcf_ctx*);
-int attn_ptc_slots(const qcf_ctx*);
-size_t attn_ptc_slot_bytes(const qcf_ctx*);
 cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
                         __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
 cudaError_t launch_lm_head(const qcf_ctx*, const __nv_bfloat16* w_lm, const __nv_bfloat16* h, int vocab, int hidden, float* logits,
@@ -156,12 +141,6 @@ cudaError_t launch_qknorm_rope(const qcf_ctx*, const __nv_bfloat16* qkv, const _
                                const float2* table, const int32_t* sel, const int32_t* n_sel, int n_ctx, int pos_off,
                                float eps, int n_rows, __nv_bfloat16* q_out, __nv_bfloat16* k_out, __nv_bfloat16* v_out,
                                cudaStream_t);
-
-cudaError_t launch_score_tc(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* q_probe, const __nv_bfloat16* k_f,
-                            float* scores, int accumulate, cudaStream_t);
-cudaError_t launch_attn_tc(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
-                           const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
-                           const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
 
 // ------------------------------------------------------------------------------------------- device helpers
 #ifdef __CUDACC__

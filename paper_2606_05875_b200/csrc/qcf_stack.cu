@@ -291,6 +291,10 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
   STK_REQUIRE(ctx, a->pool_rows >= 0 && a->anchor_rows >= 0 && a->pool_rows <= s->max_pool_rows &&
                        a->anchor_rows <= s->max_pool_rows && static_cast<size_t>(pb->t_stride) <= s->probe_rows,
               "qcf_stack_fuse: pools exceed max_pool_rows of qcf_stack_create");
+  STK_REQUIRE(ctx, mb->pool_row_end <= a->pool_rows, "qcf_stack_fuse: a chunk of the main batch lies outside pool_rows");
+  STK_REQUIRE(ctx, pb->pool_row_end <= a->anchor_rows, "qcf_stack_fuse: a chunk of the probe batch lies outside anchor_rows");
+  // |P| is fixed on the host: floor(rho N).  With stages == 2 the caller's sel / n_sel must hold exactly that many rows
+  // (include/qcf.h); the row count of every stage-2 kernel is derived from it.
   const int k_sel = qcf_n_select(N, a->ratio);
   const int n_rows = k_sel + Lq;
   STK_REQUIRE(ctx, n_rows <= s->max_rows && Lq <= s->max_rows && N + Lq <= s->max_pos,
@@ -432,6 +436,14 @@ qcf_status qcf_stack_fuse(qcf_stack* s, const qcf_batch* mb, const qcf_batch* pb
   if (qcf_status e = qcf_select_topk(ctx, mb, a->scores, a->ratio, a->sel, a->n_sel, cs)) return e;               // Eq. 11
   }
   if (!do2) return QCF_OK;
+  if (!do1) {
+    // stage 2 alone: sel / n_sel come from the caller.  Every row count below is derived from floor(rho N) on the host, so
+    // the caller's |P| must match it (not a hot-path mode: one read-back and synchronisation)
+    int32_t h_n_sel = -1;
+    STK_CUDA(ctx, cudaMemcpyAsync(&h_n_sel, a->n_sel, sizeof(int32_t), cudaMemcpyDeviceToHost, cs));
+    STK_CUDA(ctx, cudaStreamSynchronize(cs));
+    STK_REQUIRE(ctx, h_n_sel == k_sel, "qcf_stack_fuse: stages == 2 needs n_sel[0] == qcf_n_select(N, ratio)");
+  }
 
   // ---- stage 2: pipeline cache fusion.  The loader runs ahead through all remaining layers
   // (every layer has its own destination cache); the compute stream consumes them in order.

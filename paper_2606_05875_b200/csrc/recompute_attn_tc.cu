@@ -127,7 +127,7 @@ template <int D>
 __global__ void __launch_bounds__(kThreads, 2)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v, BatchDev bd, int hq,
                int hkv, int max_tiles, float scale_log2, const int32_t* __restrict__ sel,
-               const int32_t* __restrict__ n_sel, const __nv_bfloat16* __restrict__ q, int q_by_position,
+               const int32_t* __restrict__ n_sel, const __nv_bfloat16* q, int q_by_position,
                __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
   extern __shared__ unsigned char smem_raw[];
   // 128-byte-swizzle atoms need 1024-byte alignment; the launch reserves 1 KB of slack for this round-up
@@ -200,7 +200,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
       src = reinterpret_cast<const uint4*>(q + ((static_cast<size_t>(b) * bd.t_stride + src_row) * hq + g * G + hl) * D);
     }
 #pragma unroll
-    for (int c = 0; c < D / 8; ++c) qv[c] = src ? __ldg(src + c) : make_uint4(0u, 0u, 0u, 0u);
+    // coherent loads: in the stack path q is written by a predecessor this kernel's lifetime overlaps (PDL)
+    for (int c = 0; c < D / 8; ++c) qv[c] = src ? ld_nc_v4(src + c) : make_uint4(0u, 0u, 0u, 0u);
   }
   tc_fence_before();
   __syncthreads();
@@ -598,9 +599,9 @@ bool make_kv_map(CUtensorMap* m, const void* base, int batch, int t_stride, int 
 
 }  // namespace
 
-cudaError_t launch_attn_tc(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
-                           const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
-                           const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t stream) {
+cudaError_t launch_attn(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                        const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
+                        const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t stream) {
   if (b->batch == 0 || b->t_stride == 0) return cudaSuccess;
   const Layout& L = ctx->lay;
   CUtensorMap tm_k, tm_v;

@@ -83,14 +83,14 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
   const int rows = Lq * G;
   int k_begin = 0, k_end = 0, n_j = 0, n_kt = 1;          // n_kt: A tiles this CTA walks (pass 2: key tiles)
   if (PASS == 1) {
-    if (row_tile * BT >= rows) return;
+    if (row_tile * BT >= rows) { pdl_trigger(); pdl_wait(); return; }   // every CTA waits: the grid never completes before its predecessor
     const int span = (((N + a.n_splits - 1) / a.n_splits + BT - 1) / BT) * BT;
     k_begin = split * span;
     k_end = min(N, k_begin + span);
     n_j = k_end > k_begin ? (k_end - k_begin + BT - 1) / BT : 0;
   } else {
     n_kt = min(a.kt_per_cta, (N + BT - 1) / BT - key_tile);
-    if (n_kt <= 0) return;
+    if (n_kt <= 0) { pdl_trigger(); pdl_wait(); return; }
     n_j = (rows + BT - 1) / BT;
   }
 
@@ -482,8 +482,8 @@ cudaError_t launch(const qcf_ctx* ctx, const qcf_batch* b, const CUtensorMap& tm
 
 }  // namespace
 
-cudaError_t launch_score_tc(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* q_probe,
-                            const __nv_bfloat16* k_f, float* scores, int accumulate, cudaStream_t stream) {
+cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* q_probe,
+                         const __nv_bfloat16* k_f, float* scores, int accumulate, cudaStream_t stream) {
   if (b->batch == 0 || b->max_ctx == 0) return cudaSuccess;
   const Layout& L = ctx->lay;
   const int max_rows = b->max_query * L.g;

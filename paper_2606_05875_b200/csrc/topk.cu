@@ -142,11 +142,8 @@ cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* sco
   // up to 48 K keys (192 KB) are cached in shared memory; longer contexts read the remainder from L2
   const int n_cached = b->n_stride < 49152 ? b->n_stride : 49152;
   const size_t smem = static_cast<size_t>(n_cached) * sizeof(uint32_t);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
-    attr_set = true;
-  }
+  // per device / context, so set on every launch (as the other launchers do) rather than once per process
+  cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
   return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode);
 }
 

@@ -212,6 +212,20 @@ def test_topk_synthetic_scores_exact(n, ratio):
 
 # --------------------------------------------------------------------------------------------- a4 + a5
 
+def _assert_attn_close(got, want):
+    """a5 outputs [rows, Hq, d].  north_star: max-abs 2e-2 (bf16 I/O, fp32 accumulate).  With N(0,1) values and a
+    near-uniform softmax over thousands of keys the outputs themselves are ~1/sqrt(p) in size, so the absolute bound
+    alone would let a dropped key tile through on late rows: every (row, head) vector must ALSO agree to 2e-2 of its
+    own norm (one bf16 rounding of P, of V-weighted sums and of the output: ~3 * 2^-9 relative, measured ~5e-3)."""
+    assert got.shape == want.shape
+    if got.size == 0:
+        return
+    assert np.max(np.abs(got - want)) <= 2e-2                                  # north_star: max-abs 2e-2
+    num = np.linalg.norm(got - want, axis=-1)
+    den = np.linalg.norm(want, axis=-1)
+    assert np.all(num <= 2e-2 * den + 1e-3), float(np.max(num / (den + 1e-30)))
+
+
 def _run_recompute(ctx, dw, sel_list, by_position=True, q_new=None, k_new=None, v_new=None):
     sel = torch.zeros_like(dw.sel)
     n_sel = torch.zeros_like(dw.n_sel)
@@ -233,7 +247,7 @@ def _check_recompute(wl, dw, b, sel, sentinel=True):
                        O.widen_bf16(r.v_new), sel=np.asarray(sel, dtype=np.int64))
     n_r = len(sel) + lq
     got = _f64(dw.out[b, :n_r])
-    assert np.max(np.abs(got - ref["out"]), initial=0.0) <= 2e-2          # north_star: max-abs 2e-2
+    _assert_attn_close(got, ref["out"])                                   # north_star max-abs 2e-2 + per-vector relative
     # fused cache: refreshed rows and query rows are byte copies of the fresh rows
     rows = ref["rows"]
     assert np.array_equal(_bits(dw.k_fused[b])[rows], r.k_new[rows])
@@ -299,11 +313,12 @@ def test_recompute_attn_compact_rows():
 
 @pytest.mark.parametrize("ncl", [1, 2, 4])
 @pytest.mark.parametrize("name", ["c1", "t_ragged", "t_batch", "t_mid"])
-def test_recompute_attn_split_kv_cluster(name, ncl, monkeypatch):
+def test_recompute_attn_split_kv_cluster(name, ncl):
     """Split-KV over a 1/2/4-CTA cluster (forced; the default is a host heuristic): same rows, same tolerance, and
     ranks with no key tiles / rows that see none of a rank's keys merge as neutral elements."""
-    monkeypatch.setenv("QCF_ATTN_CLUSTER", str(ncl))
+    binding, _ = _binding()
     wl, ctx, dw = _setup(name)
+    ctx.qcf_debug_set(binding.QCF_DEBUG_ATTN_CLUSTER, ncl)
     rng = np.random.default_rng(11 + ncl)
     sels = []
     for r in wl.requests:
@@ -321,12 +336,10 @@ def test_recompute_attn_split_kv_cluster(name, ncl, monkeypatch):
     assert np.max(np.abs(_f64(out2[0, : r.n_ctx + r.n_query]) - want)) <= 2e-2
 
 
-@pytest.mark.parametrize("impl", ["ptc", "tc"])
 @pytest.mark.parametrize("name", SMALL)
-def test_recompute_attn_impls(name, impl, monkeypatch):
-    """Both tcgen05 attention kernels (the default one-CTA-per-tile kernel and the opt-in persistent work-list kernel
-    with split-KV partials merged by the last arriver) against the oracle on random selections, plus the dense comparator."""
-    monkeypatch.setenv("QCF_ATTN_IMPL", impl)
+def test_recompute_attn_random_selection_and_dense(name):
+    """The attention kernel against the oracle on random selections, plus the dense comparator, plus run-to-run
+    bit-identity (split partials are merged in rank order)."""
     wl, ctx, dw = _setup(name)
     rng = np.random.default_rng(5)
     sels = [np.sort(rng.choice(r.n_ctx, size=O.n_select(r.n_ctx, wl.cfg.ratio), replace=False)) for r in wl.requests]
@@ -338,21 +351,11 @@ def test_recompute_attn_impls(name, impl, monkeypatch):
     torch.cuda.synchronize()
     for b, r in enumerate(wl.requests):
         want = O.full_prefill_attn(O.widen_bf16(r.q_new), O.widen_bf16(r.k_new), O.widen_bf16(r.v_new))
-        assert np.max(np.abs(_f64(out2[b, : r.n_ctx + r.n_query]) - want)) <= 2e-2
-    # repeated launches are bit-identical (split partials are merged in chunk order)
+        _assert_attn_close(_f64(out2[b, : r.n_ctx + r.n_query]), want)
     out3 = torch.zeros_like(dw.out)
     ctx.qcf_full_prefill_attn(dw.batch, dw.q_new, dw.k_new, dw.v_new, out3)
     torch.cuda.synchronize()
     assert torch.equal(out2, out3)
-
-
-@pytest.mark.parametrize("impl", ["ptc", "tc"])
-def test_full_size_c2_attention_impls(impl, monkeypatch):
-    monkeypatch.setenv("QCF_ATTN_IMPL", impl)
-    wl, ctx, dw = _setup("c2")
-    ctx.qcf_layer_step(dw.batch, dw.layer_args())
-    torch.cuda.synchronize()
-    _check_full_size(wl, dw, 0, 31)
 
 
 # --------------------------------------------------------------------------------------------- a6
@@ -542,7 +545,7 @@ def _check_full_size(wl, dw, b, seed):
     samp = _sample_rows(k, lq, seed)
     want = O.recompute_attn(O.widen_bf16(r.q_new[rows[samp]]), rows[samp], k_f, v_f)
     got = _f64(dw.out[b])[samp]
-    assert np.max(np.abs(got - want)) <= 2e-2                                 # north_star: max-abs 2e-2
+    _assert_attn_close(got, want)                                             # north_star max-abs 2e-2 + per-vector relative
     return len(samp)
 
 
@@ -569,6 +572,34 @@ def test_full_size_c4_batched_pool(ratio):
     torch.cuda.synchronize()
     for b in (0, 2):
         _check_full_size(wl, dw, b, 23 + b)
+
+
+def test_full_size_c4_batch16_rho03():
+    """BASELINE configs[3] exactly as `bench.py` times it: all 16 requests in ONE batched launch per stage, rho = 0.3.
+    The launch heuristics depend on the CTA count (a2's key splits / key tiles per CTA, a5's cluster size), so a smaller
+    batch does not reach the paths B = 16 takes.  Scores and the selection are checked in full, attention on the declared
+    row sample, for the first, the last and two seeded requests."""
+    wl, ctx, dw = _setup("c4", ratio=0.3)
+    assert dw.B == 16 and dw.batch.n_ctx[0] == 8192
+    ctx.qcf_layer_step(dw.batch, dw.layer_args())
+    torch.cuda.synchronize()
+    picks = sorted({0, 15} | set(int(x) for x in np.random.default_rng(404).choice(np.arange(1, 15), size=2, replace=False)))
+    for b in picks:
+        assert _check_full_size(wl, dw, b, 40 + b) >= 64 + 128
+    # every request selected floor(0.3 * 8192) = 2457 rows
+    assert dw.n_sel.cpu().tolist() == [2457] * 16
+
+
+def test_layer_step_host_rejects_chunks_outside_the_pool():
+    """include/qcf.h: arguments are validated on the host before any launch — a chunk whose rows lie past pool_rows would
+    make a1 read unstaged memory."""
+    binding, device = _binding()
+    wl, ctx, dw = _setup("t_batch")
+    hw = device.DeviceWorkload(wl, ctx, device="cpu", pin=True)
+    with pytest.raises(binding.QcfError) as e:
+        ctx.qcf_layer_step_host(hw.batch, hw.layer_args(), hw.pool_rows - 1)
+    assert e.value.status == binding.QCF_ERR_INVALID_ARG and "pool" in str(e.value)
+    ctx.qcf_layer_step_host(hw.batch, hw.layer_args(), hw.pool_rows)           # the exact size is accepted
 
 
 # --------------------------------------------------------------------------------------------- ragged batch

@@ -16,6 +16,12 @@ from paper_2606_05875_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
+# Free-running stage 1: stated bound on the relative score error after the probe went through bf16
+# activations, and the selection overlap it allows on the reduced stacks (measured values are printed by the tests)
+FREE_RUNNING_EPS = 5e-2
+FREE_RUNNING_OVERLAP = 0.9
+
+
 
 def _bits(t):
     return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
@@ -78,12 +84,12 @@ def _make(name, max_rows=None):
 
 # ----------------------------------------------------------------------------------------------- qcf_linear
 
-@pytest.mark.parametrize("mt", ["0", "1", "2"])
+@pytest.mark.parametrize("mt", [0, 1, 2])
 @pytest.mark.parametrize("M,N,K", [(200, 768, 512), (131, 1536, 384), (1, 512, 1536), (300, 264, 64), (515, 1032, 4096)])
-def test_linear_store_and_residual(M, N, K, mt, monkeypatch):
-    monkeypatch.setenv("QCF_GEMM_MT", mt)
+def test_linear_store_and_residual(M, N, K, mt):
     binding = _binding()
     ctx = binding.Context(8, 2, 64, 1e6, 1, 1024, 8)
+    ctx.qcf_debug_set(binding.QCF_DEBUG_GEMM_MT, mt)      # force the tile height the heuristic picks at other sizes
     rng = np.random.default_rng(M * 7 + N)
     a = inputs.f32_to_bf16_bits(rng.standard_normal((M, K), dtype=np.float32))
     w = inputs.f32_to_bf16_bits(rng.standard_normal((N, K), dtype=np.float32) * np.float32(K ** -0.5))
@@ -104,11 +110,11 @@ def test_linear_store_and_residual(M, N, K, mt, monkeypatch):
     assert np.all(np.abs(_f64(x) - want) <= 0.5 * _ulp(want) + 2e-5 * np.sqrt(K))
 
 
-@pytest.mark.parametrize("mt", ["0", "1", "2"])
-def test_linear_swiglu(mt, monkeypatch):
-    monkeypatch.setenv("QCF_GEMM_MT", mt)
+@pytest.mark.parametrize("mt", [0, 1, 2])
+def test_linear_swiglu(mt):
     binding = _binding()
     ctx = binding.Context(8, 2, 64, 1e6, 1, 1024, 8)
+    ctx.qcf_debug_set(binding.QCF_DEBUG_GEMM_MT, mt)
     M, F, K = 300, 1160, 384
     rng = np.random.default_rng(9)
     a = inputs.f32_to_bf16_bits(rng.standard_normal((M, K), dtype=np.float32))
@@ -276,14 +282,15 @@ def _to_bits(x):
 
 
 @pytest.mark.parametrize("name", ["s_small", "s_d128"])
-def test_stack_prefill_is_bit_identical_with_and_without_pdl(name, monkeypatch):
+def test_stack_prefill_is_bit_identical_with_and_without_pdl(name):
     """The layer's kernels are chained with programmatic dependent launch (each one's prologue overlaps its
     predecessor's tail).  A stale or early read would change bits: the chained run must equal the serialised one
-    (QCF_PDL=0) exactly, every time."""
+    (qcf_debug_set(QCF_DEBUG_PDL, 0)) exactly, every time."""
+    binding = _binding()
     results = []
     for pdl in ("1", "0"):
-        monkeypatch.setenv("QCF_PDL", pdl)
         wl, ctx, stack = _make(name)
+        ctx.qcf_debug_set(binding.QCF_DEBUG_PDL, int(pdl))
         sp = wl.spec
         t = sp.n_ctx + sp.n_query
         b = ctx.batch([[sp.chunk_len] * sp.n_chunks], [[i * sp.chunk_len for i in range(sp.n_chunks)]], [sp.n_query])
@@ -299,6 +306,31 @@ def test_stack_prefill_is_bit_identical_with_and_without_pdl(name, monkeypatch):
     for hid, kc, vc in results[:-1]:
         assert torch.equal(hid, ref[0])
         assert all(torch.equal(x, y) for x, y in zip(kc, ref[1])) and all(torch.equal(x, y) for x, y in zip(vc, ref[2]))
+
+
+def _check_free_running_selection(tag, got_sel, got_sc, want_sc, k, eps_bound):
+    """Free-running stage 1: the GPU's probe queries went through bf16 activations of the layers below, so
+    its scores differ from the oracle's by a relative eps.  north_star rule applied to the BAND: a position whose oracle
+    score is above s_k (1+eps)/(1-eps) is certainly selected and one below s_{k+1} (1-eps)/(1+eps) certainly is not (any
+    score moved by at most eps cannot cross the threshold); only positions inside the band may differ.  eps is the stated
+    bound; the measured error and overlap are printed (pytest -s) and recorded in DESIGN.md §5."""
+    n = len(want_sc)
+    rel = float(np.max(np.abs(got_sc - want_sc) / np.maximum(want_sc, 1e-300)))
+    want = O.select_topk(want_sc, k)
+    inter = len(np.intersect1d(got_sel, want))
+    srt = np.sort(want_sc)[::-1]
+    gap = float((srt[k - 1] - srt[k]) / srt[k - 1]) if 0 < k < n else float("inf")
+    hi = srt[k - 1] * (1 + eps_bound) / (1 - eps_bound) if 0 < k < n else -np.inf
+    lo = srt[k] * (1 - eps_bound) / (1 + eps_bound) if 0 < k < n else np.inf
+    sure_in = np.nonzero(want_sc > hi)[0]
+    sure_out = np.nonzero(want_sc < lo)[0]
+    band = n - len(sure_in) - len(sure_out)
+    print("[free-running %s] max rel score err %.3e (bound %.1e), k/k+1 gap %.2e, overlap %d/%d = %.4f, band %d of %d positions"
+          % (tag, rel, eps_bound, gap, inter, k, inter / max(k, 1), band, n))
+    assert rel <= eps_bound
+    assert np.all(np.isin(sure_in, got_sel)), "a position clearly above the threshold band was dropped"
+    assert not np.any(np.isin(sure_out, got_sel)), "a position clearly below the threshold band was selected"
+    return rel, inter / max(k, 1), band
 
 
 @pytest.mark.parametrize("name", ["s_small", "s_d128"])
@@ -350,13 +382,11 @@ def test_stack_fuse_pipeline_free_running(name):
     pr = S.probe_stage(emb[wl.query_tokens], k_pic, v_pic, a_idx, a_ptr, layers, cfg, sp.crit_layers, sp.ratio)
     got_sc = scores.cpu().numpy().astype(np.float64)
     assert abs(got_sc.sum() - len(sp.crit_layers)) < 1e-3                      # Eq. 20: one unit of mass per layer in L*
-    # free-running: the probe queries went through bf16 activations of the layers below, so a logit moves by up to
-    # ~2^-8 |s| and the score by that relative amount: 5e-2 relative (teacher-forced a2 parity is 1e-2, test_gpu_parity)
-    np.testing.assert_allclose(got_sc, pr["scores"], rtol=5e-2, atol=1e-7)
     assert int(n_sel[0]) == k_sel == len(pr["sel"])
     got_sel = sel[:k_sel].cpu().numpy().astype(np.int64)
     assert np.array_equal(got_sel, O.select_topk(scores.cpu().numpy(), k_sel))  # integer work: exact on its own scores
-    assert len(np.intersect1d(got_sel, pr["sel"])) >= 0.9 * k_sel               # near-tied scores may swap
+    _, overlap, band = _check_free_running_selection(name, got_sel, got_sc, pr["scores"], k_sel, FREE_RUNNING_EPS)
+    assert overlap >= FREE_RUNNING_OVERLAP
     # stage 2 against the oracle run on the GPU's selection
     rows = np.concatenate([got_sel, np.arange(n, n + lq)])
     x0 = emb[np.concatenate(wl.chunk_tokens + [wl.query_tokens])[rows]]
@@ -422,11 +452,11 @@ def test_stack_fuse_other_selector_views(view):
     pr = S.probe_stage(emb[wl.query_tokens], k_pic, v_pic, a_idx, a_ptr, layers, cfg, crit, sp.ratio)
     got = run.scores.cpu().numpy().astype(np.float64)
     assert abs(got.sum() - len(crit)) < 1e-3
-    np.testing.assert_allclose(got, pr["scores"], rtol=5e-2, atol=1e-7)          # free-running bound
     k_sel = run.k_sel
     got_sel = run.sel[:k_sel].cpu().numpy().astype(np.int64)
     assert np.array_equal(got_sel, O.select_topk(run.scores.cpu().numpy(), k_sel))
-    assert len(np.intersect1d(got_sel, pr["sel"])) >= 0.9 * k_sel
+    _, overlap, band = _check_free_running_selection(view, got_sel, got, pr["scores"], k_sel, FREE_RUNNING_EPS)
+    assert overlap >= FREE_RUNNING_OVERLAP
     # stages issued separately
     run.scores.zero_(); run.hidden.zero_()
     run.fuse(stages=1)
@@ -437,6 +467,12 @@ def test_stack_fuse_other_selector_views(view):
     torch.cuda.synchronize()
     assert torch.equal(run.hidden, ref[2])
     assert all(torch.equal(a, b) for a, b in zip(run.k_fused, ref[3:]))
+    # stage 2 alone with an external selection whose size is not floor(rho N): refused (every row count is host-derived)
+    run.n_sel.fill_(k_sel - 1)
+    with pytest.raises(binding.QcfError) as e:
+        run.fuse(stages=2)
+    assert e.value.status == binding.QCF_ERR_INVALID_ARG and "n_sel" in str(e.value)
+    run.n_sel.fill_(k_sel)
     # bandwidth emulation changes timing only: same bits, and the call takes at least bytes / bandwidth
     import time
     kv_row = sp.n_kv_heads * sp.head_dim * 2
