@@ -13,6 +13,9 @@ What is computed (citations are /root/reference/PAPER.md lines + equation):
                    context positions against the stitched PIC keys of those layers, top-k -> P
   fuse_stage       Eq. 6-7, Fig. 9 stage 2: per layer, rows R = P u U only:
                    projections, refreshed K/V scattered into the fused cache, causal attention over it, MLP
+  decode_step /    generation over KV^Fuse ("the fused KV cache and the user query states are handed to
+  greedy_decode    decoding"; TTFT ends at the first token, decoding continues from it): one new token at
+                   position p attends over cache rows 0..p of every layer and appends its own K/V at row p
 
 The decoder layer is the "Qwen3-8B-shaped" block BASELINE.json names (the paper fixes nothing about it;
 DESIGN.md readings (l), (q)): pre-norm residual block, RMSNorm (eps 1e-6), GQA attention with per-head RMSNorm on
@@ -32,7 +35,10 @@ Pins (tests/test_stack_oracle_pins.py, `-m "not gpu"`): each dense op against to
 MLP; causality (perturbing a later token leaves earlier rows unchanged); prefill at positions shifted by D gives the
 same hidden states and K caches equal to Pi(D) of the unshifted ones (ties the stack's RoPE to Eq. 4);
 single-chunk prompt fused == full prefill at every layer for any P; rho = 1 multi-chunk == full prefill;
-rho = 0 == the probe path with every token an anchor (two independent code paths).
+rho = 0 == the probe path with every token an anchor (two independent code paths);
+decode_step on the caches of a T-token full prefill == the last row of a (T+1)-token full prefill (hidden state and the
+appended K/V), its attention == torch fp64 SDPA of one query row over the cache; greedy_decode == re-running the full
+prefill on the growing sequence and taking the argmax each time (brute force).
 Parity unpinned: selection QUALITY versus the paper's Recall@10 % / F1 (needs datasets and trained weights).
 """
 from __future__ import annotations
@@ -234,3 +240,46 @@ def first_token(x_last: np.ndarray, g_final: np.ndarray, w_lm: np.ndarray, eps: 
     logits = RMSNorm(x_last; g_final) W_lm^T, token = argmax (ties to the lower id).  Returns (token, logits)."""
     logits = linear(rms_norm(np.asarray(x_last, dtype=np.float64), g_final, eps), w_lm)
     return int(np.argmax(logits)), logits
+
+
+# --------------------------------------------------------------------------- decoding over KV^Fuse
+
+
+def decode_step(x_tok: np.ndarray, pos: int, k_cache: Sequence[np.ndarray], v_cache: Sequence[np.ndarray],
+                layers: Sequence[LayerWeights], cfg: StackConfig):
+    """One generated token through the stack: x_tok[hidden] is its embedding, `pos` its request
+    position (= number of rows already in every layer's cache: N + Lq + tokens generated so far).  Per layer: project the
+    single row at position pos, APPEND its bf16 K/V as cache row pos, attend causally over rows 0..pos of that layer's
+    cache (KV^Fuse followed by earlier generated tokens), finish the block.  k_cache[l] / v_cache[l] are [pos, Hkv, d];
+    returns (x_out[hidden], k_cache', v_cache') with caches of pos + 1 rows (new lists; inputs are not modified)."""
+    x = np.asarray(x_tok, dtype=np.float64)[None, :]
+    p = np.array([pos])
+    k_out, v_out = [], []
+    for l, w in enumerate(layers):
+        assert k_cache[l].shape[0] == pos and v_cache[l].shape[0] == pos
+        q, k_new, v_new = layer_qkv(x, p, w, cfg)
+        k_l = np.concatenate([k_cache[l], k_new], 0)
+        v_l = np.concatenate([v_cache[l], v_new], 0)
+        a = O.recompute_attn(q, p, k_l, v_l)                  # the row at position pos sees cache rows j <= pos
+        x = layer_finish(x, a, w, cfg)
+        k_out.append(k_l)
+        v_out.append(v_l)
+    return x[0], k_out, v_out
+
+
+def greedy_decode(first_tok: int, n_new: int, embed: np.ndarray, k_cache: Sequence[np.ndarray],
+                  v_cache: Sequence[np.ndarray], layers: Sequence[LayerWeights], cfg: StackConfig, g_final: np.ndarray,
+                  w_lm: np.ndarray):
+    """Greedy generation after TTFT: `first_tok` is the token first_token() produced from the last query row; each step
+    embeds the previous token, runs decode_step at the next position and takes argmax(RMSNorm(x) W_lm^T) (ties to the lower
+    id).  Returns (tokens[n_new] generated AFTER first_tok, logits[n_new][vocab], k_cache, v_cache)."""
+    toks, logs = [], []
+    tok = int(first_tok)
+    pos = k_cache[0].shape[0]
+    for _ in range(n_new):
+        x, k_cache, v_cache = decode_step(embed[tok], pos, k_cache, v_cache, layers, cfg)
+        tok, lg = first_token(x, g_final, w_lm, cfg.rms_eps)
+        toks.append(tok)
+        logs.append(lg)
+        pos += 1
+    return np.asarray(toks, dtype=np.int64), np.asarray(logs), k_cache, v_cache

@@ -219,3 +219,64 @@ def test_first_token_matches_torch_and_argmax_ties():
     assert tok == int(np.argmax(want))
     w2 = w.copy(); w2[7] = w2[tok]                      # an exact tie: the lower id wins
     assert S.first_token(x, g, w2, 1e-6)[0] == min(7, tok)
+
+
+# ------------------------------------------------------------------------------------------- decoding over KV^Fuse
+
+def test_decode_step_equals_last_row_of_a_longer_full_prefill():
+    """decode_step on the caches of a T-token prefill is, by the causal structure of Eq. 2, the (T+1)-th row of a
+    (T+1)-token prefill: same hidden state, same appended K/V at row T, in every layer.  A wrong position, a cache row
+    dropped or double-counted, or attention that does not include the token's own K/V fails this."""
+    wl, cfg, layers, emb = _stack("s_small")
+    toks = np.concatenate(wl.chunk_tokens)[:37]
+    x_long, ks_long, vs_long = S.full_prefill(emb[toks], layers, cfg)
+    _, ks, vs = S.full_prefill(emb[toks[:-1]], layers, cfg)
+    x, k2, v2 = S.decode_step(emb[toks[-1]], len(toks) - 1, ks, vs, layers, cfg)
+    np.testing.assert_allclose(x, x_long[-1], rtol=1e-9, atol=1e-11)
+    for l in range(cfg.n_layers):
+        assert k2[l].shape[0] == len(toks)
+        np.testing.assert_array_equal(k2[l][:-1], ks[l])           # existing rows untouched
+        np.testing.assert_allclose(k2[l], ks_long[l], rtol=0, atol=1e-12 + 2.0 ** -8 * 1e-6)
+        np.testing.assert_allclose(v2[l], vs_long[l], rtol=0, atol=1e-12 + 2.0 ** -8 * 1e-6)
+    # the inputs were not modified
+    assert ks[0].shape[0] == len(toks) - 1
+
+
+def test_decode_attention_is_single_row_sdpa():
+    """The attention inside decode_step: one query row over [cache ; own K/V] == torch fp64 SDPA (no mask needed: the row
+    is the last one), with GQA head mapping."""
+    wl, cfg, layers, emb = _stack("s_small", 1)
+    w = layers[0]
+    toks = np.concatenate(wl.chunk_tokens)[:21]
+    _, ks, vs = S.full_prefill(emb[toks[:-1]], layers, cfg)
+    x_tok = emb[toks[-1]]
+    pos = len(toks) - 1
+    q, k_new, v_new = S.layer_qkv(x_tok[None], np.array([pos]), w, cfg)
+    t = torch.from_numpy
+    k_l, v_l = np.concatenate([ks[0], k_new]), np.concatenate([vs[0], v_new])
+    a = F.scaled_dot_product_attention(t(q).transpose(0, 1)[None], t(k_l).transpose(0, 1)[None], t(v_l).transpose(0, 1)[None],
+                                       enable_gqa=True)[0].transpose(0, 1).numpy()
+    want = S.layer_finish(x_tok[None], a, w, cfg)[0]
+    got, _, _ = S.decode_step(x_tok, pos, ks, vs, layers, cfg)
+    np.testing.assert_allclose(got, want, rtol=1e-10, atol=1e-12)
+
+
+def test_greedy_decode_equals_brute_force_reprefill():
+    """greedy_decode == the definition of greedy generation written the slow way: re-run the full prefill on the whole
+    growing sequence and take argmax of the last row's logits, token by token."""
+    wl, cfg, layers, emb = _stack("s_small")
+    rng = np.random.default_rng(4)
+    g_final = 1 + 0.1 * rng.standard_normal(cfg.hidden)
+    w_lm = rng.standard_normal((wl.spec.vocab, cfg.hidden)) * 0.05
+    prompt = list(np.concatenate(wl.chunk_tokens)[:19])
+    x, ks, vs = S.full_prefill(emb[prompt], layers, cfg)
+    first, _ = S.first_token(x[-1], g_final, w_lm, cfg.rms_eps)
+    toks, logs, k2, _ = S.greedy_decode(first, 5, emb, ks, vs, layers, cfg, g_final, w_lm)
+    seq = prompt + [first]
+    for i in range(5):
+        xs, _, _ = S.full_prefill(emb[seq], layers, cfg)
+        tok, lg = S.first_token(xs[-1], g_final, w_lm, cfg.rms_eps)
+        np.testing.assert_allclose(logs[i], lg, rtol=1e-8, atol=1e-10)
+        assert tok == toks[i]
+        seq.append(tok)
+    assert k2[0].shape[0] == len(prompt) + 5
