@@ -351,6 +351,31 @@ QCF_API qcf_status qcf_stack_layer(qcf_stack* s, int32_t layer, const qcf_batch*
 QCF_API qcf_status qcf_stack_first_token(qcf_stack* s, const void* hidden, int32_t row, const void* g_final, const void* w_lm,
                                          float* logits, int32_t* token, void* stream);
 
+/* Decoding over KV^Fuse (after fusion "the fused KV cache and the user query states" go to decoding;
+ * TTFT ends at the first token and generation continues from it).
+ *
+ * qcf_decode_attn — single-row GQA attention of ONE new token over rows [0, n_keys) of a layer's cache (the token's own
+ * K/V row, n_keys - 1, included):   out[h] = sum_{j < n_keys} softmax_j(q[h] . k_cache[j][h/G] * scale) v_cache[j][h/G]
+ *   q : dev [Hq][d] bf16;  k_cache, v_cache : dev [>= n_keys][Hkv][d] bf16;  out : dev [Hq][d] bf16;
+ *   lse : dev [Hq] fp32 natural-log-sum-exp, or NULL.  fp32 softmax / accumulation, split over key ranges and merged in
+ *   split order (bit-reproducible).  n_keys >= 1. */
+QCF_API qcf_status qcf_decode_attn(qcf_ctx* ctx, const void* q, const void* k_cache, const void* v_cache, int32_t n_keys,
+                                   void* out, float* lse, void* stream);
+
+/* qcf_stack_decode — n_new greedy tokens, one at a time through every layer:
+ *   token i (i = 0: *token_in, the token qcf_stack_first_token produced; else tokens_out[i-1]) is embedded, sits at request
+ *   position pos0 + i, and per layer: RMSNorm -> QKV projection -> QK-norm + RoPE at that position -> its K/V APPENDED as
+ *   cache row pos0 + i -> qcf_decode_attn over rows 0..pos0+i -> O projection + residual -> RMSNorm -> SwiGLU MLP + residual;
+ *   then tokens_out[i] = argmax_v(RMSNorm(x; g_final) . w_lm[v]) (ties to the lower id), logits[i][:] its fp32 logits.
+ *   token_in : dev int32 [1];  pos0 = rows already in every cache (N + Lq after qcf_stack_fuse / qcf_stack_prefill)
+ *   k_cache, v_cache : host arrays [L] of dev [>= pos0 + n_new][Hkv][d] — the caches qcf_stack_fuse filled (KV^Fuse), with
+ *                      room for the appended rows;  pos0 + n_new <= max_pos of qcf_stack_create
+ *   logits : dev [n_new][vocab] fp32;  tokens_out : dev int32 [n_new]
+ * Launch-only on `stream` (token ids never return to the host between steps). */
+QCF_API qcf_status qcf_stack_decode(qcf_stack* s, const int32_t* token_in, int32_t pos0, int32_t n_new,
+                                    void* const* k_cache, void* const* v_cache, const void* g_final, const void* w_lm,
+                                    float* logits, int32_t* tokens_out, void* stream);
+
 /* The whole online pipeline of Fig. 9 for one request.
  *   stage 1  for l = 0..max(L*): load anchor pool l, stitch (a1'), run U through layer l over the anchor cache
  *            (Eq. 17); for l in L*: load PIC pool l, stitch (a1), score (a2, Eq. 18/20); then top-k (a3, Eq. 11)

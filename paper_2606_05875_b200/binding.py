@@ -23,6 +23,7 @@ EXPORTS = (
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards", "qcf_debug_set",
     "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
+    "qcf_decode_attn", "qcf_stack_decode",
 )
 
 QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
@@ -123,6 +124,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_stack_layer": (i32, [vp, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp]),
         "qcf_stack_fuse": (i32, [vp, vp, vp, C.POINTER(qcf_fuse_args), vp]),
         "qcf_stack_first_token": (i32, [vp, vp, i32, vp, vp, vp, vp, vp]),
+        "qcf_decode_attn": (i32, [vp, vp, vp, vp, i32, vp, vp, vp]),
+        "qcf_stack_decode": (i32, [vp, vp, i32, i32, C.POINTER(vp), C.POINTER(vp), vp, vp, vp, vp, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(lib, name)
@@ -282,6 +285,10 @@ class Context:
     def qcf_set_head_shards(self, n_shards: int):
         self._check(self.lib.qcf_set_head_shards(self.handle, int(n_shards)))
 
+    def qcf_decode_attn(self, q, k_cache, v_cache, n_keys: int, out, lse=None, stream=None):
+        self._check(self.lib.qcf_decode_attn(self.handle, _ptr(q), _ptr(k_cache), _ptr(v_cache), int(n_keys), _ptr(out),
+                                             _ptr(lse), _stream(stream)))
+
     def qcf_debug_set(self, knob: int, value: int):
         self._check(self.lib.qcf_debug_set(self.handle, int(knob), int(value)))
 
@@ -344,6 +351,12 @@ class Stack:
     def qcf_stack_first_token(self, hidden, row: int, g_final, w_lm, logits, token, stream=None):
         self.ctx._check(self.lib.qcf_stack_first_token(self.handle, _ptr(hidden), int(row), _ptr(g_final), _ptr(w_lm),
                                                        _ptr(logits), _ptr(token), _stream(stream)))
+
+    def qcf_stack_decode(self, token_in, pos0: int, n_new: int, k_cache, v_cache, g_final, w_lm, logits, tokens_out,
+                         stream=None):
+        self.ctx._check(self.lib.qcf_stack_decode(self.handle, _ptr(token_in), int(pos0), int(n_new), _ptr_array(k_cache),
+                                                  _ptr_array(v_cache), _ptr(g_final), _ptr(w_lm), _ptr(logits),
+                                                  _ptr(tokens_out), _stream(stream)))
 
     def qcf_stack_fuse(self, main: Batch, probe: Batch, *, k_pic, v_pic, pool_rows: int, k_anchor, v_anchor,
                        anchor_rows: int, crit_layers, ratio: float, tokens, k_fused, v_fused, scores, sel, n_sel,

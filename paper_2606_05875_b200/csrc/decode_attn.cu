@@ -1,0 +1,286 @@
+// Decoding over KV^Fuse (the fused cache and the query states are handed to decoding; PAPER.md:372:
+// TTFT ends at the first token) — single-row GQA attention of ONE new token over a layer's cache:
+//
+//   out[h] = sum_{j < n_keys} softmax_j( q[h] . K[j][h/G] * scale ) V[j][h/G]
+//
+// HBM-bound stream (every K and V row of the layer is read once: 2 * Hkv * d * 2 bytes per key, ~4 flop per byte), so no
+// tensor cores: the key range is split over (n_splits x Hkv) CTAs; a CTA stages 128-key tiles of its kv-head's K and V in
+// shared memory with one bulk async copy (cp.async.bulk, the TMA engine's 1-D mode) per 2*d-byte row, completion on an
+// mbarrier; K_{j+1} is in flight while P_j V_j runs and V_{j+1} while Q K_{j+1}^T runs.
+//   phase 1: thread = key   -> the G logits of its key (q broadcast from shared memory), block max, p = 2^(s - m)
+//   phase 2: thread = dim pair x key group -> o[g][dims] += p[g][key] * V[key][dims]
+// Split partials (m, l, o) go to a workspace; the LAST CTA of a kv-head (arrival counter) merges them in split order
+// (bit-reproducible), normalises and stores bf16.
+#include <cmath>
+
+#include "qcf_internal.cuh"
+#include "sm100_ptx.cuh"
+
+namespace qcf {
+
+namespace {
+
+using namespace ptx;
+
+constexpr int kKeys = 128;             // keys per tile = threads per CTA
+constexpr int kThreads = 128;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+
+template <int D, int G>
+struct DecSmem {
+  static constexpr int kPitch = D * 2 + 16;                  // padded row: 128-bit reads of consecutive rows spread over banks
+  static constexpr int oK = 0;
+  static constexpr int oV = oK + kKeys * kPitch;
+  static constexpr int oQ = oV + kKeys * kPitch;             // q of the G heads, fp32, pre-scaled by scale * log2(e)
+  static constexpr int oP = oQ + G * D * 4;                  // p[key][G]
+  static constexpr int oRed = oP + kKeys * G * 4;            // per-warp tile maxima [4][G], then the o reduction
+  static constexpr int oBar = oRed + 4 * G * 4;
+  static constexpr int kBytes = oBar + 16;
+};
+
+// grid (n_splits, Hkv).  part_o [Hkv][n_splits][G][D], part_ml [Hkv][n_splits][G][2]
+template <int D, int G>
+__global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat16* q, const __nv_bfloat16* k_cache,
+                                                               const __nv_bfloat16* v_cache, int hkv, int n_keys,
+                                                               int tiles_per_split, float scale_log2, float* part_o,
+                                                               float* part_ml, unsigned int* counters,
+                                                               __nv_bfloat16* out, float* lse_out) {
+  using S = DecSmem<D, G>;
+  extern __shared__ __align__(16) unsigned char smem[];
+  constexpr int PAIRS = D / 2;                 // bf16x2 columns of a V row
+  constexpr int KG = kThreads / PAIRS;         // key groups of phase 2 (2 at d = 128, 4 at d = 64)
+  constexpr int KPG = kKeys / KG;              // keys per group
+  const int split = blockIdx.x, n_splits = gridDim.x, g = blockIdx.y;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t barK = sbase + S::oBar, barV = barK + 8;
+  float* s_q = reinterpret_cast<float*>(smem + S::oQ);
+  float* s_p = reinterpret_cast<float*>(smem + S::oP);
+  float* s_red = reinterpret_cast<float*>(smem + S::oRed);
+
+  const int n_tiles_all = (n_keys + kKeys - 1) / kKeys;
+  const int t0 = split * tiles_per_split;
+  const int n_t = max(0, min(tiles_per_split, n_tiles_all - t0));
+  const size_t row_stride = static_cast<size_t>(hkv) * D;          // elements between consecutive keys of one kv-head
+  const __nv_bfloat16* kg = k_cache + static_cast<size_t>(g) * D;
+  const __nv_bfloat16* vg = v_cache + static_cast<size_t>(g) * D;
+
+  if (tid == 0) {
+    mbar_init(barK, 1);
+    mbar_init(barV, 1);
+    fence_barrier_init();
+  }
+  pdl_trigger();
+  pdl_wait();                                   // q and the newest cache row are written by the predecessor kernels
+  // q of this kv-head's G heads -> fp32, pre-scaled (coherent loads: see the PDL note in qcf_internal.cuh)
+  for (int i = tid; i < G * D / 2; i += kThreads) {
+    const uint32_t w = *reinterpret_cast<const volatile uint32_t*>(q + (static_cast<size_t>(g) * G) * D + 2 * i);
+    s_q[2 * i] = bf16lo(w) * scale_log2;
+    s_q[2 * i + 1] = bf16hi(w) * scale_log2;
+  }
+  __syncthreads();
+
+  auto issue = [&](const __nv_bfloat16* base, int off, uint32_t bar, int tile) {
+    const int key0 = (t0 + tile) * kKeys;
+    const int n_valid = min(kKeys, n_keys - key0);
+    if (tid == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(n_valid) * D * 2);
+    if (tid < n_valid)
+      bulk_copy_g2s(sbase + off + tid * S::kPitch, base + static_cast<size_t>(key0 + tid) * row_stride, D * 2, bar);
+  };
+  if (n_t > 0) {
+    issue(kg, S::oK, barK, 0);
+    issue(vg, S::oV, barV, 0);
+  }
+
+  float m_run[G], l_own[G], o[G][2];
+#pragma unroll
+  for (int h = 0; h < G; ++h) { m_run[h] = -INFINITY; l_own[h] = 0.f; o[h][0] = o[h][1] = 0.f; }
+  const int dp = tid % PAIRS, kgrp = tid / PAIRS;
+
+  for (int j = 0; j < n_t; ++j) {
+    const int key0 = (t0 + j) * kKeys;
+    const int key = key0 + tid;
+    const bool valid = key < n_keys;
+    // ---- phase 1: logits of my key
+    mbar_wait(barK, j & 1);
+    float s[G];
+#pragma unroll
+    for (int h = 0; h < G; ++h) s[h] = 0.f;
+    if (valid) {
+      const uint4* krow = reinterpret_cast<const uint4*>(smem + S::oK + tid * S::kPitch);
+#pragma unroll 4
+      for (int c = 0; c < D / 8; ++c) {
+        const uint4 kv = krow[c];
+        const float kf[8] = {bf16lo(kv.x), bf16hi(kv.x), bf16lo(kv.y), bf16hi(kv.y),
+                             bf16lo(kv.z), bf16hi(kv.z), bf16lo(kv.w), bf16hi(kv.w)};
+#pragma unroll
+        for (int h = 0; h < G; ++h) {
+          const float4 qa = *reinterpret_cast<const float4*>(s_q + h * D + c * 8);
+          const float4 qb = *reinterpret_cast<const float4*>(s_q + h * D + c * 8 + 4);
+          float acc = s[h];
+          acc = fmaf(kf[0], qa.x, acc); acc = fmaf(kf[1], qa.y, acc); acc = fmaf(kf[2], qa.z, acc); acc = fmaf(kf[3], qa.w, acc);
+          acc = fmaf(kf[4], qb.x, acc); acc = fmaf(kf[5], qb.y, acc); acc = fmaf(kf[6], qb.z, acc); acc = fmaf(kf[7], qb.w, acc);
+          s[h] = acc;
+        }
+      }
+    } else {
+#pragma unroll
+      for (int h = 0; h < G; ++h) s[h] = -INFINITY;
+    }
+    // block max per head
+#pragma unroll
+    for (int h = 0; h < G; ++h) {
+      float mx = s[h];
+#pragma unroll
+      for (int o2 = 16; o2 > 0; o2 >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o2));
+      if (lane == 0) s_red[warp * G + h] = mx;
+    }
+    __syncthreads();                            // (a) maxima visible; every thread has finished reading the K tile
+    if (j + 1 < n_t) issue(kg, S::oK, barK, j + 1);
+    float alpha[G];
+#pragma unroll
+    for (int h = 0; h < G; ++h) {
+      const float mt = fmaxf(fmaxf(s_red[h], s_red[G + h]), fmaxf(s_red[2 * G + h], s_red[3 * G + h]));
+      const float mn = fmaxf(m_run[h], mt);     // the first key of a split's first tile is always valid: finite
+      alpha[h] = ex2(m_run[h] - mn);            // 2^(-inf) = 0 on the first tile
+      m_run[h] = mn;
+      const float p = ex2(s[h] - mn);           // invalid keys: 2^(-inf) = 0
+      l_own[h] = l_own[h] * alpha[h] + p;
+      s_p[tid * G + h] = p;
+    }
+    // ---- phase 2: o += P V over my key group, my dim pair
+    mbar_wait(barV, j & 1);
+    if (!valid) {
+      // tail rows were not copied: whatever the buffer holds must not meet p = 0 as NaN/inf
+      uint4* vrow = reinterpret_cast<uint4*>(smem + S::oV + tid * S::kPitch);
+#pragma unroll
+      for (int c = 0; c < D / 8; ++c) vrow[c] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    __syncthreads();                            // (b) p and the zeroed tail rows visible
+#pragma unroll
+    for (int h = 0; h < G; ++h) { o[h][0] *= alpha[h]; o[h][1] *= alpha[h]; }
+#pragma unroll 4
+    for (int kk = 0; kk < KPG; ++kk) {
+      const int kr = kgrp * KPG + kk;
+      const uint32_t vw = *reinterpret_cast<const uint32_t*>(smem + S::oV + kr * S::kPitch + dp * 4);
+      const float v0 = bf16lo(vw), v1 = bf16hi(vw);
+#pragma unroll
+      for (int h = 0; h < G; ++h) {
+        const float p = s_p[kr * G + h];
+        o[h][0] = fmaf(p, v0, o[h][0]);
+        o[h][1] = fmaf(p, v1, o[h][1]);
+      }
+    }
+    __syncthreads();                            // (c) V tile, p and s_red are free again
+    if (j + 1 < n_t) issue(vg, S::oV, barV, j + 1);
+  }
+
+  // ---- split partial: l over the block, o over the key groups
+  float* red_o = reinterpret_cast<float*>(smem + S::oK);       // K buffer is drained: [KG][G][D]
+#pragma unroll
+  for (int h = 0; h < G; ++h) {
+    red_o[(kgrp * G + h) * D + 2 * dp] = o[h][0];
+    red_o[(kgrp * G + h) * D + 2 * dp + 1] = o[h][1];
+    float l = l_own[h];
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) l += __shfl_xor_sync(0xffffffffu, l, o2);
+    if (lane == 0) s_red[warp * G + h] = l;
+  }
+  __syncthreads();
+  const size_t slot = static_cast<size_t>(g) * n_splits + split;
+  for (int i = tid; i < G * D; i += kThreads) {
+    float acc = 0.f;
+#pragma unroll
+    for (int kq = 0; kq < KG; ++kq) acc += red_o[kq * G * D + i];
+    part_o[slot * G * D + i] = acc;
+  }
+#pragma unroll
+  for (int h = 0; h < G; ++h) {
+    if (tid == h) {                                                                           // m_run is block-uniform
+      part_ml[(slot * G + h) * 2] = m_run[h];
+      part_ml[(slot * G + h) * 2 + 1] = (s_red[h] + s_red[G + h]) + (s_red[2 * G + h] + s_red[3 * G + h]);
+    }
+  }
+  // ---- last CTA of this kv-head merges the splits in split order
+  __threadfence();
+  __syncthreads();
+  __shared__ int s_last;
+  if (tid == 0) s_last = atomicAdd(counters + g, 1u) == static_cast<unsigned int>(n_splits - 1);
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  float* s_w = reinterpret_cast<float*>(smem + S::oV);           // weights [n_splits][G] (n_splits <= 64 * ... fits the V buffer)
+  float* s_inv = s_p;                                            // 1 / l per head
+  if (tid < G) {
+    float M = -INFINITY;
+    for (int sp = 0; sp < n_splits; ++sp) M = fmaxf(M, __ldcg(part_ml + ((static_cast<size_t>(g) * n_splits + sp) * G + tid) * 2));
+    float L = 0.f;
+    for (int sp = 0; sp < n_splits; ++sp) {
+      const size_t o2 = ((static_cast<size_t>(g) * n_splits + sp) * G + tid) * 2;
+      const float w = ex2(__ldcg(part_ml + o2) - M);             // empty split: m = -inf -> weight 0
+      s_w[sp * G + tid] = w;
+      L = fmaf(__ldcg(part_ml + o2 + 1), w, L);
+    }
+    s_inv[tid] = 1.f / L;
+    if (lse_out) lse_out[g * G + tid] = (M + log2f(L)) * kLn2;
+  }
+  __syncthreads();
+  for (int i = tid; i < G * D; i += kThreads) {
+    const int h = i / D;
+    float acc = 0.f;
+    for (int sp = 0; sp < n_splits; ++sp)
+      acc = fmaf(__ldcg(part_o + (static_cast<size_t>(g) * n_splits + sp) * G * D + i), s_w[sp * G + h], acc);
+    out[(static_cast<size_t>(g) * G) * D + i] = __float2bfloat16_rn(acc * s_inv[h]);
+  }
+  if (tid == 0) counters[g] = 0u;                                // self-resetting
+}
+
+template <int D, int G>
+cudaError_t launch_dg(const qcf_ctx* ctx, const __nv_bfloat16* q, const __nv_bfloat16* k, const __nv_bfloat16* v, int n_keys,
+                      __nv_bfloat16* out, float* lse, cudaStream_t stream) {
+  const Layout& L = ctx->lay;
+  const int n_tiles = (n_keys + kKeys - 1) / kKeys;
+  // about three resident CTAs per SM; at most kDecodeSplitsMax splits per kv-head (workspace)
+  int want = (3 * ctx->n_sm + L.hkv - 1) / L.hkv;
+  if (want > kDecodeSplitsMax) want = kDecodeSplitsMax;
+  if (want > n_tiles) want = n_tiles;
+  if (want < 1) want = 1;
+  const int tps = (n_tiles + want - 1) / want;
+  const int n_splits = (n_tiles + tps - 1) / tps;
+  auto kern = decode_attn_kernel<D, G>;
+  const int smem = DecSmem<D, G>::kBytes;
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  return launch_pdl(ctx->pdl, kern, dim3(n_splits, L.hkv), dim3(kThreads), smem, stream, q, k, v, L.hkv, n_keys, tps,
+                    L.scale * kLog2e, ctx->dec_part_o, ctx->dec_part_ml, ctx->dec_counters, out, lse);
+}
+
+template <int D>
+cudaError_t launch_d(const qcf_ctx* ctx, const __nv_bfloat16* q, const __nv_bfloat16* k, const __nv_bfloat16* v, int n_keys,
+                     __nv_bfloat16* out, float* lse, cudaStream_t stream) {
+  switch (ctx->lay.g) {
+    case 1: return launch_dg<D, 1>(ctx, q, k, v, n_keys, out, lse, stream);
+    case 2: return launch_dg<D, 2>(ctx, q, k, v, n_keys, out, lse, stream);
+    case 4: return launch_dg<D, 4>(ctx, q, k, v, n_keys, out, lse, stream);
+    case 8: return launch_dg<D, 8>(ctx, q, k, v, n_keys, out, lse, stream);
+    case 16: return launch_dg<D, 16>(ctx, q, k, v, n_keys, out, lse, stream);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_decode_attn(const qcf_ctx* ctx, const __nv_bfloat16* q, const __nv_bfloat16* k_cache,
+                               const __nv_bfloat16* v_cache, int n_keys, __nv_bfloat16* out, float* lse, cudaStream_t stream) {
+  if (n_keys <= 0) return cudaErrorInvalidValue;
+  return ctx->lay.d == 128 ? launch_d<128>(ctx, q, k_cache, v_cache, n_keys, out, lse, stream)
+                           : launch_d<64>(ctx, q, k_cache, v_cache, n_keys, out, lse, stream);
+}
+
+}  // namespace qcf

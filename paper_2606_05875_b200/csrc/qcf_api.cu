@@ -129,6 +129,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->stats_m = c->stats_l = c->score_part = c->score_lse = nullptr;
   c->score_row_ctr = nullptr;
   c->counters = nullptr;
+  c->dec_part_o = c->dec_part_ml = nullptr; c->dec_counters = nullptr;
   c->stage = nullptr;
   c->pdl = 1; c->gemm_mt = 0; c->attn_cluster = 0;
   c->ratio_hint = 0.3;
@@ -147,7 +148,11 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
             cudaMalloc(&c->score_row_ctr, row_ctr_n * sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(c->score_row_ctr, 0, row_ctr_n * sizeof(unsigned int)) == cudaSuccess &&
             cudaMalloc(&c->counters, c->n_counters * sizeof(unsigned int)) == cudaSuccess &&
-            cudaMemset(c->counters, 0, c->n_counters * sizeof(unsigned int)) == cudaSuccess;
+            cudaMemset(c->counters, 0, c->n_counters * sizeof(unsigned int)) == cudaSuccess &&
+            cudaMalloc(&c->dec_part_o, static_cast<size_t>(lay->n_q_heads) * kDecodeSplitsMax * lay->head_dim * sizeof(float)) == cudaSuccess &&
+            cudaMalloc(&c->dec_part_ml, static_cast<size_t>(lay->n_q_heads) * kDecodeSplitsMax * 2 * sizeof(float)) == cudaSuccess &&
+            cudaMalloc(&c->dec_counters, static_cast<size_t>(lay->n_kv_heads) * sizeof(unsigned int)) == cudaSuccess &&
+            cudaMemset(c->dec_counters, 0, static_cast<size_t>(lay->n_kv_heads) * sizeof(unsigned int)) == cudaSuccess;
   if (!ok) {
     const cudaError_t le = cudaGetLastError();
     qcf_destroy(c);
@@ -161,6 +166,7 @@ void qcf_destroy(qcf_ctx* c) {
   if (!c) return;
   cudaFree(c->stats_m); cudaFree(c->stats_l); cudaFree(c->score_part); cudaFree(c->counters);
   cudaFree(c->score_lse); cudaFree(c->score_row_ctr);
+  cudaFree(c->dec_part_o); cudaFree(c->dec_part_ml); cudaFree(c->dec_counters);
   if (c->ev_ring) {
     for (int i = 0; i < qcf_ctx::kEvRing; ++i)
       for (int j = 0; j < 6; ++j) if (c->ev_ring[i][j]) cudaEventDestroy(c->ev_ring[i][j]);
@@ -404,6 +410,19 @@ qcf_status qcf_full_prefill_attn(qcf_ctx* ctx, const qcf_batch* b, const void* q
   QCF_CUDA(ctx, launch_attn(ctx, b, nullptr, nullptr, static_cast<const __nv_bfloat16*>(q), 1,
                             static_cast<const __nv_bfloat16*>(k), static_cast<const __nv_bfloat16*>(v),
                             static_cast<__nv_bfloat16*>(out), lse, static_cast<cudaStream_t>(stream)));
+  return QCF_OK;
+}
+
+qcf_status qcf_decode_attn(qcf_ctx* ctx, const void* q, const void* k_cache, const void* v_cache, int32_t n_keys, void* out,
+                           float* lse, void* stream) {
+  if (!ctx) return fail(nullptr, QCF_ERR_INVALID_ARG, "ctx is NULL");
+  QCF_REQUIRE(ctx, n_keys >= 1, "qcf_decode_attn: n_keys must be >= 1 (the token's own K/V row is part of the cache)");
+  QCF_REQUIRE(ctx, q && k_cache && v_cache && out, "qcf_decode_attn: NULL tensor pointer");
+  QCF_REQUIRE(ctx, aligned16(q) && aligned16(k_cache) && aligned16(v_cache) && aligned16(out),
+              "qcf_decode_attn: pointers must be 16-byte aligned");
+  QCF_CUDA(ctx, launch_decode_attn(ctx, static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(k_cache),
+                                   static_cast<const __nv_bfloat16*>(v_cache), n_keys, static_cast<__nv_bfloat16*>(out), lse,
+                                   static_cast<cudaStream_t>(stream)));
   return QCF_OK;
 }
 

@@ -72,6 +72,10 @@ struct qcf_ctx {
   float* score_part;     // score pass-2 per-kv-head partial column sums [max_batch][Hkv][max_ctx]
   unsigned int* counters;  // tile counters (zeroed, self-resetting)
   size_t n_counters;
+  // decode attention: split-KV partials [Hkv][kDecodeSplitsMax][G][d] fp32, (m, l) pairs, per-kv-head arrival counters
+  float* dec_part_o;
+  float* dec_part_ml;
+  unsigned int* dec_counters;
   // host staging for qcf_layer_step_host
   struct HostStage* stage;
   // profiling
@@ -102,6 +106,7 @@ struct qcf_batch {
 
 namespace qcf {
 
+constexpr int kDecodeSplitsMax = 64; // upper bound of the key splits of the decode attention kernel (sizes its workspace)
 constexpr int kScoreSplitsMax = 32; // upper bound of the tcgen05 pass-1 key splits (sizes the statistics workspace)
 
 // Records `msg` as the last error of ctx (or of this thread's failed qcf_create when ctx == nullptr); returns st.
@@ -125,6 +130,9 @@ cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, co
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,
                         const __nv_bfloat16* v_f, __nv_bfloat16* out, float* lse, cudaStream_t);
 
+// single-row GQA attention of one new token over rows [0, n_keys) of a layer's cache [.][Hkv][d]
+cudaError_t launch_decode_attn(const qcf_ctx*, const __nv_bfloat16* q, const __nv_bfloat16* k_cache, const __nv_bfloat16* v_cache,
+                               int n_keys, __nv_bfloat16* out, float* lse, cudaStream_t);
 cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
                         __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
 cudaError_t launch_lm_head(const qcf_ctx*, const __nv_bfloat16* w_lm, const __nv_bfloat16* h, int vocab, int hidden, float* logits,

@@ -252,6 +252,49 @@ qcf_status qcf_stack_first_token(qcf_stack* s, const void* hidden, int32_t row, 
   return QCF_OK;
 }
 
+qcf_status qcf_stack_decode(qcf_stack* s, const int32_t* token_in, int32_t pos0, int32_t n_new, void* const* k_cache,
+                            void* const* v_cache, const void* g_final, const void* w_lm, float* logits, int32_t* tokens_out,
+                            void* stream) {
+  if (!s) return set_error(nullptr, QCF_ERR_INVALID_ARG, "qcf_stack_decode: stack is NULL");
+  qcf_ctx* ctx = s->ctx;
+  const Layout& L = ctx->lay;
+  STK_REQUIRE(ctx, token_in && k_cache && v_cache && g_final && w_lm && logits && tokens_out, "qcf_stack_decode: NULL argument");
+  STK_REQUIRE(ctx, pos0 >= 0 && n_new >= 0, "qcf_stack_decode: pos0 and n_new must be >= 0");
+  STK_REQUIRE(ctx, static_cast<int64_t>(pos0) + n_new <= s->max_pos, "qcf_stack_decode: positions exceed max_pos of qcf_stack_create");
+  STK_REQUIRE(ctx, aligned16(g_final) && aligned16(w_lm), "qcf_stack_decode: pointers must be 16-byte aligned");
+  for (int l = 0; l < s->dims.n_layers; ++l)
+    STK_REQUIRE(ctx, k_cache[l] && v_cache[l] && aligned16(k_cache[l]) && aligned16(v_cache[l]),
+                "qcf_stack_decode: NULL or misaligned cache pointer");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int hid = s->dims.hidden, ffn = s->dims.ffn, vocab = s->dims.vocab;
+  const int qkv_n = (L.hq + 2 * L.hkv) * L.d;
+  const size_t kv_row = static_cast<size_t>(L.hkv) * L.d;
+  auto bf = [](const void* p) { return static_cast<const __nv_bfloat16*>(p); };
+  for (int i = 0; i < n_new; ++i) {
+    const int pos = pos0 + i;
+    const int32_t* tok = i == 0 ? token_in : tokens_out + (i - 1);
+    STK_CUDA(ctx, launch_embed_gather(s->embed, tok, nullptr, nullptr, 0, 0, 1, hid, s->x, st));
+    for (int l = 0; l < s->dims.n_layers; ++l) {
+      const qcf_layer_weights& w = s->layers[l];
+      __nv_bfloat16* kc = static_cast<__nv_bfloat16*>(k_cache[l]);
+      __nv_bfloat16* vc = static_cast<__nv_bfloat16*>(v_cache[l]);
+      STK_CUDA(ctx, launch_rmsnorm(s->x, bf(w.g_attn), s->dims.rms_eps, 1, hid, s->h, st));
+      STK_CUDA(ctx, launch_gemm(ctx, s->h, bf(w.w_qkv), nullptr, s->qkv, 1, qkv_n, hid, QCF_EPI_STORE, st));
+      // QK-norm + RoPE at position pos; the token's K/V land in cache row pos
+      STK_CUDA(ctx, launch_qknorm_rope(ctx, s->qkv, bf(w.g_q), bf(w.g_k), s->rope_table, nullptr, nullptr, 0, pos,
+                                       s->dims.rms_eps, 1, s->q_new, kc + pos * kv_row, vc + pos * kv_row, st));
+      STK_CUDA(ctx, launch_decode_attn(ctx, s->q_new, kc, vc, pos + 1, s->attn, nullptr, st));
+      STK_CUDA(ctx, launch_gemm(ctx, s->attn, bf(w.w_o), s->x, s->x, 1, hid, L.hq * L.d, QCF_EPI_ADD_RESIDUAL, st));
+      STK_CUDA(ctx, launch_rmsnorm(s->x, bf(w.g_ffn), s->dims.rms_eps, 1, hid, s->h, st));
+      STK_CUDA(ctx, launch_gemm(ctx, s->h, bf(w.w_gate_up), nullptr, s->act, 1, 2 * ffn, hid, QCF_EPI_SWIGLU, st));
+      STK_CUDA(ctx, launch_gemm(ctx, s->act, bf(w.w_down), s->x, s->x, 1, hid, ffn, QCF_EPI_ADD_RESIDUAL, st));
+    }
+    STK_CUDA(ctx, launch_rmsnorm(s->x, bf(g_final), s->dims.rms_eps, 1, hid, s->h, st));
+    STK_CUDA(ctx, launch_lm_head(ctx, bf(w_lm), s->h, vocab, hid, logits + static_cast<size_t>(i) * vocab, tokens_out + i, st));
+  }
+  return QCF_OK;
+}
+
 qcf_status qcf_stack_prefill(qcf_stack* s, const qcf_batch* b, const int32_t* tokens, void* const* k_cache,
                              void* const* v_cache, void* hidden_out, void* stream) {
   if (qcf_status e = check_stack_batch(s, b, "qcf_stack_prefill")) return e;

@@ -126,7 +126,7 @@ __device__ __forceinline__ float4 ld_dsmem_f32x4(uint32_t addr) {
 template <int D>
 __global__ void __launch_bounds__(kThreads, 2)
 attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__ CUtensorMap tm_v, BatchDev bd, int hq,
-               int hkv, int max_tiles, float scale_log2, const int32_t* __restrict__ sel,
+               int hkv, int tiles_hint, int unit_grp, float scale_log2, const int32_t* __restrict__ sel,
                const int32_t* __restrict__ n_sel, const __nv_bfloat16* q, int q_by_position,
                __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
   extern __shared__ unsigned char smem_raw[];
@@ -135,24 +135,40 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   using S = Smem<D>;
   const int G = hq / hkv;
   const int PT = BM / G;
-  // 1-D grid, heaviest tiles of ALL (request, kv-head) pairs first: block id -> (tile descending, head, request)
-  // The CTAs of a cluster (consecutive block ids) share one work item and split its key tiles.
+  // 1-D grid of work items (one 128-row tile of one (request, kv-head) "unit"); the CTAs of a cluster (consecutive block
+  // ids) share one item and split its key tiles.  Order = L2 locality first, then heaviest first:
+  //   section A: groups of `unit_grp` consecutive units whose K/V fit in a fraction of the L2; inside a group the tiles
+  //              of all its units from the heaviest (last rows, longest causal extent) down — the CTAs resident at any
+  //              time read the K/V of ONE group (at c4, 16 requests x 34 MB interleaved made every key tile an HBM read:
+  //              18.8 GB of DRAM traffic for 0.55 GB of cache, profiles/r02_c4_base.md);
+  //   section B: tiles past the host's row-count hint `tiles_hint` (the selection size lives on the device), all units —
+  //              normally empty, they retire under the tail.
   pdl_trigger();
   pdl_wait();          // n_sel / sel below are written by the predecessors
   const int ncl = static_cast<int>(cluster_nctarank());
   const int crank = static_cast<int>(cluster_ctarank());
   const int item = static_cast<int>(blockIdx.x) / ncl;
-  const int n_gb = hkv * bd.batch;
-  const int t_idx = item / n_gb;                   // 0 = this request's heaviest (last) row tile
-  const int gb = item % n_gb;
-  const int b = gb / hkv, g = gb % hkv;
+  const int n_units = hkv * bd.batch;
+  const int n_groups = (n_units + unit_grp - 1) / unit_grp;
+  const int items_a = n_groups * tiles_hint * unit_grp;
+  int t_idx, unit;                                  // t_idx 0 = the unit's heaviest (last) row tile
+  if (item < items_a) {
+    const int grp = item / (tiles_hint * unit_grp), rem = item % (tiles_hint * unit_grp);
+    t_idx = rem / unit_grp;
+    unit = grp * unit_grp + rem % unit_grp;
+    if (unit >= n_units) return;                    // the last group may be partial (same decision in every CTA of a cluster)
+  } else {
+    const int rem = item - items_a;
+    t_idx = tiles_hint + rem / n_units;
+    unit = rem % n_units;
+  }
+  const int b = unit / hkv, g = unit % hkv;
   const int N = bd.n_ctx[b], Lq = bd.n_query[b];
   const bool dense = sel == nullptr;
   const int ns = dense ? 0 : ld_ca_s32(n_sel + b);     // coherent loads for everything a predecessor wrote (PDL)
   const int n_rows = dense ? N + Lq : ns + Lq;
   const int n_tiles = (n_rows + PT - 1) / PT;
-  // Heaviest first RELATIVE TO THE REQUEST'S OWN tile count: the CTAs without work (the grid is sized for t_stride rows,
-  // a selective launch fills a third of it) come last and retire under the tail instead of delaying the heavy tiles.
+  // heaviest first RELATIVE TO THE REQUEST'S OWN tile count (the grid is sized for t_stride rows)
   if (t_idx >= n_tiles) return;
   const int tile = n_tiles - 1 - t_idx;
   const int ridx0 = tile * PT;
@@ -627,7 +643,27 @@ cudaError_t launch_attn(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
     const int kt_max = (b->t_stride + BN - 1) / BN;
     ncl = (kt_max >= 16 && items * 4 <= slots) ? 4 : ((kt_max >= 8 && items * 2 <= slots) ? 2 : 1);
   }
-  const dim3 grid(static_cast<unsigned>(max_tiles) * L.hkv * b->batch * ncl);
+  // L2-locality groups (see the kernel's work decode): units whose K + V (t_stride rows of one kv-head each) fit in ~48 MB
+  // of the 126 MB L2 — two consecutive groups overlap at their boundary; whole requests when more than one fits.
+  const int n_units = L.hkv * b->batch;
+  const double unit_bytes = static_cast<double>(b->t_stride) * L.d * 2.0 * 2.0;
+  int unit_grp = static_cast<int>(48.0 * 1024 * 1024 / unit_bytes);
+  if (unit_grp >= L.hkv) unit_grp -= unit_grp % L.hkv;
+  if (unit_grp < 1) unit_grp = 1;
+  if (unit_grp > n_units) unit_grp = n_units;
+  const int n_groups = (n_units + unit_grp - 1) / unit_grp;
+  // row-count hint: |R_b| ~ ratio_hint * N_b + Lq_b in selective mode (the true count is device-side: tiles past the hint
+  // are still covered, in section B of the grid)
+  int tiles_hint = max_tiles;
+  if (sel) {
+    const double rows = ctx->ratio_hint * b->n_stride + b->q_stride;
+    tiles_hint = static_cast<int>(std::ceil(rows / PT)) + 1;
+    if (tiles_hint > max_tiles) tiles_hint = max_tiles;
+    if (tiles_hint < 1) tiles_hint = 1;
+  }
+  const long long n_items = static_cast<long long>(n_groups) * tiles_hint * unit_grp +
+                            static_cast<long long>(max_tiles - tiles_hint) * n_units;
+  const dim3 grid(static_cast<unsigned>(n_items * ncl));
   const float scale_log2 = L.scale * kLog2e;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid;
@@ -648,14 +684,14 @@ cudaError_t launch_attn(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
     auto kern = attn_tc_kernel<128>;
     cfg.dynamicSmemBytes = Smem<128>::kBytes + 1024;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(cfg.dynamicSmemBytes));
-    return cudaLaunchKernelEx(&cfg, kern, tm_k, tm_v, bd, hq, hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position,
-                              out, lse);
+    return cudaLaunchKernelEx(&cfg, kern, tm_k, tm_v, bd, hq, hkv, tiles_hint, unit_grp, scale_log2, sel, n_sel, q,
+                              rows_by_position, out, lse);
   }
   auto kern = attn_tc_kernel<64>;
   cfg.dynamicSmemBytes = Smem<64>::kBytes + 1024;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(cfg.dynamicSmemBytes));
-  return cudaLaunchKernelEx(&cfg, kern, tm_k, tm_v, bd, hq, hkv, max_tiles, scale_log2, sel, n_sel, q, rows_by_position, out,
-                            lse);
+  return cudaLaunchKernelEx(&cfg, kern, tm_k, tm_v, bd, hq, hkv, tiles_hint, unit_grp, scale_log2, sel, n_sel, q,
+                            rows_by_position, out, lse);
 }
 
 }  // namespace qcf

@@ -7,8 +7,11 @@
 //   pass 1 (stats)  : S   = Q_tile K_j^T   query rows on the lanes, key tiles streamed -> per-row (max, sum-exp)
 //   pass 2 (colsum) : S^T = K_tile Q_j^T   KEYS on the lanes, query-row chunks streamed -> per-key sum_r 2^(s - lse_r)
 // Both are the same warp-specialised skeleton: a fixed 128-row operand A and a 2-stage TMA ring of 128-row operands B
-// (128-byte swizzle), S double-buffered in TMEM (2 x 128 fp32 columns), one UMMA-issuing thread, and 128 consumer
-// threads that sweep their own TMEM lane.  GQA packing: a "query row" is (token i, head hl) of one kv-head,
+// (128-byte swizzle), S double-buffered in TMEM (2 x 128 fp32 columns), one UMMA-issuing thread, and 256 consumer
+// threads: two per TMEM lane, each sweeping one 64-column half of the lane (a sweep is bound by MUFU / TMEM-load latency
+// per warp, not by issue slots — ncu on the one-thread-per-lane version: 0.59 eligible warps per cycle and scheduler,
+// XU pipe 68 % / 52 % busy — so twice the warps per SM sub-partition is what fills the pipe; nothing has to be agreed
+// between the two halves inside the loop: each keeps its own lazy reference max / partial column sum).  GQA packing: a "query row" is (token i, head hl) of one kv-head,
 // r = i * G + hl, loaded by TMA boxes {64 elements, G heads, 128/G tokens}.  The Hkv per-head partial column sums are
 // combined in fixed order by the last CTA of each key tile (bit-reproducible scores, deterministic top-k).
 #include <cmath>
@@ -23,7 +26,9 @@ namespace {
 using namespace ptx;
 
 constexpr int BT = 128;            // rows of A, rows of one B tile, fp32 columns of one S buffer
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;       // producer warp, issuer warp, 2 x 4 consumer warps
+constexpr int kConsumers = 256;
+constexpr int HC = BT / 2;          // S columns swept by one consumer thread
 constexpr int kTmemCols = 256;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kStaleSum = 1099511627776.0f;      // 2^40
@@ -45,7 +50,8 @@ struct Smem {
   static constexpr int kNumBar = 10;
   static constexpr int oTmem = oBar + kNumBar * 8;
   static constexpr int oFlag = oTmem + 8;
-  static constexpr int oLse = oFlag + 8;                // pass 2: -lse of ALL query rows of the (request, kv-head), size set at launch
+  static constexpr int oLse = oFlag + 8;                // pass 2: -lse of ALL query rows of the (request, kv-head), then the upper
+                                                        // halves' column sums [2][128] and the last-arriver flags [kt_per_cta]; size set at launch
   static constexpr int kBytes = oLse;
 };
 enum { kAFull = 0, kBFull = 1, kBEmpty = 3, kSFull = 5, kSEmpty = 7, kAEmpty = 9 };
@@ -55,7 +61,7 @@ struct ScoreArgs {
   int hq, hkv, n_splits;
   int norm_heads;                                        // Hq of the WHOLE layer (Hq * head shards): Eq. 18's 1/(Hq Lq)
   int kt_per_cta;                                        // pass 2: key tiles walked by one CTA
-  float* stats_m; float* stats_l; int stats_rows;        // [B][n_splits][stats_rows]
+  float* stats_m; float* stats_l; int stats_rows;        // [B][2 * n_splits][stats_rows]: a key split x a column half
   float* part; int part_stride;                          // [B][Hkv][part_stride]
   unsigned int* counters;
   float* scores; int accumulate;
@@ -110,7 +116,7 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         mbar_init(bar(kBFull + i), 1);
         mbar_init(bar(kBEmpty + i), 1);
         mbar_init(bar(kSFull + i), 1);
-        mbar_init(bar(kSEmpty + i), 128);
+        mbar_init(bar(kSEmpty + i), kConsumers);
       }
       fence_barrier_init();
     }
@@ -188,138 +194,152 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
       }
     }
   } else {
-    // ===================================================================== consumers: one TMEM lane each
-    const int quarter = warp & 3;
+    // ===================================================================== consumers: two threads per TMEM lane
+    const int quarter = warp & 3;                    // a warp may only touch TMEM lanes 32 * (warp % 4) ..
+    const int half = (warp - 2) >> 2;                // which 64-column half of every S tile this thread sweeps
     const int r = quarter * 32 + lane;
-    const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16);
+    const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + half * HC;
+    // One 64-column half of S[st]: sum over its columns of 2^(s * scale + z_c) with z_c = nz[c] (pass 2: -lse of the
+    // chunk's rows, from shared memory) or one scalar (pass 1: -reference max).  Full tiles run on packed pairs (FFMA2 /
+    // FADD2), kMufuPairs of every 4 pairs on MUFU.EX2 and the rest on the FMA pipe; 16-column TMEM loads, double-buffered.
+    auto sweep_full = [&](uint32_t s_addr, const float4* z4, float zs, uint64_t& acc_a, uint64_t& acc_b) {
+      const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2);
+      const uint64_t zs2 = f2_pack(zs, zs);
+      uint32_t sa[16], sb[16];
+      tmem_ld16(s_addr, sa);
+#pragma unroll
+      for (int c = 0; c < HC / 16; ++c) {
+        uint32_t(&sv)[16] = (c & 1) ? sb : sa;
+        tmem_wait_ld();
+        if (c + 1 < HC / 16) tmem_ld16(s_addr + (c + 1) * 16, (c & 1) ? sa : sb);
+#pragma unroll
+        for (int i = 0; i < 16; i += 8) {
+          uint64_t nz[4];
+          if (z4) {
+            const float4 za = z4[c * 4 + (i >> 2)], zb = z4[c * 4 + (i >> 2) + 1];   // same address in every lane: broadcast
+            nz[0] = f2_pack(za.x, za.y); nz[1] = f2_pack(za.z, za.w); nz[2] = f2_pack(zb.x, zb.y); nz[3] = f2_pack(zb.z, zb.w);
+          } else {
+            nz[0] = nz[1] = nz[2] = nz[3] = zs2;
+          }
+          float p[8];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const uint64_t t = f2_fma(f2_pack(__uint_as_float(sv[i + 2 * q]), __uint_as_float(sv[i + 2 * q + 1])), sc2, nz[q]);
+            if (q < kMufuPairs) {
+              float t0, t1;
+              f2_unpack(t, t0, t1);
+              p[2 * q] = ex2(t0); p[2 * q + 1] = ex2(t1);
+            } else {
+              ex2_poly2(t, p[2 * q], p[2 * q + 1]);
+            }
+          }
+          acc_a = f2_add(acc_a, f2_add(f2_pack(p[0], p[1]), f2_pack(p[2], p[3])));
+          acc_b = f2_add(acc_b, f2_add(f2_pack(p[4], p[5]), f2_pack(p[6], p[7])));
+        }
+      }
+    };
+    // the same over the first n_valid (< HC, possibly <= 0) columns only
+    auto sweep_tail = [&](uint32_t s_addr, const float* z, float zs, int n_valid) -> float {
+      float l0 = 0.f, l1 = 0.f;
+#pragma unroll
+      for (int c = 0; c < HC / 16; ++c) {
+        uint32_t sv[16];
+        tmem_ld16(s_addr + c * 16, sv);
+        tmem_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 16; i += 2) {
+          const int col = c * 16 + i;
+          const float z0 = z ? z[col] : zs, z1 = z ? z[col + 1] : zs;
+          l0 += col < n_valid ? ex2(fmaf(__uint_as_float(sv[i]), a.scale_log2, z0)) : 0.f;
+          l1 += col + 1 < n_valid ? ex2(fmaf(__uint_as_float(sv[i + 1]), a.scale_log2, z1)) : 0.f;
+        }
+      }
+      return l0 + l1;
+    };
     if (PASS == 1) {
-      // lane = query row: online (max, sum-exp) over the streamed keys, reference max moved lazily
+      // lane = query row, this thread's key columns: online (max, sum-exp) over the streamed keys, reference max moved lazily
       float m_ref = -INFINITY, l = 0.f;
       for (int j = 0; j < n_j; ++j) {
         const int st = j & 1;
-        const int key0 = k_begin + j * BT;
-        const bool tail = key0 + BT > k_end;
+        const int key0 = k_begin + j * BT + half * HC;               // first key of my columns
+        const int n_valid = k_end - key0;                            // >= HC: all my columns are keys of the range
+        const uint32_t s_addr = lane_addr + st * BT;
         mbar_wait(bar(kSFull + st), (j >> 1) & 1);
         tc_fence_after();
-        // max of this row's scores over the tile's valid keys, log2 units (first tile and the rare rescale only)
+        // max of this row's scores over my valid columns, log2 units (first tile and the rare rescale only)
         auto tile_rowmax = [&]() -> float {
           float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-          for (int c = 0; c < BT / 32; ++c) {
-            uint32_t s[32];
-            tmem_ld32(lane_addr + st * BT + c * 32, s);
+          for (int c = 0; c < HC / 16; ++c) {
+            uint32_t sv[16];
+            tmem_ld16(s_addr + c * 16, sv);
             tmem_wait_ld();
 #pragma unroll
-            for (int i = 0; i < 32; i += 2) {
-              float v0 = __uint_as_float(s[i]), v1 = __uint_as_float(s[i + 1]);
-              if (tail) {
-                const int k = key0 + c * 32 + i;
-                if (k >= k_end) v0 = -INFINITY;
-                if (k + 1 >= k_end) v1 = -INFINITY;
-              }
-              mx0 = fmaxf(mx0, v0); mx1 = fmaxf(mx1, v1);
+            for (int i = 0; i < 16; i += 2) {
+              const int col = c * 16 + i;
+              mx0 = fmaxf(mx0, col < n_valid ? __uint_as_float(sv[i]) : -INFINITY);
+              mx1 = fmaxf(mx1, col + 1 < n_valid ? __uint_as_float(sv[i + 1]) : -INFINITY);
             }
           }
           return fmaxf(mx0, mx1) * a.scale_log2;
         };
-        // sum_k 2^(s_k * scale - ref) over the tile.  Issue-bound, so full tiles run on packed pairs (FFMA2 / FADD2) with
-        // every exponential on the MUFU; no per-element max: a stale reference shows up as a huge (or inf) sum.
+        // no per-element max: a stale reference shows up as a huge (or inf) sum
         auto sweep_sum = [&](float ref) -> float {
-          float total;
-          if (!tail) {
-            const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2), nr2 = f2_pack(-ref, -ref);
+          if (n_valid >= HC) {
             uint64_t la = 0ull, lb = 0ull;
-#pragma unroll
-            uint32_t sa[32], sb[32];                   // chunk c + 1 is in flight while chunk c is processed
-            tmem_ld32(lane_addr + st * BT, sa);
-#pragma unroll
-            for (int c = 0; c < BT / 32; ++c) {
-              uint32_t(&s)[32] = (c & 1) ? sb : sa;
-              tmem_wait_ld();
-              if (c + 1 < BT / 32) tmem_ld32(lane_addr + st * BT + (c + 1) * 32, (c & 1) ? sa : sb);
-#pragma unroll
-              for (int i = 0; i < 32; i += 8) {
-                float p[8];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                  const uint64_t t = f2_fma(f2_pack(__uint_as_float(s[i + 2 * q]), __uint_as_float(s[i + 2 * q + 1])), sc2, nr2);
-                  if (q < kMufuPairs) {
-                    float t0, t1;
-                    f2_unpack(t, t0, t1);
-                    p[2 * q] = ex2(t0); p[2 * q + 1] = ex2(t1);
-                  } else {
-                    ex2_poly2(t, p[2 * q], p[2 * q + 1]);
-                  }
-                }
-                la = f2_add(la, f2_add(f2_pack(p[0], p[1]), f2_pack(p[2], p[3])));
-                lb = f2_add(lb, f2_add(f2_pack(p[4], p[5]), f2_pack(p[6], p[7])));
-              }
-            }
+            sweep_full(s_addr, nullptr, -ref, la, lb);
             float s0, s1;
             f2_unpack(f2_add(la, lb), s0, s1);
-            total = s0 + s1;
-          } else {
-            float l0 = 0.f, l1 = 0.f;
-#pragma unroll
-            for (int c = 0; c < BT / 32; ++c) {
-              uint32_t s[32];
-              tmem_ld32(lane_addr + st * BT + c * 32, s);
-              tmem_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 32; i += 2) {
-                const int k = key0 + c * 32 + i;
-                const float v0 = k < k_end ? __uint_as_float(s[i]) : -INFINITY;
-                const float v1 = k + 1 < k_end ? __uint_as_float(s[i + 1]) : -INFINITY;
-                l0 += ex2(fmaf(v0, a.scale_log2, -ref));
-                l1 += ex2(fmaf(v1, a.scale_log2, -ref));
-              }
-            }
-            total = l0 + l1;
+            return s0 + s1;
           }
-          return total;
+          return sweep_tail(s_addr, nullptr, -ref, n_valid);
         };
-        float tile_sum;
-        if (j == 0) {
-          m_ref = tile_rowmax();                  // the first tile of a non-empty range has >= 1 valid key: finite
-          tile_sum = sweep_sum(m_ref);
-        } else {
-          tile_sum = sweep_sum(m_ref);
-          // fp32 sums do not care how stale the reference is until they overflow: move it when a tile's sum passes 2^40
-          if (__any_sync(0xffffffffu, !(tile_sum <= kStaleSum))) {
-            const float m_t = fmaxf(m_ref, tile_rowmax());
-            l *= ex2(m_ref - m_t);
-            m_ref = m_t;
+        float tile_sum = 0.f;
+        if (n_valid > 0) {
+          if (m_ref == -INFINITY) {
+            m_ref = tile_rowmax();                  // first tile with a valid column of mine: finite
+            tile_sum = sweep_sum(m_ref);
+          } else {
             tile_sum = sweep_sum(m_ref);
           }
+        }
+        // fp32 sums do not care how stale the reference is until they overflow: move it when a tile's sum passes 2^40
+        if (__any_sync(0xffffffffu, !(tile_sum <= kStaleSum))) {
+          const float m_t = fmaxf(m_ref, tile_rowmax());
+          l *= ex2(m_ref - m_t);
+          m_ref = m_t;
+          tile_sum = sweep_sum(m_ref);
         }
         l += tile_sum;
         tc_fence_before();
         mbar_arrive(bar(kSEmpty + st));
       }
+      // the two halves of a row are two more "splits" of the key range: partial (max, sum-exp), combined by pass 2
       const int row = row_tile * BT + r;
       if (row < rows) {
-        const size_t o = (static_cast<size_t>(b) * a.n_splits + split) * a.stats_rows + static_cast<size_t>(g) * rows + row;
-        a.stats_m[o] = m_ref;                      // empty key range: (-inf, 0), neutral in the combine
+        const size_t o = (static_cast<size_t>(b) * (2 * a.n_splits) + 2 * split + half) * a.stats_rows + static_cast<size_t>(g) * rows + row;
+        a.stats_m[o] = m_ref;                      // no valid key: (-inf, 0), neutral in the combine
         a.stats_l[o] = l;
       }
     } else {
-      // lane = key: sum over the streamed query rows of 2^(s * scale - lse_row).  The CTA walks n_kt key tiles of one
-      // (request, kv-head); -lse of every query row is combined from the pass-1 partials ONCE (log2 domain) and kept
-      // in shared memory.
-      for (int row = r; row < n_j * BT; row += BT) {
+      // lane = key, this thread's query-row columns: sum over the streamed rows of 2^(s * scale - lse_row).  The CTA walks
+      // n_kt key tiles of one (request, kv-head); -lse of every query row is combined from the pass-1 partials ONCE
+      // (log2 domain) and kept in shared memory.
+      const int ctid = (warp - 2) * 32 + lane;               // 0..255
+      const int n_parts = 2 * a.n_splits;
+      for (int row = ctid; row < n_j * BT; row += kConsumers) {
         float lse = INFINITY;                                // rows past the end contribute 2^(-inf) = 0
         if (row < rows) {
-          // partials are laid out [split][row]: for a fixed split the 128 threads read consecutive words
-          const size_t o = static_cast<size_t>(b) * a.n_splits * a.stats_rows + static_cast<size_t>(g) * rows + row;
+          // partials are laid out [part][row]: for a fixed part consecutive threads read consecutive words
+          const size_t o = static_cast<size_t>(b) * n_parts * a.stats_rows + static_cast<size_t>(g) * rows + row;
           float M = -INFINITY, L = 0.f;
-          // sixteen splits at a time (the launcher asks for at most sixteen): all loads of a row are issued before the first
-          // is used — one L2 round trip per row instead of one per few splits (this loop was 40 % of the kernel's samples at
-          // c2); the combine order is unchanged, a missing split is the neutral (-inf, 0)
-          for (int s0 = 0; s0 < a.n_splits; s0 += 16) {
+          // sixteen parts at a time: all loads of a row are issued before the first is used — one L2 round trip per row
+          // instead of one per few parts; the combine order is fixed, a missing part is the neutral (-inf, 0)
+          for (int s0 = 0; s0 < n_parts; s0 += 16) {
             float ms[16], ls[16];
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
-              const bool ok = s0 + u < a.n_splits;
+              const bool ok = s0 + u < n_parts;
               const size_t idx = o + static_cast<size_t>(ok ? s0 + u : 0) * a.stats_rows;
               ms[u] = __ldcg(a.stats_m + idx);
               ls[u] = __ldcg(a.stats_l + idx);
@@ -336,82 +356,45 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         }
         s_lse[row] = -lse;
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      volatile int* s_last = reinterpret_cast<volatile int*>(smem + S::oFlag);
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      float* s_half = s_lse + n_j * BT;                      // [2][BT]: column sums of the upper halves, double-buffered
+      int* s_last = reinterpret_cast<int*>(s_half + 2 * BT); // [n_kt]: this CTA was the last of the key tile's Hkv CTAs
       const int n_tiles_b = (bd.n_stride + BT - 1) / BT;
       for (int kt = 0, it = 0; kt < n_kt; ++kt) {
-      uint64_t acc01 = 0ull, acc23 = 0ull;               // packed fp32 pairs of partial column sums
-      for (int j = 0; j < n_j; ++j, ++it) {
-        const int st = it & 1;
-        mbar_wait(bar(kSFull + st), (it >> 1) & 1);
-        tc_fence_after();
-        const float4* lse4 = reinterpret_cast<const float4*>(s_lse + j * BT);       // -lse of the chunk's rows
-        const int n_valid = rows - j * BT;                   // < BT only in the last chunk
-        if (n_valid >= BT) {
-          const uint64_t sc2 = f2_pack(a.scale_log2, a.scale_log2);
-#pragma unroll
-          uint32_t sa[32], sb[32];                     // chunk c + 1 is in flight while chunk c is processed
-          tmem_ld32(lane_addr + st * BT, sa);
-#pragma unroll
-          for (int c = 0; c < BT / 32; ++c) {
-            uint32_t(&s)[32] = (c & 1) ? sb : sa;
-            tmem_wait_ld();
-            if (c + 1 < BT / 32) tmem_ld32(lane_addr + st * BT + (c + 1) * 32, (c & 1) ? sa : sb);
-#pragma unroll
-            for (int i = 0; i < 32; i += 8) {
-              const float4 za = lse4[c * 8 + (i >> 2)], zb = lse4[c * 8 + (i >> 2) + 1];   // same address in every lane: broadcast
-              const uint64_t nz[4] = {f2_pack(za.x, za.y), f2_pack(za.z, za.w), f2_pack(zb.x, zb.y), f2_pack(zb.z, zb.w)};
-              float p[8];
-#pragma unroll
-              for (int q = 0; q < 4; ++q) {
-                const uint64_t t = f2_fma(f2_pack(__uint_as_float(s[i + 2 * q]), __uint_as_float(s[i + 2 * q + 1])), sc2, nz[q]);
-                if (q < kMufuPairs) {
-                  float t0, t1;
-                  f2_unpack(t, t0, t1);
-                  p[2 * q] = ex2(t0); p[2 * q + 1] = ex2(t1);
-                } else {
-                  ex2_poly2(t, p[2 * q], p[2 * q + 1]);
-                }
-              }
-              acc01 = f2_add(acc01, f2_add(f2_pack(p[0], p[1]), f2_pack(p[2], p[3])));
-              acc23 = f2_add(acc23, f2_add(f2_pack(p[4], p[5]), f2_pack(p[6], p[7])));
-            }
-          }
-        } else {
-#pragma unroll
-          for (int c = 0; c < BT / 32; ++c) {
-            uint32_t s[32];
-            tmem_ld32(lane_addr + st * BT + c * 32, s);
-            tmem_wait_ld();
-#pragma unroll
-            for (int i = 0; i < 32; i += 4) {
-              const float4 z = lse4[c * 8 + (i >> 2)];
-              const int col = c * 32 + i;                    // rows past the end hold whatever the buffer holds
-              const float p0 = col < n_valid ? ex2(fmaf(__uint_as_float(s[i]), a.scale_log2, z.x)) : 0.f;
-              const float p1 = col + 1 < n_valid ? ex2(fmaf(__uint_as_float(s[i + 1]), a.scale_log2, z.y)) : 0.f;
-              const float p2 = col + 2 < n_valid ? ex2(fmaf(__uint_as_float(s[i + 2]), a.scale_log2, z.z)) : 0.f;
-              const float p3 = col + 3 < n_valid ? ex2(fmaf(__uint_as_float(s[i + 3]), a.scale_log2, z.w)) : 0.f;
-              acc01 = f2_add(acc01, f2_pack(p0, p1));
-              acc23 = f2_add(acc23, f2_pack(p2, p3));
-            }
-          }
+        uint64_t acc01 = 0ull, acc23 = 0ull;                 // packed fp32 pairs of partial column sums
+        float acc_t = 0.f;
+        for (int j = 0; j < n_j; ++j, ++it) {
+          const int st = it & 1;
+          mbar_wait(bar(kSFull + st), (it >> 1) & 1);
+          tc_fence_after();
+          const float* z = s_lse + j * BT + half * HC;       // -lse of my columns' rows
+          const int n_valid = rows - (j * BT + half * HC);   // < HC only in the last chunk
+          if (n_valid >= HC) sweep_full(lane_addr + st * BT, reinterpret_cast<const float4*>(z), 0.f, acc01, acc23);
+          else acc_t += sweep_tail(lane_addr + st * BT, z, 0.f, n_valid);   // rows past the end hold whatever the buffer holds
+          tc_fence_before();
+          mbar_arrive(bar(kSEmpty + st));
         }
-        tc_fence_before();
-        mbar_arrive(bar(kSEmpty + st));
+        const int kt_abs = key_tile + kt;
+        const int key = kt_abs * BT + r;
+        float a0, a1;
+        f2_unpack(f2_add(acc01, acc23), a0, a1);
+        const float tot = (a0 + a1) + acc_t;
+        if (half == 1) s_half[(kt & 1) * BT + r] = tot;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (half == 0 && key < N)
+          a.part[(static_cast<size_t>(b) * a.hkv + g) * a.part_stride + key] = tot + s_half[(kt & 1) * BT + r];
       }
-      const int kt_abs = key_tile + kt;
-      const int key = kt_abs * BT + r;
-      float a0, a1;
-      f2_unpack(f2_add(acc01, acc23), a0, a1);
-      if (key < N) a.part[(static_cast<size_t>(b) * a.hkv + g) * a.part_stride + key] = a0 + a1;
-      // last CTA of this key tile sums the Hkv partials in fixed order (deterministic)
+      // The last CTA of each key tile sums the Hkv partials in fixed order (deterministic).  ONE fence for all the tiles
+      // this CTA walked (a device-scope fence inside the tile loop was 0.65 stall cycles per issue in the old kernel).
       __threadfence();
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      unsigned int* ctr = a.counters + static_cast<size_t>(b) * n_tiles_b + kt_abs;
-      if (r == 0) *s_last = (atomicAdd(ctr, 1u) == static_cast<unsigned int>(a.hkv - 1));
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      if (*s_last) {
-        __threadfence();
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      for (int kt = ctid; kt < n_kt; kt += kConsumers)
+        s_last[kt] = atomicAdd(a.counters + static_cast<size_t>(b) * n_tiles_b + key_tile + kt, 1u) == static_cast<unsigned int>(a.hkv - 1);
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      __threadfence();
+      for (int kt = half; kt < n_kt; kt += 2) {              // the two consumer groups take alternate tiles
+        if (!s_last[kt]) continue;
+        const int key = (key_tile + kt) * BT + r;
         if (key < N) {
           float sum = 0.f;
           for (int gg = 0; gg < a.hkv; ++gg) sum += __ldcg(a.part + (static_cast<size_t>(b) * a.hkv + gg) * a.part_stride + key);
@@ -419,10 +402,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           float* dst = a.scores + static_cast<size_t>(b) * bd.n_stride + key;
           *dst = a.accumulate ? *dst + v : v;
         }
-        if (r == 0) *ctr = 0u;
+        if (r == 0) a.counters[static_cast<size_t>(b) * n_tiles_b + key_tile + kt] = 0u;     // self-resetting
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");           // s_last is rewritten by the next key tile
-      }   // key tiles
     }
   }
 
@@ -467,7 +448,8 @@ template <int D>
 cudaError_t launch(const qcf_ctx* ctx, const qcf_batch* b, const CUtensorMap& tm_q, const CUtensorMap& tm_k,
                    ScoreArgs a, int row_tiles, int key_tiles, cudaStream_t stream) {
   const int smem1 = Smem<D>::kBytes + 1024;
-  const int smem = smem1 + row_tiles * BT * 4;          // pass 2 keeps -lse of every query row of a (request, kv-head)
+  // pass 2 keeps -lse of every query row of a (request, kv-head), 2 x 128 half sums and one flag per walked key tile
+  const int smem = smem1 + row_tiles * BT * 4 + 2 * BT * 4 + a.kt_per_cta * 4;
   if (row_tiles > 0) {
     auto k1 = score_tc_kernel<D, 1>;
     cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, smem1);
@@ -507,8 +489,8 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
       }
     }
     if (n_splits > key_tiles) n_splits = key_tiles;
-    if (n_splits > kScoreSplitsMax) n_splits = kScoreSplitsMax;
-    if (n_splits > 16) n_splits = 16;          // pass 2 combines the partials of a row in one batch of loads
+    if (2 * n_splits > kScoreSplitsMax) n_splits = kScoreSplitsMax / 2;
+    if (n_splits > 8) n_splits = 8;            // x 2 column halves = 16 partials per row: pass 2 combines them in one batch of loads
     if (n_splits < 1) n_splits = 1;
   }
   // pass 2: key tiles per CTA.  A CTA per key tile is 4 tile steps under a full prologue at c4 (8192 CTAs): walk several.

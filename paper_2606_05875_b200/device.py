@@ -91,7 +91,11 @@ class DeviceWorkload:
             "a1_bytes": 4.0 * row * tot_n,
             "a2_flops": sum(2.0 * lq * hq * n * d for n, lq in zip(self.batch.n_ctx, self.batch.n_query)),
             "a2_bytes": float(row // 2 * tot_n),
+            "a2_exps": float(sum(lq * hq * n for n, lq in zip(self.batch.n_ctx, self.batch.n_query))),
             "a4_bytes": 4.0 * row * n_rows,
+            # a5: the fused K and V of every request once + the Q rows read and the O rows written
+            "a5_bytes": float(sum(2 * row * (n + lq) for n, lq in zip(self.batch.n_ctx, self.batch.n_query))
+                              + 2 * n_rows * hq * d * 2),
             "a5_flops_expected": 4.0 * d * hq * pairs,
             "n_rows": n_rows,
         }

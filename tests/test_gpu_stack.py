@@ -18,8 +18,11 @@ pytestmark = pytest.mark.gpu
 
 # Free-running stage 1: stated bound on the relative score error after the probe went through bf16
 # activations, and the selection overlap it allows on the reduced stacks (measured values are printed by the tests)
-FREE_RUNNING_EPS = 5e-2
-FREE_RUNNING_OVERLAP = 0.9
+FREE_RUNNING_EPS = 1e-2          # measured 0.8e-3 .. 2.3e-3 on the reduced stacks: the north-star score bound holds
+FREE_RUNNING_OVERLAP = 0.99      # measured 100 %
+# free-running logits after every layer ran on bf16 activations: bound relative to the largest logit (measured values are
+# printed by the test and recorded in DESIGN.md §5)
+DECODE_LOGIT_TOL = 1e-2       # measured 1.2e-2 .. 2.2e-2 absolute on logits up to 5 (0.4 % of the largest logit)
 
 
 
@@ -69,7 +72,7 @@ def _oracle_stack(wl, n_layers=None):
     return cfg, layers
 
 
-def _make(name, max_rows=None):
+def _make(name, max_rows=None, extra_pos=0):
     binding = _binding()
     wl = inputs.make_stack_workload(name)
     sp = wl.spec
@@ -77,7 +80,7 @@ def _make(name, max_rows=None):
     ctx = binding.Context(sp.n_q_heads, sp.n_kv_heads, sp.head_dim, sp.rope_theta, 1, max(sp.n_ctx, 1024), sp.n_query)
     dl = _device_layers(wl)
     emb = _dev(wl.embed)
-    stack = binding.Stack(ctx, sp.n_layers, sp.hidden, sp.ffn, sp.vocab, sp.rms_eps, dl, emb, max_rows or t, t,
+    stack = binding.Stack(ctx, sp.n_layers, sp.hidden, sp.ffn, sp.vocab, sp.rms_eps, dl, emb, max_rows or t, t + extra_pos,
                           max_pool_rows=sp.n_ctx)
     return wl, ctx, stack
 
@@ -605,3 +608,132 @@ def test_first_token_parity():
         assert t == tok
     else:
         assert want[t] >= top2[1] - 2 * tol
+
+
+# ----------------------------------------------------------------------------------------------- decoding over KV^Fuse (§8(f).4)
+
+@pytest.mark.parametrize("hq,hkv,d", [(4, 2, 64), (8, 2, 128), (32, 8, 128), (64, 8, 128), (16, 1, 64), (2, 2, 128)])
+@pytest.mark.parametrize("n_keys", [1, 5, 127, 128, 129, 1000, 4100])
+def test_decode_attn_parity(hq, hkv, d, n_keys):
+    """qcf_decode_attn (one new token over a layer's cache) against the oracle's causal attention of a
+    single row at position n_keys - 1: max-abs 2e-2 (north_star) plus the per-vector relative criterion, lse, rows past
+    n_keys never read (poisoned with NaN), run-to-run bit identity (splits merged in split order)."""
+    binding = _binding()
+    ctx = binding.Context(hq, hkv, d, 1e6, 1, 8192, 8)
+    rng = np.random.default_rng(n_keys * 131 + hq * 7 + d)
+    q = inputs.f32_to_bf16_bits(rng.standard_normal((hq, d), dtype=np.float32))
+    k = inputs.f32_to_bf16_bits(rng.standard_normal((n_keys, hkv, d), dtype=np.float32))
+    v = inputs.f32_to_bf16_bits(rng.standard_normal((n_keys, hkv, d), dtype=np.float32))
+    if n_keys > 100:                                              # a few heavy hitters: the softmax is not near-uniform
+        k[rng.choice(n_keys, 5, replace=False)] = inputs.f32_to_bf16_bits(
+            4 * rng.standard_normal((5, hkv, d), dtype=np.float32))
+    pad = np.full((7, hkv, d), 0x7FC0, dtype=np.uint16)           # bf16 NaN rows behind the valid ones
+    kc, vc = _dev(np.concatenate([k, pad])), _dev(np.concatenate([v, pad]))
+    out = torch.full((hq, d), 9.0, dtype=torch.bfloat16, device="cuda")
+    lse = torch.zeros(hq, device="cuda")
+    ctx.qcf_decode_attn(_dev(q), kc, vc, n_keys, out, lse)
+    torch.cuda.synchronize()
+    want, want_lse = O.recompute_attn(O.widen_bf16(q)[None], np.array([n_keys - 1]), O.widen_bf16(k), O.widen_bf16(v),
+                                      return_lse=True)
+    got = _f64(out)
+    assert np.all(np.isfinite(got))
+    assert np.max(np.abs(got - want[0])) <= 2e-2
+    num, den = np.linalg.norm(got - want[0], axis=-1), np.linalg.norm(want[0], axis=-1)
+    assert np.all(num <= 2e-2 * den + 1e-3), float(np.max(num / den))
+    np.testing.assert_allclose(lse.cpu().numpy(), want_lse[0], rtol=0, atol=2e-2)
+    out2 = torch.zeros_like(out)
+    ctx.qcf_decode_attn(_dev(q), kc, vc, n_keys, out2, None)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
+
+
+@pytest.mark.parametrize("name", ["s_small", "s_d128"])
+def test_stack_decode_over_kv_fuse(name):
+    """Closes the TTFT -> generation loop: qcf_stack_fuse fills KV^Fuse, qcf_stack_first_token
+    gives token 0, qcf_stack_decode generates 8 greedy tokens reading and extending those caches.  The oracle runs the same
+    pipeline (stage 2 on the GPU's selection, as in test_stack_fuse_pipeline_free_running) and decodes from ITS caches.
+    Logits within the stated free-running bound; token ids exact wherever the oracle's top-2 logit gap exceeds twice that
+    bound (else the GPU's token must be within the bound of the best); the appended K/V rows against the oracle's."""
+    binding = _binding()
+    n_new = 8
+    wl, ctx, stack = _make(name, extra_pos=n_new)
+    sp = wl.spec
+    cfg, layers = _oracle_stack(wl)
+    emb, k_pic, v_pic = _pic_from_oracle(wl, cfg, layers)
+    n, lq, L = sp.n_ctx, sp.n_query, sp.n_layers
+    hkv, d = sp.n_kv_heads, sp.head_dim
+    a_idx, a_ptr = wl.anchor_idx, wl.anchor_ptr
+    hk = [_dev(_to_bits(np.concatenate(k_pic[l], 0))) for l in range(L)]
+    hv = [_dev(_to_bits(np.concatenate(v_pic[l], 0))) for l in range(L)]
+    anchors = lambda pic: np.concatenate([c[a_idx[a_ptr[i]: a_ptr[i + 1]]] for i, c in enumerate(pic)], 0)
+    ak = [_dev(_to_bits(anchors(k_pic[l]))) for l in range(L)]
+    av = [_dev(_to_bits(anchors(v_pic[l]))) for l in range(L)]
+    lens = [sp.chunk_len] * sp.n_chunks
+    off = [i * sp.chunk_len for i in range(sp.n_chunks)]
+    mb = ctx.batch([lens], [off], [lq])
+    pb = ctx.batch([np.diff(a_ptr)], [a_ptr[:-1]], [lq], chunk_pos=[off])
+    toks = torch.from_numpy(np.concatenate(wl.chunk_tokens + [wl.query_tokens]).astype(np.int32)).cuda()
+    k_sel = binding.qcf_n_select(n, sp.ratio)
+    n_r = k_sel + lq
+    t = n + lq
+    kf = [torch.zeros((t + n_new, hkv, d), dtype=torch.bfloat16, device="cuda") for _ in range(L)]     # room for the new rows
+    vf = [torch.zeros_like(x) for x in kf]
+    scores = torch.zeros(n, device="cuda")
+    sel = torch.zeros(n, dtype=torch.int32, device="cuda")
+    n_sel = torch.zeros(1, dtype=torch.int32, device="cuda")
+    hid = torch.zeros((n_r, sp.hidden), dtype=torch.bfloat16, device="cuda")
+    stack.qcf_stack_fuse(mb, pb, k_pic=hk, v_pic=hv, pool_rows=n, k_anchor=ak, v_anchor=av, anchor_rows=int(a_ptr[-1]),
+                         crit_layers=sp.crit_layers, ratio=sp.ratio, tokens=toks, k_fused=kf, v_fused=vf, scores=scores,
+                         sel=sel, n_sel=n_sel, hidden_out=hid)
+    rng = np.random.default_rng(77)
+    g_bits = inputs.f32_to_bf16_bits(np.float32(1.0) + np.float32(0.1) * rng.standard_normal(sp.hidden, dtype=np.float32))
+    w_bits = inputs.f32_to_bf16_bits(rng.standard_normal((sp.vocab, sp.hidden), dtype=np.float32) * np.float32(0.05))
+    g_fin, w_lm = _dev(g_bits), _dev(w_bits)
+    logits0 = torch.zeros(sp.vocab, device="cuda")
+    tok0 = torch.zeros(1, dtype=torch.int32, device="cuda")
+    stack.qcf_stack_first_token(hid, n_r - 1, g_fin, w_lm, logits0, tok0)
+    logits = torch.zeros((n_new, sp.vocab), device="cuda")
+    toks_out = torch.full((n_new,), -1, dtype=torch.int32, device="cuda")
+    stack.qcf_stack_decode(tok0, t, n_new, kf, vf, g_fin, w_lm, logits, toks_out)
+    torch.cuda.synchronize()
+
+    # ---- oracle: stage 2 on the GPU's selection -> KV^Fuse per layer + final hidden -> first token -> greedy decode
+    got_sel = sel[:k_sel].cpu().numpy().astype(np.int64)
+    rows = np.concatenate([got_sel, np.arange(n, n + lq)])
+    x = emb[np.concatenate(wl.chunk_tokens + [wl.query_tokens])[rows]]
+    ks, vs = [], []
+    for l in range(L):
+        k_ctx, v_ctx = O.reposition(k_pic[l], v_pic[l], sp.rope_theta)
+        r = S.fuse_layer(x, rows, k_sel, k_ctx, v_ctx, layers[l], cfg)
+        x = r["x"]
+        ks.append(r["k_fused"]); vs.append(r["v_fused"])
+    G, W = O.widen_bf16(g_bits), O.widen_bf16(w_bits)
+    first, lg0 = S.first_token(x[-1], G, W, sp.rms_eps)
+    want_toks, want_logits, k2, v2 = S.greedy_decode(first, n_new, emb, ks, vs, layers, cfg, G, W)
+
+    tol = DECODE_LOGIT_TOL * max(1.0, float(np.abs(want_logits).max()))
+    def check_token(got_tok, got_lg, want_lg, tag):
+        err = float(np.max(np.abs(got_lg - want_lg)))
+        top2 = np.sort(want_lg)[-2:]
+        print("[decode %s %s] max|logit err| %.3e (tol %.3e), oracle top-2 gap %.3e" % (name, tag, err, tol, top2[1] - top2[0]))
+        assert err <= tol
+        assert got_tok == int(np.argmax(got_lg)), "argmax of its own logits"
+        if top2[1] - top2[0] > 2 * tol:
+            assert got_tok == int(np.argmax(want_lg))
+        else:
+            assert want_lg[got_tok] >= top2[1] - 2 * tol
+        return got_tok == int(np.argmax(want_lg))
+
+    same = check_token(int(tok0[0]), logits0.cpu().numpy().astype(np.float64), lg0, "first")
+    got_toks = toks_out.cpu().numpy()
+    got_logits = logits.cpu().numpy().astype(np.float64)
+    for i in range(n_new):
+        if not same:
+            break                       # a justified near-tie flip: the two sequences legitimately diverge from here
+        same = check_token(int(got_toks[i]), got_logits[i], want_logits[i], "step %d" % i)
+        # the K/V rows this token appended (free-running bound of DESIGN.md §5 for caches)
+        for l in (0, L - 1):
+            assert _rel_rms_err(_f64(kf[l][t + i])[None].reshape(1, -1), k2[l][t + i][None].reshape(1, -1)) <= 5e-2
+            assert _rel_rms_err(_f64(vf[l][t + i])[None].reshape(1, -1), v2[l][t + i][None].reshape(1, -1)) <= 5e-2
+    # KV^Fuse itself was not disturbed by decoding
+    assert _rel_rms_err(_f64(kf[L - 1][:t]).reshape(t, -1), ks[L - 1].reshape(t, -1)) <= 5e-2
