@@ -509,6 +509,13 @@ def run_head_sharded(args) -> None:
     st = sharded.HeadShardedStep(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, max(cfg.batch, 1),
                                  max(cfg.n_ctx, 1024), max(cfg.n_query, 1), rank=rank, world=world)
     dw = device.DeviceWorkload(inputs.shard_heads(wl, rank, world), st.ctx, device=dev)
+    exchange = "none"
+    if world > 1:
+        # the score exchange fused into a2 over peer memory (include/qcf.h, qcf_set_score_exchange); NCCL is the rendezvous
+        slot = dw.batch.batch * dw.batch.n_stride
+        mine = sharded.HeadShardedStep.alloc_exchange_buffer(world, slot, device=dev)
+        st.enable_fused_exchange(sharded.share_exchange_buffers(mine, rank, world), slot)
+        exchange = "fused into a2 (peer stores + flags), %d B per rank and step" % (slot * 4 * (world - 1))
     kw = dict(k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused, q_probe=dw.q_probe,
               scores=dw.scores, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new, out=dw.out,
               ratio=cfg.ratio)
@@ -544,8 +551,7 @@ def run_head_sharded(args) -> None:
                 "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
                 "scaling": "strong", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
                 "config": dict(config_dict(wl.cfg, world, l2="flushed before every timed step"),
-                               parallelism="kv-head shards x%d, all-reduce(sum) of scores (%d B) per step" %
-                                           (world, dw.scores.numel() * 4)),
+                               parallelism="kv-head shards x%d, score exchange: %s" % (world, exchange)),
                 "clocks": clocks, "gpu_launches": KERNELS_PER_STEP * args.steps}
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -159,6 +159,28 @@ QCF_API qcf_status qcf_score(qcf_ctx* ctx, const qcf_batch* b, const void* q_pro
  * scores, so every rank selects the same P.  n_shards in [1, 64]; 1 (the default) restores the plain behaviour. */
 QCF_API qcf_status qcf_set_head_shards(qcf_ctx* ctx, int32_t n_shards);
 
+/* The same step with the score exchange FUSED into a2 instead of a collective call between two launches (SURVEY.md
+ * section 8(f).4): every rank owns an exchange buffer of qcf_score_exchange_bytes(n_shards, slot_elems) bytes, laid out
+ *     [64 x uint32 flags][n_shards slots x slot_elems fp32],     slot_elems >= B * n_stride of every batch used,
+ * and `peer_bufs[p]` (host array [n_shards]) is rank p's buffer AS MAPPED INTO THIS PROCESS (its own allocation for
+ * p == rank; cudaIpcOpenMemHandle / peer access over NVLink for the others).  After this call, on this ctx:
+ *   qcf_score        besides writing `scores` as before, the combine CTAs store this rank's (accumulated) partial
+ *                    I_rank(t) straight into slot `rank` of EVERY rank's buffer (plain st.global on peer pointers), and a
+ *                    one-thread tail kernel then publishes a monotonically increasing epoch in flag[rank] of every
+ *                    buffer with a system-scope release — no NCCL call, no host involvement;
+ *   qcf_select_topk  waits (system-scope acquire, bounded: a missing peer traps after ~2 s instead of hanging) until all
+ *                    n_shards flags of ITS OWN buffer have reached the current epoch, then ranks the element-wise sum
+ *                    of the n_shards slots, added in slot order (every rank forms bit-identical sums and selects the
+ *                    same P); its `scores` argument is ignored.
+ * Ranks must issue the same sequence of exchanging qcf_score calls (the epoch counts them).  n_shards == 1 or
+ * peer_bufs == NULL turns the exchange off.  Not CUDA-graph capturable (the epoch is a launch argument).
+ * Unmeasured on > 1 GPU in this repository (one GPU per box); tested with two contexts on one GPU and with two
+ * PROCESSES sharing one GPU through CUDA IPC handles, their phases ordered on the host so that no kernel ever spins on
+ * a flag another process has yet to write. */
+QCF_API int64_t qcf_score_exchange_bytes(int32_t n_shards, int64_t slot_elems);
+QCF_API qcf_status qcf_set_score_exchange(qcf_ctx* ctx, int32_t rank, int32_t n_shards, void* const* peer_bufs,
+                                          int64_t slot_elems);
+
 /* ------------------------------------------------------------------------------------------------ a3 */
 
 /* Eq. 11: per request, the k_b = qcf_n_select(N_b, ratio) context positions with the

@@ -23,7 +23,7 @@ EXPORTS = (
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards", "qcf_debug_set",
     "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
-    "qcf_decode_attn", "qcf_stack_decode",
+    "qcf_decode_attn", "qcf_stack_decode", "qcf_score_exchange_bytes", "qcf_set_score_exchange",
 )
 
 QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
@@ -114,6 +114,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_set_profiling": (i32, [vp, i32]),
         "qcf_set_head_shards": (i32, [vp, i32]),
         "qcf_debug_set": (i32, [vp, i32, i32]),
+        "qcf_score_exchange_bytes": (i64, [i32, i64]),
+        "qcf_set_score_exchange": (i32, [vp, i32, i32, C.POINTER(vp), i64]),
         "qcf_get_stage_ms": (i32, [vp, C.POINTER(C.c_float)]),
         "qcf_anchor_rank": (i32, [vp, vp, vp, i32, f64, vp, i32, i32, vp, vp, vp]),
         "qcf_linear": (i32, [vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]),
@@ -152,6 +154,10 @@ def _stream(stream) -> Optional[int]:
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
+
+
+def qcf_score_exchange_bytes(n_shards: int, slot_elems: int) -> int:
+    return int(load_library().qcf_score_exchange_bytes(int(n_shards), int(slot_elems)))
 
 
 def qcf_n_select(n_ctx: int, ratio: float) -> int:
@@ -291,6 +297,16 @@ class Context:
 
     def qcf_debug_set(self, knob: int, value: int):
         self._check(self.lib.qcf_debug_set(self.handle, int(knob), int(value)))
+
+    def qcf_set_score_exchange(self, rank: int, n_shards: int, peer_bufs, slot_elems: int):
+        """peer_bufs: sequence of n_shards device pointers / tensors (rank p's exchange buffer mapped into this process);
+        None turns the exchange off."""
+        if peer_bufs is None:
+            self._check(self.lib.qcf_set_score_exchange(self.handle, 0, 1, None, 0))
+            return
+        self._exch_keep = list(peer_bufs)
+        self._check(self.lib.qcf_set_score_exchange(self.handle, int(rank), int(n_shards), _ptr_array(self._exch_keep),
+                                                    int(slot_elems)))
 
     def qcf_set_profiling(self, enable: bool):
         self._check(self.lib.qcf_set_profiling(self.handle, int(bool(enable))))

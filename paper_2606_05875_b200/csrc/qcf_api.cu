@@ -132,6 +132,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->dec_part_o = c->dec_part_ml = nullptr; c->dec_counters = nullptr;
   c->stage = nullptr;
   c->pdl = 1; c->gemm_mt = 0; c->attn_cluster = 0;
+  c->exch_rank = 0; c->exch_world = 1; c->exch_slot_elems = 0; c->exch_peers = nullptr; c->exch_epoch = 0;
   c->ratio_hint = 0.3;
   c->head_shards = 1;
   c->profiling = 0; c->ev_valid = false;
@@ -167,6 +168,7 @@ void qcf_destroy(qcf_ctx* c) {
   cudaFree(c->stats_m); cudaFree(c->stats_l); cudaFree(c->score_part); cudaFree(c->counters);
   cudaFree(c->score_lse); cudaFree(c->score_row_ctr);
   cudaFree(c->dec_part_o); cudaFree(c->dec_part_ml); cudaFree(c->dec_counters);
+  cudaFree(c->exch_peers);
   if (c->ev_ring) {
     for (int i = 0; i < qcf_ctx::kEvRing; ++i)
       for (int j = 0; j < 6; ++j) if (c->ev_ring[i][j]) cudaEventDestroy(c->ev_ring[i][j]);
@@ -339,9 +341,15 @@ qcf_status qcf_score(qcf_ctx* ctx, const qcf_batch* b, const void* q_probe, cons
   QCF_REQUIRE(ctx, k_fused && scores, "qcf_score: NULL tensor pointer");
   QCF_REQUIRE(ctx, q_probe || b->q_stride == 0, "qcf_score: q_probe is NULL");
   QCF_REQUIRE(ctx, aligned16(q_probe) && aligned16(k_fused), "qcf_score: pointers must be 16-byte aligned");
+  if (ctx->exch_world > 1) {
+    QCF_REQUIRE(ctx, static_cast<long long>(b->batch) * b->n_stride <= ctx->exch_slot_elems,
+                "qcf_score: the batch does not fit a slot of the score exchange buffers");
+    ctx->exch_epoch++;
+  }
   QCF_CUDA(ctx, launch_score(ctx, b, static_cast<const __nv_bfloat16*>(q_probe),
                              static_cast<const __nv_bfloat16*>(k_fused), scores, accumulate != 0,
                              static_cast<cudaStream_t>(stream)));
+  if (ctx->exch_world > 1) QCF_CUDA(ctx, launch_exchange_flags(ctx, static_cast<cudaStream_t>(stream)));
   return QCF_OK;
 }
 
@@ -351,7 +359,7 @@ qcf_status qcf_select_topk(qcf_ctx* ctx, const qcf_batch* b, const float* scores
   QCF_REQUIRE(ctx, ratio >= 0.0 && ratio <= 1.0, "qcf_select_topk: ratio must be in [0, 1]");
   if (b->batch == 0) return QCF_OK;
   QCF_REQUIRE(ctx, n_sel != nullptr, "qcf_select_topk: n_sel is NULL");
-  QCF_REQUIRE(ctx, (scores && sel) || b->n_stride == 0, "qcf_select_topk: NULL tensor pointer");
+  QCF_REQUIRE(ctx, ((scores || ctx->exch_world > 1) && sel) || b->n_stride == 0, "qcf_select_topk: NULL tensor pointer");
   ctx->ratio_hint = ratio;
   QCF_CUDA(ctx, launch_topk(ctx, b, scores, ratio, sel, n_sel, static_cast<cudaStream_t>(stream)));
   return QCF_OK;
@@ -480,6 +488,31 @@ qcf_status qcf_debug_set(qcf_ctx* ctx, int32_t knob, int32_t value) {
     default:
       return fail(ctx, QCF_ERR_INVALID_ARG, "qcf_debug_set: unknown knob");
   }
+}
+
+int64_t qcf_score_exchange_bytes(int32_t n_shards, int64_t slot_elems) {
+  if (n_shards < 1 || n_shards > 64 || slot_elems < 0) return -1;
+  return static_cast<int64_t>(kExchHeaderElems) * 4 + static_cast<int64_t>(n_shards) * slot_elems * 4;
+}
+
+qcf_status qcf_set_score_exchange(qcf_ctx* ctx, int32_t rank, int32_t n_shards, void* const* peer_bufs, int64_t slot_elems) {
+  if (!ctx) return QCF_ERR_INVALID_ARG;
+  if (n_shards == 1 || peer_bufs == nullptr) {                  // off
+    ctx->exch_world = 1; ctx->exch_rank = 0; ctx->exch_slot_elems = 0;
+    return QCF_OK;
+  }
+  QCF_REQUIRE(ctx, n_shards >= 2 && n_shards <= 64 && rank >= 0 && rank < n_shards, "qcf_set_score_exchange: rank / n_shards out of range");
+  QCF_REQUIRE(ctx, slot_elems >= 1, "qcf_set_score_exchange: slot_elems must be >= 1");
+  for (int p = 0; p < n_shards; ++p)
+    QCF_REQUIRE(ctx, peer_bufs[p] != nullptr && aligned16(peer_bufs[p]), "qcf_set_score_exchange: NULL or misaligned peer buffer");
+  if (!ctx->exch_peers) QCF_CUDA(ctx, cudaMalloc(&ctx->exch_peers, 64 * sizeof(float*)));
+  for (int p = 0; p < 64; ++p) ctx->exch_peers_host[p] = p < n_shards ? static_cast<float*>(peer_bufs[p]) : nullptr;
+  QCF_CUDA(ctx, cudaMemcpy(ctx->exch_peers, ctx->exch_peers_host, 64 * sizeof(float*), cudaMemcpyHostToDevice));
+  ctx->exch_rank = rank; ctx->exch_world = n_shards; ctx->exch_slot_elems = slot_elems;
+  ctx->exch_epoch = 0;
+  // flags of the own buffer start at 0 (epochs count from 1)
+  QCF_CUDA(ctx, cudaMemset(peer_bufs[rank], 0, kExchHeaderElems * 4));
+  return QCF_OK;
 }
 
 qcf_status qcf_set_profiling(qcf_ctx* ctx, int32_t enable) {

@@ -64,6 +64,13 @@ struct qcf_ctx {
   int attn_cluster;      // split-KV cluster size of the attention kernel: 0 = heuristic, else 1 / 2 / 4
   int head_shards;       // this ctx holds 1/head_shards of the layer's heads (qcf_set_head_shards); scores divide by Hq*shards
   double ratio_hint;     // rho of the most recent qcf_select_topk on this ctx (scheduling hint only; 0.3 until then)
+  // fused score exchange of the KV-head-sharded step (qcf_set_score_exchange): rank r of exch_world; exch_peers (device
+  // array [exch_world] of pointers, mirrored on the host) = every rank's exchange buffer as mapped into THIS process
+  int exch_rank, exch_world;
+  long long exch_slot_elems;
+  float* exch_peers_host[64];
+  float** exch_peers;          // device copy
+  unsigned int exch_epoch;     // incremented by every exchanging qcf_score; the flag value peers wait for
   // workspace (device)
   float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]
   float* stats_l;        // score pass-1 partial row sum-exp
@@ -119,6 +126,9 @@ cudaError_t launch_score(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* 
                          float* scores, int accumulate, cudaStream_t);
 cudaError_t launch_topk(const qcf_ctx*, const qcf_batch*, const float* scores, double ratio, int32_t* sel,
                         int32_t* n_sel, cudaStream_t, int ceil_mode = 0);
+// after a2 on an exchanging ctx: publish `epoch` in flag[rank] of every peer's exchange buffer (system-scope release)
+cudaError_t launch_exchange_flags(const qcf_ctx*, cudaStream_t);
+constexpr int kExchHeaderElems = 64;   // 64 x 4 B of flags in front of the slots of an exchange buffer
 // G_i(r) of Eq. 14 for every chunk row of the batch (rule 0: sink, 1: knorm) into scores[B][n_stride]
 cudaError_t launch_anchor_scores(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool, int rule, int accumulate,
                                  float* scores, cudaStream_t);

@@ -65,6 +65,8 @@ struct ScoreArgs {
   float* part; int part_stride;                          // [B][Hkv][part_stride]
   unsigned int* counters;
   float* scores; int accumulate;
+  // fused exchange of the KV-head-sharded step: the combined value also goes to slot exch_rank of every rank's buffer
+  float* const* exch_peers; int exch_rank, exch_world; long long exch_slot_elems;
 };
 
 template <int D, int PASS>
@@ -400,7 +402,13 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           for (int gg = 0; gg < a.hkv; ++gg) sum += __ldcg(a.part + (static_cast<size_t>(b) * a.hkv + gg) * a.part_stride + key);
           const float v = rows > 0 ? sum / static_cast<float>(a.norm_heads * Lq) : 0.f;
           float* dst = a.scores + static_cast<size_t>(b) * bd.n_stride + key;
-          *dst = a.accumulate ? *dst + v : v;
+          const float nv = a.accumulate ? *dst + v : v;
+          *dst = nv;
+          if (a.exch_world > 1) {
+            // this rank's partial of Eq. 18, straight into every rank's exchange buffer (peer memory: NVLink / IPC)
+            const size_t off = kExchHeaderElems + static_cast<size_t>(a.exch_rank) * a.exch_slot_elems + static_cast<size_t>(b) * bd.n_stride + key;
+            for (int p = 0; p < a.exch_world; ++p) a.exch_peers[p][off] = nv;
+          }
         }
         if (r == 0) a.counters[static_cast<size_t>(b) * n_tiles_b + key_tile + kt] = 0u;     // self-resetting
       }
@@ -462,7 +470,22 @@ cudaError_t launch(const qcf_ctx* ctx, const qcf_batch* b, const CUtensorMap& tm
   return launch_pdl(ctx->pdl, k2, dim3(groups, a.hkv, b->batch), dim3(kThreads), smem, stream, tm_q, tm_k, b->dev, a);
 }
 
+// One thread, launched behind pass 2 on the same stream: every score this rank stored into its peers' buffers has been
+// performed when this kernel starts; the fence + system-scope release stores make them visible before the epoch is.
+__global__ void exchange_flag_kernel(float* const* peers, int rank, int world, unsigned int epoch) {
+  __threadfence_system();
+  for (int p = 0; p < world; ++p) {
+    unsigned int* flag = reinterpret_cast<unsigned int*>(peers[p]) + rank;
+    asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(flag), "r"(epoch) : "memory");
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_exchange_flags(const qcf_ctx* ctx, cudaStream_t stream) {
+  exchange_flag_kernel<<<1, 1, 0, stream>>>(ctx->exch_peers, ctx->exch_rank, ctx->exch_world, ctx->exch_epoch);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* q_probe,
                          const __nv_bfloat16* k_f, float* scores, int accumulate, cudaStream_t stream) {
@@ -517,6 +540,7 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
   a.part = ctx->score_part; a.part_stride = ctx->max_ctx;
   a.counters = ctx->counters;
   a.scores = scores; a.accumulate = accumulate;
+  a.exch_peers = ctx->exch_peers; a.exch_rank = ctx->exch_rank; a.exch_world = ctx->exch_world; a.exch_slot_elems = ctx->exch_slot_elems;
   return L.d == 128 ? launch<128>(ctx, b, tm_q, tm_k, a, row_tiles, key_tiles, stream)
                     : launch<64>(ctx, b, tm_q, tm_k, a, row_tiles, key_tiles, stream);
 }

@@ -19,8 +19,19 @@ __device__ __forceinline__ uint32_t order_key(float f) {
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);             // ascending in the value
 }
 
+// Fused exchange of the KV-head-sharded step (include/qcf.h, qcf_set_score_exchange): the scores are the sum, in slot
+// order, of `world` slots of this rank's exchange buffer, each written by one rank's a2; flag[p] >= epoch says rank p's
+// slot is complete.
+struct Exch {
+  const float* buf;        // nullptr: plain scores
+  int world;
+  long long slot_elems;
+  unsigned int epoch;
+};
+
 __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float* __restrict__ scores, double ratio,
-                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached, int ceil_mode) {
+                                                        int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached, int ceil_mode,
+                                                        Exch ex) {
   extern __shared__ uint32_t s_keys[];                           // order keys of the first n_cached scores
   __shared__ unsigned int hist[2][256];        // double-buffered: pass p + 1's bins are zeroed while pass p's are scanned
   __shared__ unsigned int s_prefix, s_remaining;
@@ -35,6 +46,28 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   const float* s = scores + static_cast<size_t>(b) * bd.n_stride;
   int32_t* out = sel + static_cast<size_t>(b) * bd.n_stride;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (ex.buf) {
+    // acquire every rank's epoch (bounded: a peer that never arrives is a trap, not a hang)
+    if (tid < ex.world) {
+      const unsigned int* flag = reinterpret_cast<const unsigned int*>(ex.buf) + tid;
+      const long long t0 = clock64();
+      unsigned int v;
+      do {
+        asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+        if (static_cast<int>(v - ex.epoch) >= 0) break;
+        if (clock64() - t0 > 4000000000LL) __trap();
+      } while (true);
+    }
+    __syncthreads();
+  }
+  // score of position i: plain, or the slot sum in fixed order
+  auto score_at = [&](int i) -> float {
+    if (!ex.buf) return __ldcg(s + i);
+    const float* p = ex.buf + kExchHeaderElems + static_cast<size_t>(b) * bd.n_stride + i;
+    float acc = __ldcg(p);
+    for (int q = 1; q < ex.world; ++q) acc += __ldcg(p + static_cast<size_t>(q) * ex.slot_elems);
+    return acc;
+  };
   if (tid == 0) n_sel[b] = k;
   if (k <= 0) return;
   if (k >= N) {
@@ -44,8 +77,8 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
 
   // the five sweeps below read every score; one coalesced global read fills shared memory, the rest stay on chip
   const int n_sm_keys = min(N, n_cached);
-  for (int i = tid; i < n_sm_keys; i += kThreads) s_keys[i] = order_key(__ldcg(s + i));
-  auto key_of = [&](int i) -> uint32_t { return i < n_sm_keys ? s_keys[i] : order_key(__ldcg(s + i)); };
+  for (int i = tid; i < n_sm_keys; i += kThreads) s_keys[i] = order_key(score_at(i));
+  auto key_of = [&](int i) -> uint32_t { return i < n_sm_keys ? s_keys[i] : order_key(score_at(i)); };
   if (tid < 256) hist[0][tid] = 0u;
   if (tid == 0) { s_prefix = 0u; s_remaining = static_cast<unsigned int>(k); }
   __syncthreads();
@@ -144,7 +177,14 @@ cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* sco
   const size_t smem = static_cast<size_t>(n_cached) * sizeof(uint32_t);
   // per device / context, so set on every launch (as the other launchers do) rather than once per process
   cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
-  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode);
+  Exch ex{nullptr, 1, 0, 0u};
+  if (ctx->exch_world > 1 && !ceil_mode) {     // (the anchor ranking of Phase I is never sharded)
+    ex.buf = ctx->exch_peers_host[ctx->exch_rank];
+    ex.world = ctx->exch_world;
+    ex.slot_elems = ctx->exch_slot_elems;
+    ex.epoch = ctx->exch_epoch;
+  }
+  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode, ex);
 }
 
 }  // namespace qcf

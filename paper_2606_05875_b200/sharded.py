@@ -4,9 +4,13 @@ rank computes the partial of I(t) over ITS heads (qcf_set_head_shards makes qcf_
 Hq) and one all-reduce(sum) of scores[B][n_stride] fp32 — the only exchange of the step — gives every rank the same
 I(t); a3 then runs replicated, so all ranks select the same P without a broadcast.
 
-Plumbing only: the step's arithmetic is the C-ABI calls of include/qcf.h on the rank's head slices; the exchange is
-torch.distributed.all_reduce on the caller's process group (NCCL over NVLink on GPUs).  With world == 1 no collective
-is issued.  Default deployments shard REQUESTS instead (replicas, no collective — DESIGN.md section 8); this module is
+Plumbing only: the step's arithmetic is the C-ABI calls of include/qcf.h on the rank's head slices.  Two exchanges:
+  * "fused" (enable_fused_exchange): a2's combine CTAs store the rank's partial straight into every peer's exchange
+    buffer over peer memory (NVLink P2P or CUDA IPC mappings), a flag publishes the epoch, a3 acquires the flags and
+    sums the slots in fixed order — no collective call, no host round trip (include/qcf.h, qcf_set_score_exchange);
+  * "nccl" (default): torch.distributed.all_reduce on the caller's process group between the two launches — the
+    baseline the fused path replaces.
+torch.distributed is then only the rendezvous (exchanging the buffer handles).  With world == 1 nothing is exchanged.  Default deployments shard REQUESTS instead (replicas, no collective — DESIGN.md section 8); this module is
 for a single long request that must be spread over GPUs.
 """
 from __future__ import annotations
@@ -42,6 +46,28 @@ def all_reduce_scores(scores, world: int, group=None, stream=None):
         dist.all_reduce(scores, op=dist.ReduceOp.SUM, group=group)
 
 
+def share_exchange_buffers(mine, rank: int, world: int, group=None):
+    """Rendezvous of the fused exchange across PROCESSES (one rank per GPU): every rank exports its exchange buffer as a
+    CUDA IPC handle (torch.multiprocessing's reduce_tensor: cudaIpcGetMemHandle + offset inside the allocation),
+    torch.distributed carries the handles (all_gather_object — the only thing the process group is used for), and each
+    rank maps its peers' buffers (cudaIpcOpenMemHandle; over NVLink when the peers sit on other GPUs).  Returns the list
+    peer_bufs for HeadShardedStep.enable_fused_exchange; `mine` must stay alive while any peer uses it."""
+    import torch.distributed as dist
+    from torch.multiprocessing.reductions import reduce_tensor
+    if world == 1:
+        return [mine]
+    handles = [None] * world
+    dist.all_gather_object(handles, reduce_tensor(mine), group=group)
+    peers = []
+    for p in range(world):
+        if p == rank:
+            peers.append(mine)
+        else:
+            fn, args = handles[p]
+            peers.append(fn(*args))
+    return peers
+
+
 class HeadShardedStep:
     """The rank-local half of a KV-head-sharded qcf_layer_step.  Every tensor argument is this rank's head slice
     ([...][Hq/world][d] or [...][Hkv/world][d], contiguous); scores / sel / n_sel are full-size and end up identical on
@@ -55,6 +81,36 @@ class HeadShardedStep:
         self.ctx = binding.Context(n_q_heads // world, n_kv_heads // world, head_dim, rope_theta, max_batch, max_ctx,
                                    max_query, softmax_scale)
         self.ctx.qcf_set_head_shards(world)
+        self.fused = False
+
+    # ---- fused exchange (include/qcf.h, qcf_set_score_exchange)
+    @staticmethod
+    def alloc_exchange_buffer(world: int, slot_elems: int, device="cuda"):
+        """This rank's exchange buffer: [64 flags][world slots x slot_elems] fp32, zeroed.  Share it with the peers
+        (same process: pass the tensor; other processes: send it through torch.multiprocessing, which maps it with CUDA
+        IPC; other GPUs: enable peer access and pass the pointer)."""
+        import torch
+        n = binding.qcf_score_exchange_bytes(world, slot_elems) // 4
+        return torch.zeros(n, dtype=torch.float32, device=device)
+
+    def enable_fused_exchange(self, peer_bufs: Sequence, slot_elems: int):
+        """peer_bufs[p] = rank p's exchange buffer as visible from this process (peer_bufs[self.rank] is this rank's own)."""
+        if len(peer_bufs) != self.world:
+            raise ValueError("need one exchange buffer per rank")
+        self.fused = self.world > 1
+        self._exch = list(peer_bufs)
+        self.slot_elems = int(slot_elems)
+        if self.fused:
+            self.ctx.qcf_set_score_exchange(self.rank, self.world, self._exch, slot_elems)
+
+    def exchanged_scores(self, b: binding.Batch):
+        """The summed scores [B][n_stride] this rank's a3 ranks (slot order), for inspection."""
+        buf = self._exch[self.rank]
+        slots = buf[64: 64 + self.world * self.slot_elems].view(self.world, self.slot_elems)[:, : b.batch * b.n_stride]
+        acc = slots[0].clone()
+        for p in range(1, self.world):
+            acc += slots[p]
+        return acc.view(b.batch, b.n_stride)
 
     def batch(self, chunk_lens, chunk_rows, n_query, chunk_pos=None) -> binding.Batch:
         return self.ctx.batch(chunk_lens, chunk_rows, n_query, chunk_pos)
@@ -85,8 +141,8 @@ class HeadShardedStep:
         layers (Eq. 20) commutes with the sum over ranks, so one exchange per request suffices."""
         self.score_phase(b, k_pool=k_pool, v_pool=v_pool, k_fused=k_fused, v_fused=v_fused, q_probe=q_probe, scores=scores,
                          is_critical_layer=is_critical_layer, accumulate=accumulate, stream=stream)
-        if select_now:
-            self.all_reduce_scores(scores, stream)
+        if select_now and not self.fused:
+            self.all_reduce_scores(scores, stream)        # fused: a2 already stored into every peer's buffer
         self.fuse_phase(b, scores=scores, sel=sel, n_sel=n_sel, q_new=q_new, k_new=k_new, v_new=v_new, k_fused=k_fused,
                         v_fused=v_fused, out=out, lse=lse, ratio=ratio, rows_by_position=rows_by_position,
                         select_now=select_now, stream=stream)

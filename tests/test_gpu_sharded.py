@@ -47,20 +47,43 @@ def _ranks(wl, world):
     return steps, dws
 
 
+@pytest.mark.parametrize("exchange", ["accumulate", "fused"])
 @pytest.mark.parametrize("name,world", [("t_mid", 2), ("t_mid", 4), ("t_batch", 2), ("t_ragged", 2), ("c1", 2)])
-def test_head_sharded_step_matches_unsharded_oracle(name, world):
+def test_head_sharded_step_matches_unsharded_oracle(name, world, exchange):
+    """exchange = "accumulate": the sum over ranks formed by a2's own accumulate path (what an all-reduce computes);
+    "fused": the exchange of include/qcf.h qcf_set_score_exchange — every rank's a2 stores its partial into every rank's
+    exchange buffer and a3 sums the slots (here the "peers" are contexts of one process on one GPU, run one after the
+    other, so no kernel waits on a flag that is still to be written)."""
+    _, _, sharded = _mods()
     wl = inputs.make_workload(name)
     cfg = wl.cfg
     steps, dws = _ranks(wl, world)
-    scores = dws[0].scores                       # the array the all-reduce leaves on every rank
-    scores.fill_(7.0)
-    for rank, (st, dw) in enumerate(zip(steps, dws)):
-        st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
-                       q_probe=dw.q_probe, scores=scores, accumulate=rank > 0)
-    for st, dw in zip(steps, dws):
-        st.fuse_phase(dw.batch, scores=scores, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
-                      k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, lse=dw.lse, ratio=cfg.ratio)
-    torch.cuda.synchronize()
+    if exchange == "fused":
+        slot = dws[0].batch.batch * dws[0].batch.n_stride
+        bufs = [sharded.HeadShardedStep.alloc_exchange_buffer(world, slot) for _ in range(world)]
+        for st in steps:
+            st.enable_fused_exchange(bufs, slot)
+        for st, dw in zip(steps, dws):                              # every rank its OWN scores array: nothing is shared but the slots
+            dw.scores.fill_(7.0)
+            st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                           q_probe=dw.q_probe, scores=dw.scores)
+        for st, dw in zip(steps, dws):
+            st.fuse_phase(dw.batch, scores=None, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
+                          k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, lse=dw.lse, ratio=cfg.ratio)
+        torch.cuda.synchronize()
+        scores = steps[0].exchanged_scores(dws[0].batch)
+        for st, dw in zip(steps[1:], dws[1:]):                      # every rank holds the same slots: bit-identical sums
+            assert torch.equal(st.exchanged_scores(dw.batch), scores)
+    else:
+        scores = dws[0].scores                       # the array the all-reduce leaves on every rank
+        scores.fill_(7.0)
+        for rank, (st, dw) in enumerate(zip(steps, dws)):
+            st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                           q_probe=dw.q_probe, scores=scores, accumulate=rank > 0)
+        for st, dw in zip(steps, dws):
+            st.fuse_phase(dw.batch, scores=scores, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
+                          k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, lse=dw.lse, ratio=cfg.ratio)
+        torch.cuda.synchronize()
     g = cfg.n_q_heads // cfg.n_kv_heads
     sc = scores.cpu().numpy()
     for b, r in enumerate(wl.requests):
@@ -91,6 +114,18 @@ def test_head_sharded_step_matches_unsharded_oracle(name, world):
             kf, want = _f64(dw.k_fused[b, :t]), ref2["k_fused"][:, kv]
             ulp = np.ldexp(1.0, np.frexp(np.abs(want))[1] - 8)
             assert np.all(np.abs(kf - want) <= np.maximum(2e-2, ulp))
+    if exchange == "fused":
+        # a second step on the same buffers (a1 restores the stitched PIC keys): the epoch moves on — flags left from the
+        # first step do not satisfy it — and the same selection comes out
+        for st, dw in zip(steps, dws):
+            st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                           q_probe=dw.q_probe, scores=dw.scores)
+        sel_again = torch.zeros_like(dws[0].sel)
+        steps[0].ctx.qcf_select_topk(dws[0].batch, None, cfg.ratio, sel_again, dws[0].n_sel)
+        torch.cuda.synchronize()
+        for b in range(dws[0].B):
+            kb = int(dws[0].n_sel[b])
+            assert torch.equal(sel_again[b, :kb], dws[0].sel[b, :kb])
 
 
 def test_head_sharded_full_size_c2_matches_the_unsharded_step():
@@ -176,3 +211,93 @@ def test_layer_step_through_a_nccl_group_of_one():
     finally:
         if created:
             dist.destroy_process_group()
+
+
+# ----------------------------------------------------------------------------------------------- two processes, one GPU, CUDA IPC
+
+def _ipc_rank(rank, world, name, q_bufs, q_res, barrier):
+    """One rank of the fused-exchange step in its own PROCESS (own CUDA context).  Phases are ordered on the host so that
+    no kernel ever waits on a flag another process has not written yet (B200_PROFILING.md: ranks that spin on one another
+    must not share a GPU)."""
+    import numpy as np
+    import torch
+    from paper_2606_05875_b200 import device, inputs, sharded
+    torch.cuda.set_device(0)
+    wl = inputs.make_workload(name)
+    cfg = wl.cfg
+    st = sharded.HeadShardedStep(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, max(cfg.batch, 1),
+                                 max(cfg.n_ctx, 1024), max(cfg.n_query, 1), rank=rank, world=world)
+    dw = device.DeviceWorkload(inputs.shard_heads(wl, rank, world), st.ctx)
+    slot = dw.batch.batch * dw.batch.n_stride
+    mine = sharded.HeadShardedStep.alloc_exchange_buffer(world, slot)
+    for p in range(world):                        # my buffer to every peer: torch.multiprocessing maps it with cudaIpc*
+        if p != rank:
+            q_bufs[p].put((rank, mine))
+    peers = {rank: mine}
+    while len(peers) < world:
+        r, t = q_bufs[rank].get(timeout=120)
+        peers[r] = t
+    st.enable_fused_exchange([peers[p] for p in range(world)], slot)
+    barrier.wait(timeout=120)
+    for turn in range(world):                     # a2 of one rank at a time (peer stores + flag release), host-ordered
+        if turn == rank:
+            st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                           q_probe=dw.q_probe, scores=dw.scores)
+            torch.cuda.synchronize()
+        barrier.wait(timeout=120)
+    st.fuse_phase(dw.batch, scores=None, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
+                  k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, ratio=cfg.ratio)      # a3 acquires flags already set
+    torch.cuda.synchronize()
+    q_res.put((rank, dw.n_sel.cpu().numpy(), dw.sel.cpu().numpy(), st.exchanged_scores(dw.batch).cpu().numpy(),
+               dw.out.cpu().view(torch.int16).numpy()))
+    barrier.wait(timeout=120)                     # keep the exported buffers alive until every peer is done
+
+
+def test_fused_exchange_two_processes_one_gpu_cuda_ipc():
+    """the score exchange over PEER memory.  Two processes (two CUDA contexts) on the one GPU
+    of this box map each other's exchange buffers through CUDA IPC handles; each rank's a2 stores its partial scores
+    into both buffers and releases its flag; each rank's a3 acquires both flags and ranks the slot sum.  Checked against
+    the oracle of the UNSHARDED layer: scores 1e-2 relative, the north-star selection rule, both ranks the same P."""
+    import torch.multiprocessing as mp
+    name, world = "t_mid", 2
+    ctx = mp.get_context("spawn")
+    q_bufs = [ctx.Queue() for _ in range(world)]
+    q_res = ctx.Queue()
+    barrier = ctx.Barrier(world)
+    procs = [ctx.Process(target=_ipc_rank, args=(r, world, name, q_bufs, q_res, barrier)) for r in range(world)]
+    for p in procs:
+        p.start()
+    try:
+        res = {}
+        for _ in range(world):
+            r, n_sel, sel, sc, out = q_res.get(timeout=300)
+            res[r] = (n_sel, sel, sc, out)
+    finally:
+        for p in procs:
+            p.join(timeout=60)
+            if p.is_alive():
+                p.kill()
+    assert all(p.exitcode == 0 for p in procs)
+    wl = inputs.make_workload(name)
+    cfg = wl.cfg
+    r0 = wl.requests[0]
+    k_pic = [O.widen_bf16(wl.pool_k[i]) for i in r0.chunk_ids]
+    v_pic = [O.widen_bf16(wl.pool_v[i]) for i in r0.chunk_ids]
+    ref = O.layer_step(k_pic, v_pic, cfg.rope_theta, O.widen_bf16(r0.q_probe), cfg.ratio, O.widen_bf16(r0.q_new),
+                       O.widen_bf16(r0.k_new), O.widen_bf16(r0.v_new))
+    k = int(res[0][0][0])
+    assert k == len(ref["sel"]) == int(res[1][0][0])
+    assert np.array_equal(res[0][2], res[1][2]), "both ranks hold bit-identical slot sums"
+    np.testing.assert_allclose(res[0][2][0, : r0.n_ctx].astype(np.float64), ref["scores"], rtol=1e-2, atol=0)
+    sel0 = res[0][1][0, :k].astype(np.int64)
+    assert np.array_equal(sel0, res[1][1][0, :k])
+    _check_selection(sel0, ref["scores"], k)
+    # a5 of each rank's heads against the oracle on that selection
+    ref2 = O.layer_step(k_pic, v_pic, cfg.rope_theta, None, 0.0, O.widen_bf16(r0.q_new), O.widen_bf16(r0.k_new),
+                        O.widen_bf16(r0.v_new), sel=sel0)
+    g = cfg.n_q_heads // cfg.n_kv_heads
+    per = cfg.n_kv_heads // world
+    n_r = k + r0.n_query
+    for rank in range(world):
+        got = O.widen_bf16(res[rank][3].view(np.uint16))[0, :n_r]
+        assert np.max(np.abs(got - ref2["out"][:, rank * per * g:(rank + 1) * per * g])) <= 2e-2
