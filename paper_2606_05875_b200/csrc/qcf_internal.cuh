@@ -145,6 +145,9 @@ cudaError_t launch_decode_attn(const qcf_ctx*, const __nv_bfloat16* q, const __n
                                int n_keys, __nv_bfloat16* out, float* lse, cudaStream_t);
 cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
                         __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
+// one row: c[N] = epilogue(x[K] . w[N][K]^T); gain != nullptr: x is RMS-normalised with that gain first (rounded to bf16)
+cudaError_t launch_gemv(const qcf_ctx*, const __nv_bfloat16* x, const __nv_bfloat16* w, const __nv_bfloat16* gain, float eps,
+                        const __nv_bfloat16* residual, __nv_bfloat16* c, int N, int K, int epilogue, cudaStream_t);
 cudaError_t launch_lm_head(const qcf_ctx*, const __nv_bfloat16* w_lm, const __nv_bfloat16* h, int vocab, int hidden, float* logits,
                            int32_t* token, cudaStream_t);
 cudaError_t launch_stamp(unsigned long long* t0, cudaStream_t);

@@ -278,16 +278,15 @@ qcf_status qcf_stack_decode(qcf_stack* s, const int32_t* token_in, int32_t pos0,
       const qcf_layer_weights& w = s->layers[l];
       __nv_bfloat16* kc = static_cast<__nv_bfloat16*>(k_cache[l]);
       __nv_bfloat16* vc = static_cast<__nv_bfloat16*>(v_cache[l]);
-      STK_CUDA(ctx, launch_rmsnorm(s->x, bf(w.g_attn), s->dims.rms_eps, 1, hid, s->h, st));
-      STK_CUDA(ctx, launch_gemm(ctx, s->h, bf(w.w_qkv), nullptr, s->qkv, 1, qkv_n, hid, QCF_EPI_STORE, st));
+      // one row: weight-streaming GEMVs with the RMSNorm folded into their prologue (6 launches per layer, PDL-chained)
+      STK_CUDA(ctx, launch_gemv(ctx, s->x, bf(w.w_qkv), bf(w.g_attn), s->dims.rms_eps, nullptr, s->qkv, qkv_n, hid, QCF_EPI_STORE, st));
       // QK-norm + RoPE at position pos; the token's K/V land in cache row pos
       STK_CUDA(ctx, launch_qknorm_rope(ctx, s->qkv, bf(w.g_q), bf(w.g_k), s->rope_table, nullptr, nullptr, 0, pos,
                                        s->dims.rms_eps, 1, s->q_new, kc + pos * kv_row, vc + pos * kv_row, st));
       STK_CUDA(ctx, launch_decode_attn(ctx, s->q_new, kc, vc, pos + 1, s->attn, nullptr, st));
-      STK_CUDA(ctx, launch_gemm(ctx, s->attn, bf(w.w_o), s->x, s->x, 1, hid, L.hq * L.d, QCF_EPI_ADD_RESIDUAL, st));
-      STK_CUDA(ctx, launch_rmsnorm(s->x, bf(w.g_ffn), s->dims.rms_eps, 1, hid, s->h, st));
-      STK_CUDA(ctx, launch_gemm(ctx, s->h, bf(w.w_gate_up), nullptr, s->act, 1, 2 * ffn, hid, QCF_EPI_SWIGLU, st));
-      STK_CUDA(ctx, launch_gemm(ctx, s->act, bf(w.w_down), s->x, s->x, 1, hid, ffn, QCF_EPI_ADD_RESIDUAL, st));
+      STK_CUDA(ctx, launch_gemv(ctx, s->attn, bf(w.w_o), nullptr, 0.f, s->x, s->x, hid, L.hq * L.d, QCF_EPI_ADD_RESIDUAL, st));
+      STK_CUDA(ctx, launch_gemv(ctx, s->x, bf(w.w_gate_up), bf(w.g_ffn), s->dims.rms_eps, nullptr, s->act, 2 * ffn, hid, QCF_EPI_SWIGLU, st));
+      STK_CUDA(ctx, launch_gemv(ctx, s->act, bf(w.w_down), nullptr, 0.f, s->x, s->x, hid, ffn, QCF_EPI_ADD_RESIDUAL, st));
     }
     STK_CUDA(ctx, launch_rmsnorm(s->x, bf(g_final), s->dims.rms_eps, 1, hid, s->h, st));
     STK_CUDA(ctx, launch_lm_head(ctx, bf(w_lm), s->h, vocab, hid, logits + static_cast<size_t>(i) * vocab, tokens_out + i, st));

@@ -36,7 +36,7 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (relative to the reference max) exceeds 2^8
 #ifndef QCF_ATTN_MUFU_PAIRS
-#define QCF_ATTN_MUFU_PAIRS 4
+#define QCF_ATTN_MUFU_PAIRS 3
 #endif
 // Measured dead ends on this kernel (all parity-green, all slower on c2; kept out of the code):
 //   * two threads per row (8 softmax warps, 32 key columns each, barrier.red agreement per tile): 82 -> 92 us, and a lone
@@ -67,8 +67,10 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 // loads, the exponentials and the S loads removed still takes 75.3 of its 75.8 us at c2: the step is bound by the tensor
 // pipe shared between the two CTAs plus ~0.1 us of sweep ALU work and ring barriers per CTA step, and the launch by the
 // heaviest tile's 81-step chain (3.3 us prologue + 81 x 0.80 us).
-// Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Measured on c2: 4 -> 84 us,
-// 3 -> 91 us, 2 -> 104 us: the sweep is issue-bound, not MUFU-bound, so every exponential goes to the MUFU.
+// Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Round 1 (before the elected-lane
+// issue fix, when the sweep was issue-bound) measured 4 -> 84 us, 3 -> 91 us on c2.  Re-measured in round 2 on the current
+// kernel: c2 76.7 vs 76.8 us (neutral), c4 x 16 2.84 -> 2.80 ms, c5 2.57 -> 2.49 ms with 3 — MUFU and tensor pipe are both
+// ~60 % busy (profiles/r02_c4.md), a quarter of the exponentials on the FMA pipe unloads the tighter of the two.
 constexpr int kMufuPairs = QCF_ATTN_MUFU_PAIRS;
 
 // Two CTAs are resident per SM (96 KB of shared memory, 256 TMEM columns and <= 168 registers each).  Inside a CTA

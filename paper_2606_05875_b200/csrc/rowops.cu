@@ -159,6 +159,94 @@ __global__ void __launch_bounds__(256) anchor_score_kernel(BatchDev bd, int row_
   }
 }
 
+// Decoding pushes ONE row through the block: y[N] = x[K] . W[N][K]^T is a pure weight stream
+// (386 MB per layer at config 3, ~1 flop per byte), so it is a warp-per-output-row-pair GEMV, not a tensor-core tile:
+// x (optionally RMS-normalised with its gain on the way in, rounded to bf16 exactly as the batched path stores h) sits in
+// shared memory, every lane streams 128-bit weight vectors with 8 loads in flight, a shuffle tree finishes the two dot
+// products, lane 0 applies the epilogue of qcf_linear (store / + residual / SwiGLU on interleaved gate-up rows).
+template <int EPI, bool NORM>
+__global__ void __launch_bounds__(256) gemv_kernel(const uint4* __restrict__ w, const uint4* x, const uint4* __restrict__ gain,
+                                                   float eps, const __nv_bfloat16* residual, __nv_bfloat16* c, int N, int k8) {
+  extern __shared__ uint4 s_x[];
+  __shared__ float s_part[8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  pdl_trigger();
+  pdl_wait();                                   // x / residual are written by the predecessor kernel
+  float ss = 0.f;
+  for (int i = threadIdx.x; i < k8; i += blockDim.x) {
+    const uint4 v = ld_nc_v4(x + i);            // coherent (not .nc): see the PDL note in qcf_internal.cuh
+    s_x[i] = v;
+    if (NORM) {
+      const uint32_t u[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { const float a = bf16lo(u[k]), b = bf16hi(u[k]); ss = fmaf(a, a, ss); ss = fmaf(b, b, ss); }
+    }
+  }
+  if (NORM) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    if (lane == 0) s_part[warp] = ss;
+    __syncthreads();
+    float tot = 0.f;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) tot += s_part[q];
+    const float inv = rsqrtf(tot / static_cast<float>(k8 * 8) + eps);
+    for (int i = threadIdx.x; i < k8; i += blockDim.x) {
+      const uint4 v = s_x[i], gg = __ldg(gain + i);
+      const uint32_t u[4] = {v.x, v.y, v.z, v.w}, gw[4] = {gg.x, gg.y, gg.z, gg.w};
+      uint32_t o[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) o[k] = pack_bf16(bf16lo(u[k]) * inv * bf16lo(gw[k]), bf16hi(u[k]) * inv * bf16hi(gw[k]));
+      s_x[i] = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+  }
+  __syncthreads();
+  for (int rp = blockIdx.x * 8 + warp; rp < N / 2; rp += gridDim.x * 8) {
+    const uint4* w0 = w + static_cast<size_t>(2 * rp) * k8;
+    const uint4* w1 = w0 + k8;
+    float acc0 = 0.f, acc1 = 0.f;
+    for (int i0 = lane; i0 < k8; i0 += 128) {
+      uint4 a0[4], a1[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + 32 * u;
+        if (i < k8) { a0[u] = ld_nc_v4(w0 + i); a1[u] = ld_nc_v4(w1 + i); }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + 32 * u;
+        if (i < k8) {
+          const uint4 b = s_x[i];
+          const uint32_t p0[4] = {a0[u].x, a0[u].y, a0[u].z, a0[u].w}, p1[4] = {a1[u].x, a1[u].y, a1[u].z, a1[u].w};
+          const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const float x0 = bf16lo(bw[k]), x1 = bf16hi(bw[k]);
+            acc0 = fmaf(bf16lo(p0[k]), x0, acc0); acc0 = fmaf(bf16hi(p0[k]), x1, acc0);
+            acc1 = fmaf(bf16lo(p1[k]), x0, acc1); acc1 = fmaf(bf16hi(p1[k]), x1, acc1);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      acc0 += __shfl_xor_sync(0xffffffffu, acc0, o);
+      acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
+    }
+    if (lane == 0) {
+      if (EPI == QCF_EPI_SWIGLU) {
+        c[rp] = __float2bfloat16_rn(acc0 / (1.f + __expf(-acc0)) * acc1);
+      } else if (EPI == QCF_EPI_ADD_RESIDUAL) {
+        c[2 * rp] = __float2bfloat16_rn(__bfloat162float(residual[2 * rp]) + acc0);
+        c[2 * rp + 1] = __float2bfloat16_rn(__bfloat162float(residual[2 * rp + 1]) + acc1);
+      } else {
+        c[2 * rp] = __float2bfloat16_rn(acc0);
+        c[2 * rp + 1] = __float2bfloat16_rn(acc1);
+      }
+    }
+  }
+}
+
 // First generated token (the end of TTFT): logits[v] = h . W_lm[v] for one normalised hidden row — a 268 MB
 // weight stream at config 3, one warp per vocabulary row, 128-bit loads, h held in shared memory — then an argmax with ties
 // to the lower token id.
@@ -248,6 +336,32 @@ cudaError_t launch_lm_head(const qcf_ctx* ctx, const __nv_bfloat16* w_lm, const 
   if (e != cudaSuccess) return e;
   argmax_kernel<<<1, 1024, 0, stream>>>(logits, vocab, token);
   return cudaGetLastError();
+}
+
+cudaError_t launch_gemv(const qcf_ctx* ctx, const __nv_bfloat16* x, const __nv_bfloat16* w, const __nv_bfloat16* gain, float eps,
+                        const __nv_bfloat16* residual, __nv_bfloat16* c, int N, int K, int epilogue, cudaStream_t stream) {
+  if (N <= 0) return cudaSuccess;
+  int blocks = (N / 2 + 7) / 8;
+  if (blocks > ctx->n_sm * 8) blocks = ctx->n_sm * 8;
+  const size_t smem = static_cast<size_t>(K) * 2;
+  const uint4* w4 = reinterpret_cast<const uint4*>(w);
+  const uint4* x4 = reinterpret_cast<const uint4*>(x);
+  const uint4* g4 = reinterpret_cast<const uint4*>(gain);
+#define QCF_GEMV(EPI, NORM)                                                                                              \
+  do {                                                                                                                   \
+    auto kern = gemv_kernel<EPI, NORM>;                                                                                  \
+    if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)); \
+    return launch_pdl(ctx->pdl, kern, dim3(blocks), dim3(256), smem, stream, w4, x4, g4, eps, residual, c, N, K / 8);     \
+  } while (0)
+  if (gain) {
+    if (epilogue == QCF_EPI_SWIGLU) QCF_GEMV(QCF_EPI_SWIGLU, true);
+    if (epilogue == QCF_EPI_ADD_RESIDUAL) QCF_GEMV(QCF_EPI_ADD_RESIDUAL, true);
+    QCF_GEMV(QCF_EPI_STORE, true);
+  }
+  if (epilogue == QCF_EPI_SWIGLU) QCF_GEMV(QCF_EPI_SWIGLU, false);
+  if (epilogue == QCF_EPI_ADD_RESIDUAL) QCF_GEMV(QCF_EPI_ADD_RESIDUAL, false);
+  QCF_GEMV(QCF_EPI_STORE, false);
+#undef QCF_GEMV
 }
 
 cudaError_t launch_stamp(unsigned long long* t0, cudaStream_t stream) {

@@ -29,6 +29,9 @@ struct Exch {
   unsigned int epoch;
 };
 
+// EXCH is a template parameter so that the plain kernel's sweeps keep their simple loop bodies (with the slot path as a
+// run-time branch inside them the plain top-k went 36 -> 54 us at N = 32768).
+template <bool EXCH>
 __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float* __restrict__ scores, double ratio,
                                                         int32_t* __restrict__ sel, int32_t* __restrict__ n_sel, int n_cached, int ceil_mode,
                                                         Exch ex) {
@@ -46,7 +49,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   const float* s = scores + static_cast<size_t>(b) * bd.n_stride;
   int32_t* out = sel + static_cast<size_t>(b) * bd.n_stride;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (ex.buf) {
+  if (EXCH) {
     // acquire every rank's epoch (bounded: a peer that never arrives is a trap, not a hang)
     if (tid < ex.world) {
       const unsigned int* flag = reinterpret_cast<const unsigned int*>(ex.buf) + tid;
@@ -62,7 +65,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   }
   // score of position i: plain, or the slot sum in fixed order
   auto score_at = [&](int i) -> float {
-    if (!ex.buf) return __ldcg(s + i);
+    if (!EXCH) return __ldcg(s + i);
     const float* p = ex.buf + kExchHeaderElems + static_cast<size_t>(b) * bd.n_stride + i;
     float acc = __ldcg(p);
     for (int q = 1; q < ex.world; ++q) acc += __ldcg(p + static_cast<size_t>(q) * ex.slot_elems);
@@ -176,15 +179,17 @@ cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* sco
   const int n_cached = b->n_stride < 49152 ? b->n_stride : 49152;
   const size_t smem = static_cast<size_t>(n_cached) * sizeof(uint32_t);
   // per device / context, so set on every launch (as the other launchers do) rather than once per process
-  cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
+  cudaFuncSetAttribute(topk_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
+  cudaFuncSetAttribute(topk_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
   Exch ex{nullptr, 1, 0, 0u};
   if (ctx->exch_world > 1 && !ceil_mode) {     // (the anchor ranking of Phase I is never sharded)
     ex.buf = ctx->exch_peers_host[ctx->exch_rank];
     ex.world = ctx->exch_world;
     ex.slot_elems = ctx->exch_slot_elems;
     ex.epoch = ctx->exch_epoch;
+    return launch_pdl(ctx->pdl, topk_kernel<true>, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode, ex);
   }
-  return launch_pdl(ctx->pdl, topk_kernel, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode, ex);
+  return launch_pdl(ctx->pdl, topk_kernel<false>, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode, ex);
 }
 
 }  // namespace qcf

@@ -113,12 +113,14 @@ def test_linear_store_and_residual(M, N, K, mt):
     assert np.all(np.abs(_f64(x) - want) <= 0.5 * _ulp(want) + 2e-5 * np.sqrt(K))
 
 
+@pytest.mark.parametrize("M", [300, 1])
 @pytest.mark.parametrize("mt", [0, 1, 2])
-def test_linear_swiglu(mt):
+def test_linear_swiglu(mt, M):
+    """M = 1 with the default heuristic takes the decode GEMV (a weight stream), any forced tile height the MMA kernel."""
     binding = _binding()
     ctx = binding.Context(8, 2, 64, 1e6, 1, 1024, 8)
     ctx.qcf_debug_set(binding.QCF_DEBUG_GEMM_MT, mt)
-    M, F, K = 300, 1160, 384
+    F, K = 1160, 384
     rng = np.random.default_rng(9)
     a = inputs.f32_to_bf16_bits(rng.standard_normal((M, K), dtype=np.float32))
     wg = inputs.f32_to_bf16_bits(rng.standard_normal((F, K), dtype=np.float32) * np.float32(0.1))
