@@ -5,6 +5,11 @@
 // 16-byte vectors — and keeps that slot's 8 (cos, sin) values of the chunk's rotation in registers while it walks
 // the rows of its work item, so the only memory traffic in the loop is 128-bit coalesced K/V loads and stores.
 #include "qcf_internal.cuh"
+#include "sm100_ptx.cuh"
+
+#ifndef QCF_REPO_TMA
+#define QCF_REPO_TMA 1
+#endif
 
 namespace qcf {
 
@@ -128,6 +133,84 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   }
 }
 
+// ---- TMA-staged variant: the rows of a work item are contiguous in the pool (source) and in the fused cache
+// (destination), so each tensor moves as ONE bulk async copy global -> shared (cp.async.bulk, completion on an mbarrier)
+// and ONE bulk copy shared -> global; V never touches a register, K is rotated in place in shared memory in between.
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) reposition_tma_kernel(BatchDev bd, int hkv, const __nv_bfloat16* k_pool,
+                                                             const __nv_bfloat16* v_pool, __nv_bfloat16* k_f,
+                                                             __nv_bfloat16* v_f) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ __align__(8) unsigned long long s_bar;
+  constexpr int kSlotsPerHead = D / 16;
+  const int slots = hkv * kSlotsPerHead;
+  const int row_elems = hkv * D;
+  const uint32_t row_bytes = static_cast<uint32_t>(row_elems) * 2u;
+  const int4 w0 = __ldg(bd.repo_items + 2 * blockIdx.x), w1 = __ldg(bd.repo_items + 2 * blockIdx.x + 1);
+  const size_t src_row = (static_cast<size_t>(static_cast<uint32_t>(w0.y)) << 32) | static_cast<uint32_t>(w0.x);
+  const size_t dst_row = (static_cast<size_t>(static_cast<uint32_t>(w0.w)) << 32) | static_cast<uint32_t>(w0.z);
+  const int rows = w1.x;
+  const int c = w1.y;
+  const bool identity = w1.z != 0;
+  const uint32_t bytes = static_cast<uint32_t>(rows) * row_bytes;
+  const uint32_t sK = smem_u32(smem), sV = sK + (k_pool ? kRepoRows * row_bytes : 0u);
+  const uint32_t bar = smem_u32(&s_bar);
+  if (threadIdx.x == 0) {
+    ptx::mbar_init(bar, 1);
+    ptx::fence_barrier_init();
+  }
+  pdl_trigger();
+  __syncthreads();
+  pdl_wait();                          // before the first pool read / cache write
+  if (threadIdx.x == 0) {
+    ptx::mbar_arrive_expect_tx(bar, bytes * ((k_pool ? 1u : 0u) + (v_pool ? 1u : 0u)));
+    if (k_pool) bulk_g2s(sK, k_pool + src_row * row_elems, bytes, bar);
+    if (v_pool) bulk_g2s(sV, v_pool + src_row * row_elems, bytes, bar);
+  }
+  // the chunk's rotation for this thread's pair slot, fetched while the tiles are in flight
+  const int slot = threadIdx.x % slots;
+  const int rsub = threadIdx.x / slots;
+  const int rows_per_pass = blockDim.x / slots;
+  const int head = slot / kSlotsPerHead, jc = slot % kSlotsPerHead;
+  const int e0 = head * D + jc * 8;
+  float cs[8], sn[8];
+  if (k_pool && !identity) {
+    const float4* rt = reinterpret_cast<const float4*>(bd.rot + static_cast<size_t>(c) * (D / 2) + jc * 8);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float4 t = __ldg(rt + i);
+      cs[2 * i] = t.x; sn[2 * i] = t.y; cs[2 * i + 1] = t.z; sn[2 * i + 1] = t.w;
+    }
+  }
+  ptx::mbar_wait(bar, 0);
+  if (k_pool && !identity) {
+    for (int r = rsub; r < rows; r += rows_per_pass) {
+      uint4* pa = reinterpret_cast<uint4*>(smem + static_cast<size_t>(r) * row_bytes + e0 * 2);
+      uint4* pb = reinterpret_cast<uint4*>(smem + static_cast<size_t>(r) * row_bytes + (e0 + D / 2) * 2);
+      uint4 oa, ob;
+      rotate8(*pa, *pb, cs, sn, oa, ob);
+      *pa = oa;
+      *pb = ob;
+    }
+    ptx::fence_proxy_async_smem();      // the rotated rows (generic-proxy writes) are read by the bulk store (async proxy)
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (k_pool) bulk_s2g(k_f + dst_row * row_elems, sK, bytes);
+    if (v_pool) bulk_s2g(v_f + dst_row * row_elems, sV, bytes);
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // shared memory may be released once it has been read
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_reposition(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* k_pool,
@@ -139,6 +222,22 @@ cudaError_t launch_reposition(const qcf_ctx* ctx, const qcf_batch* b, const __nv
   if (rpp < 1) rpp = 1;
   if (rpp > kRepoRows) rpp = kRepoRows;
   const int threads = slots * rpp;     // slots <= 512 is enforced at qcf_create
+#if QCF_REPO_TMA
+  {
+    const size_t row_bytes = static_cast<size_t>(ctx->lay.hkv) * ctx->lay.d * 2;
+    const size_t smem = kRepoRows * row_bytes * ((k_pool ? 1 : 0) + (v_pool ? 1 : 0));
+    if (threads <= 256 && smem <= 200 * 1024) {
+      if (ctx->lay.d == 128) {
+        auto kern = reposition_tma_kernel<128>;
+        if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+        return launch_pdl(ctx->pdl, kern, dim3(b->repo_blocks), dim3(threads), smem, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
+      }
+      auto kern = reposition_tma_kernel<64>;
+      if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+      return launch_pdl(ctx->pdl, kern, dim3(b->repo_blocks), dim3(threads), smem, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
+    }
+  }
+#endif
   if (ctx->lay.d == 128)
     return launch_pdl(ctx->pdl, reposition_kernel<128>, dim3(b->repo_blocks), dim3(threads), 0, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
   return launch_pdl(ctx->pdl, reposition_kernel<64>, dim3(b->repo_blocks), dim3(threads), 0, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);

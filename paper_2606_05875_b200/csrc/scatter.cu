@@ -2,10 +2,58 @@
 // the same positions, and append the user query's own K/V rows at N..N+Lq-1 (U is the online suffix).
 // Pure row gather/scatter: 2 * Hkv * d * 2 bytes read and written per refreshed row, 128-bit vectors.
 #include "qcf_internal.cuh"
+#include "sm100_ptx.cuh"
 
 namespace qcf {
 
 namespace {
+
+// TMA-staged variant (the default whenever a row fits its 16 KB slot budget): a refreshed row is one contiguous
+// Hkv*d*2-byte run at its source and at its destination, so it moves as ONE bulk async copy global -> shared
+// (cp.async.bulk, completion on an mbarrier) and ONE bulk copy shared -> global, never through registers.  A CTA is a single
+// warp whose lanes 0..15 each own a (row slot, K or V) pair with its own mbarrier: 8 rows x 2 tensors in flight per CTA,
+// ~7 CTAs per SM.  Measured against the register-staged kernel below on c4 x 16: see DESIGN.md section 7.
+constexpr int kScatterSlots = 16;
+
+__global__ void __launch_bounds__(32) scatter_tma_kernel(BatchDev bd, uint32_t row_bytes, const int32_t* sel,
+                                                         const int32_t* n_sel, const unsigned char* k_new,
+                                                         const unsigned char* v_new, int rows_by_position,
+                                                         unsigned char* k_f, unsigned char* v_f) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ __align__(8) unsigned long long s_bar[kScatterSlots];
+  const int lane = threadIdx.x;
+  const int b = blockIdx.y;
+  const int N = bd.n_ctx[b], Lq = bd.n_query[b];
+  if (lane < kScatterSlots) ptx::mbar_init(smem_u32(&s_bar[lane]), 1);
+  ptx::fence_barrier_init();
+  pdl_trigger();
+  __syncwarp();
+  pdl_wait();
+  const int ns = __ldcg(n_sel + b);         // coherent loads: written by a predecessor this kernel may overlap (PDL)
+  const int n_rows = ns + Lq;
+  const int slot = lane >> 1, which = lane & 1;
+  const size_t base = static_cast<size_t>(b) * bd.t_stride;
+  const uint32_t bar = smem_u32(&s_bar[lane & (kScatterSlots - 1)]);
+  const uint32_t buf = smem_u32(smem) + static_cast<uint32_t>(lane & (kScatterSlots - 1)) * row_bytes;
+  uint32_t phase = 0;
+  for (int r0 = blockIdx.x * 8; r0 < n_rows; r0 += gridDim.x * 8) {
+    const int r = r0 + slot;
+    if (lane < kScatterSlots && r < n_rows) {
+      const int p = r < ns ? __ldcg(sel + static_cast<size_t>(b) * bd.n_stride + r) : N + (r - ns);
+      const size_t src = (base + (rows_by_position ? p : r)) * row_bytes;
+      const size_t dst = (base + p) * row_bytes;
+      ptx::mbar_arrive_expect_tx(bar, row_bytes);
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(buf), "l"((which ? v_new : k_new) + src), "r"(row_bytes), "r"(bar) : "memory");
+      ptx::mbar_wait(bar, phase);
+      phase ^= 1u;
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                   ::"l"((which ? v_f : k_f) + dst), "r"(buf), "r"(row_bytes) : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the slot is reused by the next row
+    }
+  }
+}
 
 // grid (row blocks, B); each warp moves whole rows (K then V) — a row is Hkv*d*2 bytes (2 KB at 8 x 128).
 __global__ void __launch_bounds__(256) scatter_kernel(BatchDev bd, int row_vec, const int32_t* __restrict__ sel,
@@ -46,6 +94,22 @@ cudaError_t launch_scatter(const qcf_ctx* ctx, const qcf_batch* b, const int32_t
   if (b->batch == 0 || b->t_stride == 0) return cudaSuccess;
   const int row_vec = ctx->lay.hkv * ctx->lay.d / 8;
   const int max_rows = b->t_stride;                      // |R_b| <= N_b + Lq_b
+  const uint32_t row_bytes = static_cast<uint32_t>(row_vec) * 16u;
+  // Size-based choice, by measurement: the bulk-copy kernel moves a row as load -> wait -> store -> wait, a ~2.5 us chain
+  // that wins once the launch is bandwidth-bound (c4 x 16, 170 MB: 68 -> 57 us = 0.91 of the HBM copy peak; rho = 0.5:
+  // 0.96) and loses while it is latency-bound (c2, 6.5 MB: 8.5 -> 10.1 us); c5 (20 MB) is a tie.  The row count is a
+  // host-side estimate (the selection size lives on the device).
+  const double est_bytes = (ctx->ratio_hint * b->n_stride + b->q_stride) * static_cast<double>(b->batch) * row_bytes * 2.0;
+  if (row_bytes <= 4096 && est_bytes >= 12.0 * 1024 * 1024) {     // 16 slots x row <= 64 KB per one-warp CTA
+    int blocks = (max_rows + 7) / 8;
+    const int cap = ctx->n_sm * 16;
+    if (blocks > cap) blocks = cap;
+    const size_t smem = static_cast<size_t>(kScatterSlots) * row_bytes;
+    if (smem > 48 * 1024) cudaFuncSetAttribute(scatter_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    return launch_pdl(ctx->pdl, scatter_tma_kernel, dim3(blocks, b->batch), dim3(32), smem, stream, b->dev, row_bytes, sel, n_sel,
+                      reinterpret_cast<const unsigned char*>(k_new), reinterpret_cast<const unsigned char*>(v_new),
+                      rows_by_position, reinterpret_cast<unsigned char*>(k_f), reinterpret_cast<unsigned char*>(v_f));
+  }
   int blocks = (max_rows + 7) / 8;
   const int cap = ctx->n_sm * 8;
   if (blocks > cap) blocks = cap;

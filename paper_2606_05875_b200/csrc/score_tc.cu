@@ -516,16 +516,22 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
     if (n_splits > 8) n_splits = 8;            // x 2 column halves = 16 partials per row: pass 2 combines them in one batch of loads
     if (n_splits < 1) n_splits = 1;
   }
-  // pass 2: key tiles per CTA.  A CTA per key tile is 4 tile steps under a full prologue at c4 (8192 CTAs): walk several.
-  // Small problems: one resident wave; large ones: at most three waves' worth of CTAs.
+  // pass 2: key tiles per CTA.  A CTA costs ~kt tile walks plus a fixed part worth about one walk (barrier setup, TMEM
+  // allocation, combining the pass-1 partials into lse, the fence + last-arriver combine at the end); the launch takes
+  // ceil(CTAs / resident slots) rounds of that: pick the kt (<= 32) minimising rounds x (kt + 1).  c5: 7 (296 CTAs, exactly
+  // one round) instead of the former 3 (688 CTAs, 2.3 rounds): a2 218 -> 194 us; c4 x 16 is flat in kt (33-36 tile units).
+  // (Publishing lse from pass 1's last-arriving split instead, so that pass 2 only loads it, was measured: c2 23.6 -> 25.6 us
+  // — a fence + atomic round trip at the end of every pass-1 CTA — and no gain at c4.)
   int kt_per_cta = 1;
   {
     const int pairs = L.hkv * b->batch;
-    const int items = pairs * key_tiles;
-    const int budget = items <= 3 * slots ? slots : 3 * slots;
-    int per_pair = budget / pairs;
-    if (per_pair < 1) per_pair = 1;
-    kt_per_cta = (key_tiles + per_pair - 1) / per_pair;
+    double best = 1e30;
+    for (int kt = 1; kt <= 32 && kt <= key_tiles; ++kt) {
+      const int groups = (key_tiles + kt - 1) / kt;
+      const double rounds = std::ceil(static_cast<double>(groups) * pairs / slots);
+      const double cost = rounds * (kt + 1.0);
+      if (cost < best - 1e-9) { best = cost; kt_per_cta = kt; }
+    }
   }
   CUtensorMap tm_q, tm_k;
   // q_probe may be NULL when no request has query tokens: map a valid dummy address (never dereferenced: n_j == 0)
