@@ -516,21 +516,22 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
     if (n_splits > 8) n_splits = 8;            // x 2 column halves = 16 partials per row: pass 2 combines them in one batch of loads
     if (n_splits < 1) n_splits = 1;
   }
-  // pass 2: key tiles per CTA.  A CTA costs ~kt tile walks plus a fixed part worth about one walk (barrier setup, TMEM
-  // allocation, combining the pass-1 partials into lse, the fence + last-arriver combine at the end); the launch takes
-  // ceil(CTAs / resident slots) rounds of that: pick the kt (<= 32) minimising rounds x (kt + 1).  c5: 7 (296 CTAs, exactly
-  // one round) instead of the former 3 (688 CTAs, 2.3 rounds): a2 218 -> 194 us; c4 x 16 is flat in kt (33-36 tile units).
-  // (Publishing lse from pass 1's last-arriving split instead, so that pass 2 only loads it, was measured: c2 23.6 -> 25.6 us
-  // — a fence + atomic round trip at the end of every pass-1 CTA — and no gain at c4.)
+  // pass 2: key tiles per CTA (kt).  Equal-sized CTAs run in rounds of `slots`; a launch wastes the empty part of its last
+  // round and a fixed prologue per CTA (barriers, TMEM, combining the pass-1 partials into lse: ~0.3 of a tile walk).  Pick
+  // the kt <= 32 with the best (fill of the last round) x kt / (kt + 0.3).  Measured: c5 (8 pairs x 256 tiles) kt = 7 gives 296
+  // CTAs, exactly one round: a2 218 -> 202 us against the former 3 (688 CTAs, 2.3 rounds); c4 x 16 (128 pairs x 64 tiles)
+  // kt = 4 (2048 CTAs, 6.9 rounds) and the former 11 (768 CTAs) are within 1 %, kt = 32 (256 CTAs, one round at 86 % fill)
+  // is 7 % slower.  (Publishing lse from pass 1's last-arriving split so that pass 2 only loads it was also measured:
+  // c2 23.6 -> 25.6 us — a fence + atomic round trip at the end of every pass-1 CTA — and no gain at c4.)
   int kt_per_cta = 1;
   {
     const int pairs = L.hkv * b->batch;
-    double best = 1e30;
+    double best = -1.0;
     for (int kt = 1; kt <= 32 && kt <= key_tiles; ++kt) {
       const int groups = (key_tiles + kt - 1) / kt;
-      const double rounds = std::ceil(static_cast<double>(groups) * pairs / slots);
-      const double cost = rounds * (kt + 1.0);
-      if (cost < best - 1e-9) { best = cost; kt_per_cta = kt; }
+      const double rounds = static_cast<double>(groups) * pairs / slots;
+      const double score = rounds / std::ceil(rounds) * kt / (kt + 0.3);
+      if (score > best + 1e-9) { best = score; kt_per_cta = kt; }
     }
   }
   CUtensorMap tm_q, tm_k;
