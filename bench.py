@@ -468,12 +468,12 @@ def run_qcf(args) -> None:
     if sub == "all":
         # the other BASELINE configs, same code, fewer steps: one driver run reproduces every row of DESIGN.md §7
         cfgs = {}
-        for name in ("c2", "c5"):
+        for key, name, ratio in (("c2", "c2", None), ("c5", "c5", None), ("c4_rho0.1", "c4", 0.1), ("c4_rho0.5", "c4", 0.5)):
             s2 = ClockSampler(local); s2.start(); time.sleep(0.2)
-            r = measure_layer_config(name, None, max(10, min(args.steps, 50)), args.warmup, dev, dist, world,
-                                     want_e2e=False, want_cpu=False)
+            n_steps = max(10, min(args.steps, 50)) if ratio is None else 10        # configs[3] sweeps rho in {0.1, 0.3, 0.5}
+            r = measure_layer_config(name, ratio, n_steps, args.warmup, dev, dist, world, want_e2e=False, want_cpu=False)
             r["clocks"] = s2.stop()
-            cfgs[name] = r
+            cfgs[key] = r
         try:
             cfgs["c3"] = c3_record(args, steps=max(3, min(args.steps, 5)), light=True)
         except Exception as e:                               # the headline number must survive a failing sub-record
@@ -666,6 +666,14 @@ def c3_record(args, steps: int, light: bool) -> dict:
     run.stack.qcf_stack_first_token(run.hidden, run.n_rows - 1, g_fin, w_lm, logits, tok)
     decode_ms = timed(lambda: run.stack.qcf_stack_decode(tok, run.t, n_dec, run.k_fused, run.v_fused, g_fin, w_lm, dec_logits, dec_toks),
                       3, 1)
+    # the decode attention kernel alone: one new token over every layer's cache in turn (1.5 GB of K/V > L2, so each call
+    # reads its 42 MB from HBM)
+    q1 = torch.randn((sp.n_q_heads, sp.head_dim), device=dev).to(torch.bfloat16)
+    o1 = torch.empty_like(q1)
+    n_keys = run.t + n_dec
+    dattn_ms = timed(lambda: [ctx.qcf_decode_attn(q1, run.k_fused[l], run.v_fused[l], n_keys, o1) for l in range(sp.n_layers)], 3, 1)
+    dattn_us = float(dattn_ms.mean()) * 1e3 / sp.n_layers
+    dattn_gbps = 2.0 * n_keys * kv_row_b / (dattn_us * 1e-6) / 1e9
     clocks = sampler.stop()
 
     fl = run.flops()
@@ -704,6 +712,8 @@ def c3_record(args, steps: int, light: bool) -> dict:
                      "full_prefill_TFLOPps": (fl["gemm_full"] + fl["attn_full"]) / (float(full_ms.mean()) * 1e-3) / 1e12,
                      "ttft_ms_pinned_host": float(ttft_ms.mean()), "ttft_full_prefill_ms": float(ttft_full_ms.mean()),
                      "decode_ms_per_token": float(decode_ms.mean()) / n_dec,
+                     "decode_attn_us_per_layer": dattn_us, "decode_attn_GBps": dattn_gbps,
+                     "decode_attn_frac_hbm": dattn_gbps / float(load_peaks()[0]["hbm_gbs"]),
                      "decode_weight_stream_GBps": (13.9e9 * sp.n_layers / 36.0 + 2.0 * sp.vocab * sp.hidden) / (float(decode_ms.mean()) / n_dec * 1e-3) / 1e9,
                      "phase1_build_s": phase1_s, "selectors_pinned_host": selectors,
                      "pipeline_ms_vs_load_gbps": sweep},

@@ -5,8 +5,9 @@
 //
 // HBM-bound stream (every K and V row of the layer is read once: 2 * Hkv * d * 2 bytes per key, ~4 flop per byte), so no
 // tensor cores: the key range is split over (n_splits x Hkv) CTAs; a CTA stages 128-key tiles of its kv-head's K and V in
-// shared memory with one bulk async copy (cp.async.bulk, the TMA engine's 1-D mode) per 2*d-byte row, completion on an
-// mbarrier; K_{j+1} is in flight while P_j V_j runs and V_{j+1} while Q K_{j+1}^T runs.
+// shared memory with 16-byte asynchronous copies (cp.async, 16 consecutive threads per 2*d-byte row: fully coalesced);
+// K_{j+1} is in flight while P_j V_j runs and V_{j+1} while Q K_{j+1}^T runs.  (One cp.async.bulk per row was the first
+// version: 256 bulk copies of 256 B per tile ran at 1.3 TB/s — the per-copy cost of the bulk engine dominates at that size.)
 //   phase 1: thread = key   -> the G logits of its key (q broadcast from shared memory), block max, p = 2^(s - m)
 //   phase 2: thread = dim pair x key group -> o[g][dims] += p[g][key] * V[key][dims]
 // Split partials (m, l, o) go to a workspace; the LAST CTA of a kv-head (arrival counter) merges them in split order
@@ -26,12 +27,6 @@ constexpr int kKeys = 128;             // keys per tile = threads per CTA
 constexpr int kThreads = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
-
-__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
-               : "memory");
-}
 
 template <int D, int G>
 struct DecSmem {
@@ -60,7 +55,6 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
   const int split = blockIdx.x, n_splits = gridDim.x, g = blockIdx.y;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t sbase = smem_u32(smem);
-  const uint32_t barK = sbase + S::oBar, barV = barK + 8;
   float* s_q = reinterpret_cast<float*>(smem + S::oQ);
   float* s_p = reinterpret_cast<float*>(smem + S::oP);
   float* s_red = reinterpret_cast<float*>(smem + S::oRed);
@@ -72,32 +66,32 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
   const __nv_bfloat16* kg = k_cache + static_cast<size_t>(g) * D;
   const __nv_bfloat16* vg = v_cache + static_cast<size_t>(g) * D;
 
-  if (tid == 0) {
-    mbar_init(barK, 1);
-    mbar_init(barV, 1);
-    fence_barrier_init();
-  }
   pdl_trigger();
   pdl_wait();                                   // q and the newest cache row are written by the predecessor kernels
+  // tile `tile` of K or V -> shared memory: D/8 16-byte chunks per row, chunk index = thread-major so that 16 (d = 128) or 8
+  // (d = 64) consecutive threads copy one row; always ONE commit group per call (an empty one past the end keeps the
+  // wait_group arithmetic uniform)
+  auto issue = [&](const __nv_bfloat16* base, int off, int tile) {
+    if (tile < n_t) {
+      const int key0 = (t0 + tile) * kKeys;
+      const int n_valid = min(kKeys, n_keys - key0);
+      constexpr int CPR = D / 8;                               // chunks per row
+      for (int idx = tid; idx < n_valid * CPR; idx += kThreads) {
+        const int r = idx / CPR, c = idx % CPR;
+        cp_async16(sbase + off + r * S::kPitch + c * 16, base + static_cast<size_t>(key0 + r) * row_stride + c * 8);
+      }
+    }
+    cp_async_commit();
+  };
+  issue(kg, S::oK, 0);                          // the first tiles are in flight while q is fetched and scaled
+  issue(vg, S::oV, 0);
   // q of this kv-head's G heads -> fp32, pre-scaled (coherent loads: see the PDL note in qcf_internal.cuh)
   for (int i = tid; i < G * D / 2; i += kThreads) {
     const uint32_t w = *reinterpret_cast<const volatile uint32_t*>(q + (static_cast<size_t>(g) * G) * D + 2 * i);
     s_q[2 * i] = bf16lo(w) * scale_log2;
     s_q[2 * i + 1] = bf16hi(w) * scale_log2;
   }
-  __syncthreads();
-
-  auto issue = [&](const __nv_bfloat16* base, int off, uint32_t bar, int tile) {
-    const int key0 = (t0 + tile) * kKeys;
-    const int n_valid = min(kKeys, n_keys - key0);
-    if (tid == 0) mbar_arrive_expect_tx(bar, static_cast<uint32_t>(n_valid) * D * 2);
-    if (tid < n_valid)
-      bulk_copy_g2s(sbase + off + tid * S::kPitch, base + static_cast<size_t>(key0 + tid) * row_stride, D * 2, bar);
-  };
-  if (n_t > 0) {
-    issue(kg, S::oK, barK, 0);
-    issue(vg, S::oV, barV, 0);
-  }
+  // (no barrier here: the first __syncthreads of the tile loop orders s_q before its readers)
 
   float m_run[G], l_own[G], o[G][2];
 #pragma unroll
@@ -108,8 +102,9 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
     const int key0 = (t0 + j) * kKeys;
     const int key = key0 + tid;
     const bool valid = key < n_keys;
-    // ---- phase 1: logits of my key
-    mbar_wait(barK, j & 1);
+    // ---- phase 1: logits of my key.  Pending groups here: K(j), V(j) -> K(j) has landed once at most one is pending
+    cp_async_wait<1>();
+    __syncthreads();                            // every thread's chunks of K(j) are visible
     float s[G];
 #pragma unroll
     for (int h = 0; h < G; ++h) s[h] = 0.f;
@@ -143,7 +138,7 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
       if (lane == 0) s_red[warp * G + h] = mx;
     }
     __syncthreads();                            // (a) maxima visible; every thread has finished reading the K tile
-    if (j + 1 < n_t) issue(kg, S::oK, barK, j + 1);
+    issue(kg, S::oK, j + 1);                    // pending: V(j), K(j+1)
     float alpha[G];
 #pragma unroll
     for (int h = 0; h < G; ++h) {
@@ -156,7 +151,7 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
       s_p[tid * G + h] = p;
     }
     // ---- phase 2: o += P V over my key group, my dim pair
-    mbar_wait(barV, j & 1);
+    cp_async_wait<1>();                         // V(j) has landed (K(j+1) may still be in flight)
     if (!valid) {
       // tail rows were not copied: whatever the buffer holds must not meet p = 0 as NaN/inf
       uint4* vrow = reinterpret_cast<uint4*>(smem + S::oV + tid * S::kPitch);
@@ -179,9 +174,10 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
       }
     }
     __syncthreads();                            // (c) V tile, p and s_red are free again
-    if (j + 1 < n_t) issue(vg, S::oV, barV, j + 1);
+    issue(vg, S::oV, j + 1);                    // pending: K(j+1), V(j+1)
   }
 
+  cp_async_wait<0>();                           // (only empty groups can still be pending)
   // ---- split partial: l over the block, o over the key groups
   float* red_o = reinterpret_cast<float*>(smem + S::oK);       // K buffer is drained: [KG][G][D]
 #pragma unroll
@@ -216,28 +212,51 @@ __global__ void __launch_bounds__(kThreads) decode_attn_kernel(const __nv_bfloat
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  float* s_w = reinterpret_cast<float*>(smem + S::oV);           // weights [n_splits][G] (n_splits <= 64 * ... fits the V buffer)
+  // (The first version walked the splits with one dependent global load per step: ~40 L2 round trips in a row were 25 of the
+  // kernel's 32 us at c3.  Now the (m, l) pairs are staged in shared memory by all threads at once and the O partials are
+  // read eight splits at a time.)
+  float* s_ml = reinterpret_cast<float*>(smem + S::oV);          // [n_splits][G][2]
+  float* s_w = s_ml + n_splits * G * 2;                          // weights [n_splits][G]
   float* s_inv = s_p;                                            // 1 / l per head
+  for (int i = tid; i < n_splits * G * 2; i += kThreads) s_ml[i] = __ldcg(part_ml + static_cast<size_t>(g) * n_splits * G * 2 + i);
+  __syncthreads();
   if (tid < G) {
     float M = -INFINITY;
-    for (int sp = 0; sp < n_splits; ++sp) M = fmaxf(M, __ldcg(part_ml + ((static_cast<size_t>(g) * n_splits + sp) * G + tid) * 2));
+    for (int sp = 0; sp < n_splits; ++sp) M = fmaxf(M, s_ml[(sp * G + tid) * 2]);
     float L = 0.f;
-    for (int sp = 0; sp < n_splits; ++sp) {
-      const size_t o2 = ((static_cast<size_t>(g) * n_splits + sp) * G + tid) * 2;
-      const float w = ex2(__ldcg(part_ml + o2) - M);             // empty split: m = -inf -> weight 0
+    for (int sp = 0; sp < n_splits; ++sp) {                      // split order: bit-reproducible
+      const float w = ex2(s_ml[(sp * G + tid) * 2] - M);         // empty split: m = -inf -> weight 0
       s_w[sp * G + tid] = w;
-      L = fmaf(__ldcg(part_ml + o2 + 1), w, L);
+      L = fmaf(s_ml[(sp * G + tid) * 2 + 1], w, L);
     }
     s_inv[tid] = 1.f / L;
     if (lse_out) lse_out[g * G + tid] = (M + log2f(L)) * kLn2;
   }
   __syncthreads();
-  for (int i = tid; i < G * D; i += kThreads) {
-    const int h = i / D;
-    float acc = 0.f;
-    for (int sp = 0; sp < n_splits; ++sp)
-      acc = fmaf(__ldcg(part_o + (static_cast<size_t>(g) * n_splits + sp) * G * D + i), s_w[sp * G + h], acc);
-    out[(static_cast<size_t>(g) * G) * D + i] = __float2bfloat16_rn(acc * s_inv[h]);
+  // one float4 column group per thread, sixteen splits in flight: the whole merge is ceil(n_splits / 16) L2 round trips
+  for (int i4 = tid; i4 < G * D / 4; i4 += kThreads) {
+    const int h = (i4 * 4) / D;
+    const float4* src = reinterpret_cast<const float4*>(part_o + static_cast<size_t>(g) * n_splits * G * D) + i4;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int sp0 = 0; sp0 < n_splits; sp0 += 16) {
+      float4 v[16];
+#pragma unroll
+      for (int u = 0; u < 16; ++u)
+        v[u] = sp0 + u < n_splits ? __ldcg(src + static_cast<size_t>(sp0 + u) * (G * D / 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int u = 0; u < 16; ++u) {
+        if (sp0 + u < n_splits) {                                  // split order: bit-reproducible
+          const float w = s_w[(sp0 + u) * G + h];
+          acc.x = fmaf(v[u].x, w, acc.x); acc.y = fmaf(v[u].y, w, acc.y);
+          acc.z = fmaf(v[u].z, w, acc.z); acc.w = fmaf(v[u].w, w, acc.w);
+        }
+      }
+    }
+    const float inv = s_inv[h];
+    uint2 packed;
+    packed.x = pack_bf16(acc.x * inv, acc.y * inv);
+    packed.y = pack_bf16(acc.z * inv, acc.w * inv);
+    *reinterpret_cast<uint2*>(out + (static_cast<size_t>(g) * G) * D + i4 * 4) = packed;
   }
   if (tid == 0) counters[g] = 0u;                                // self-resetting
 }

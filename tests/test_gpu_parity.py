@@ -574,20 +574,23 @@ def test_full_size_c4_batched_pool(ratio):
         _check_full_size(wl, dw, b, 23 + b)
 
 
-def test_full_size_c4_batch16_rho03():
-    """BASELINE configs[3] exactly as `bench.py` times it: all 16 requests in ONE batched launch per stage, rho = 0.3.
-    The launch heuristics depend on the CTA count (a2's key splits / key tiles per CTA, a5's cluster size), so a smaller
-    batch does not reach the paths B = 16 takes.  Scores and the selection are checked in full, attention on the declared
-    row sample, for the first, the last and two seeded requests."""
-    wl, ctx, dw = _setup("c4", ratio=0.3)
+@pytest.mark.parametrize("ratio,k", [(0.3, 2457), (0.1, 819), (0.5, 4096)])
+def test_full_size_c4_batch16(ratio, k):
+    """BASELINE configs[3] exactly as `bench.py` times it: all 16 requests in ONE batched launch per stage, rho swept over
+    {0.1, 0.3, 0.5}.  The launch heuristics depend on the CTA count and on rho (a2's key splits / key tiles per CTA, a5's
+    cluster size, L2 groups and row-count hint, a4's bulk-copy choice), so a smaller batch does not reach the paths B = 16
+    takes.  Scores and the selection are checked in full, attention on the declared row sample — at the headline rho = 0.3
+    for the first, the last and two seeded requests, at the other two ratios for the first and the last."""
+    wl, ctx, dw = _setup("c4", ratio=ratio)
     assert dw.B == 16 and dw.batch.n_ctx[0] == 8192
     ctx.qcf_layer_step(dw.batch, dw.layer_args())
     torch.cuda.synchronize()
-    picks = sorted({0, 15} | set(int(x) for x in np.random.default_rng(404).choice(np.arange(1, 15), size=2, replace=False)))
-    for b in picks:
+    picks = {0, 15}
+    if ratio == 0.3:
+        picks |= set(int(x) for x in np.random.default_rng(404).choice(np.arange(1, 15), size=2, replace=False))
+    for b in sorted(picks):
         assert _check_full_size(wl, dw, b, 40 + b) >= 64 + 128
-    # every request selected floor(0.3 * 8192) = 2457 rows
-    assert dw.n_sel.cpu().tolist() == [2457] * 16
+    assert dw.n_sel.cpu().tolist() == [k] * 16                     # floor(rho * 8192), the seven pins of reading (g)
 
 
 def test_layer_step_host_rejects_chunks_outside_the_pool():
