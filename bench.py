@@ -351,9 +351,12 @@ def measure_layer_config(name, ratio, steps, warmup, dev, dist, world, want_e2e,
         torch.cuda.synchronize()
         e2e_s = (time.perf_counter() - t0) / n_e2e
         nb = lambda t: t.numel() * t.element_size()
-        h2d = nb(hw.k_pool) + nb(hw.v_pool) + nb(hw.q_probe) + nb(hw.q_new) + nb(hw.k_new) + nb(hw.v_new)
         q_row_b = cfg.n_q_heads * cfg.head_dim * 2
+        kv_row_b = cfg.n_kv_heads * cfg.head_dim * 2
         out_rows = sum(binding.qcf_n_select(n, cfg.ratio) + lq for n, lq in zip(hw.batch.n_ctx, hw.batch.n_query))
+        # bytes that cross the bus per step: the pool rows some request reads (shared chunks once), the probe, and — the host
+        # buffers are pinned, so the a4 / a5 kernels gather them straight from host memory — the |R_b| fresh rows only
+        h2d = 2 * int(hw.batch.pool_rows_touched) * kv_row_b + nb(hw.q_probe) + out_rows * (q_row_b + 2 * kv_row_b)
         d2h = out_rows * q_row_b + nb(hw.sel) + nb(hw.n_sel) + nb(hw.scores)      # only the |R_b| written rows of `out` come back
         e2e = (e2e_s, h2d, d2h, n_e2e)
         del hw, hargs
@@ -416,7 +419,8 @@ def measure_layer_config(name, ratio, steps, warmup, dev, dist, world, want_e2e,
     if e2e:
         rec["e2e"] = {"value": tokens_per_step * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(e2e[1]),
                       "d2h_bytes_per_step": int(e2e[2]), "ms_per_step": e2e_s * 1e3, "steps": e2e[3],
-                      "api": "qcf_layer_step_host (pinned host buffers, stream-synchronised per step)"}
+                      "api": "qcf_layer_step_host (pinned host buffers: pool rows and probe uploaded, fresh rows gathered zero-copy by the "
+                             "a4 / a5 kernels, |R| output rows downloaded; stream-synchronised per step)"}
     if want_cpu:
         wl1 = inputs.make_workload(name, ratio=ratio, batch=1) if cfg.batch != 1 else wl
         rec["cpu_baseline"] = cpu_baseline_record(wl1, cfg)

@@ -90,6 +90,7 @@ typedef struct {
   int32_t n_stride;    /* max_b N_b                                                                     */
   int32_t q_stride;    /* max_b Lq_b                                                                    */
   int64_t total_ctx;   /* sum_b N_b                                                                     */
+  int64_t pool_rows_touched; /* rows of the PIC pool the batch reads (union over requests: shared chunks count once) */
 } qcf_batch_info;
 
 /* ---------------------------------------------------------------------------------------------- lifetime */
@@ -273,6 +274,11 @@ typedef struct {
 QCF_API qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* args, void* stream);
 
 /* pool_rows: rows of host->k_pool / v_pool; every chunk of the batch must lie inside them (QCF_ERR_INVALID_ARG otherwise).
+ * Only the pool rows some request of the batch reads are uploaded (qcf_batch_info.pool_rows_touched rows per tensor).
+ * With rows_by_position != 0 and q_new / k_new / v_new in pinned, device-mapped host memory (cudaHostAlloc,
+ * cudaHostRegister, torch.pin_memory) those three buffers are not uploaded at all: the a4 and a5 kernels read the |R_b| rows
+ * they need straight from host memory (zero-copy gather; P is only known on the device after a3).  Pageable buffers are
+ * staged through a full upload as before.
  * Same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe
  * and fresh rows, runs qcf_layer_step on the context's internal device buffers, downloads the |R_b| written rows of `out`, `sel`,
  * `n_sel` (and the fused cache if k_fused / v_fused are non-NULL), and synchronises `stream` before

@@ -50,7 +50,7 @@ class qcf_request(C.Structure):
 
 class qcf_batch_info(C.Structure):
     _fields_ = [("batch", C.c_int32), ("t_stride", C.c_int32), ("n_stride", C.c_int32), ("q_stride", C.c_int32),
-                ("total_ctx", C.c_int64)]
+                ("total_ctx", C.c_int64), ("pool_rows_touched", C.c_int64)]
 
 
 class qcf_layer_args(C.Structure):
@@ -194,6 +194,7 @@ class Batch:
         ctx.lib.qcf_batch_get_info(self.handle, C.byref(info))
         self.batch, self.t_stride, self.n_stride, self.q_stride = info.batch, info.t_stride, info.n_stride, info.q_stride
         self.total_ctx = info.total_ctx
+        self.pool_rows_touched = info.pool_rows_touched
         self.n_ctx = [int(np.sum(c)) for c in chunk_lens]
         self.n_query = [int(q) for q in n_query]
 

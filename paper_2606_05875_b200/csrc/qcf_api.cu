@@ -131,6 +131,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->counters = nullptr;
   c->dec_part_o = c->dec_part_ml = nullptr; c->dec_counters = nullptr;
   c->stage = nullptr;
+  c->q_gather_src = nullptr; c->q_gather_dst = nullptr;
   c->pdl = 1; c->gemm_mt = 0; c->attn_cluster = 0;
   c->exch_rank = 0; c->exch_world = 1; c->exch_slot_elems = 0; c->exch_peers = nullptr; c->exch_epoch = 0;
   c->ratio_hint = 0.3;
@@ -235,12 +236,33 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
 
   qcf_batch* qb = new (std::nothrow) qcf_batch();
   if (!qb) return fail(ctx, QCF_ERR_WORKSPACE, "out of host memory");
-  qb->ctx = ctx; qb->blob = nullptr;
+  qb->ctx = ctx; qb->blob = nullptr; qb->h_pool_iv = nullptr; qb->n_pool_iv = 0; qb->pool_rows_touched = 0;
   qb->batch = batch; qb->n_chunks = n_chunks;
   qb->t_stride = t_stride; qb->n_stride = n_stride; qb->q_stride = q_stride;
   qb->max_ctx = n_stride; qb->max_query = q_stride; qb->total_ctx = total_ctx;
   qb->repo_blocks = c_blk.back();
   qb->pool_row_end = pool_row_end;
+  // union of the pool row ranges the batch reads (chunks shared by requests or adjacent in the pool merge): what a host-side
+  // step has to upload
+  {
+    std::vector<std::pair<int64_t, int64_t>> iv;
+    for (int c = 0; c < n_chunks; ++c) iv.emplace_back(c_row[c], c_row[c] + c_len[c]);
+    std::sort(iv.begin(), iv.end());
+    std::vector<int64_t> flat;
+    int64_t touched = 0;
+    for (size_t i = 0; i < iv.size();) {
+      int64_t lo = iv[i].first, hi = iv[i].second;
+      size_t j = i + 1;
+      while (j < iv.size() && iv[j].first <= hi) { hi = std::max(hi, iv[j].second); ++j; }
+      flat.push_back(lo); flat.push_back(hi - lo);
+      touched += hi - lo;
+      i = j;
+    }
+    qb->n_pool_iv = static_cast<int32_t>(flat.size() / 2);
+    qb->pool_rows_touched = touched;
+    qb->h_pool_iv = static_cast<int64_t*>(std::malloc(sizeof(int64_t) * (flat.empty() ? 1 : flat.size())));
+    if (!flat.empty()) std::memcpy(qb->h_pool_iv, flat.data(), sizeof(int64_t) * flat.size());
+  }
   qb->h_n_ctx = static_cast<int32_t*>(std::malloc(sizeof(int32_t) * (batch > 0 ? batch : 1)));
   qb->h_n_query = static_cast<int32_t*>(std::malloc(sizeof(int32_t) * (batch > 0 ? batch : 1)));
   if (batch > 0) {
@@ -307,6 +329,7 @@ void qcf_batch_destroy(qcf_batch* b) {
   if (b->blob) cudaFree(b->blob);
   std::free(b->h_n_ctx);
   std::free(b->h_n_query);
+  std::free(b->h_pool_iv);
   delete b;
 }
 
@@ -314,6 +337,7 @@ qcf_status qcf_batch_get_info(const qcf_batch* b, qcf_batch_info* info) {
   if (!b || !info) return QCF_ERR_INVALID_ARG;
   info->batch = b->batch; info->t_stride = b->t_stride; info->n_stride = b->n_stride; info->q_stride = b->q_stride;
   info->total_ctx = b->total_ctx;
+  info->pool_rows_touched = b->pool_rows_touched;
   return QCF_OK;
 }
 
@@ -401,8 +425,17 @@ qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
   QCF_CUDA(ctx, launch_scatter(ctx, b, sel_nn, n_sel, static_cast<const __nv_bfloat16*>(k_new),
                                static_cast<const __nv_bfloat16*>(v_new), rows_by_position != 0,
                                static_cast<__nv_bfloat16*>(k_fused), static_cast<__nv_bfloat16*>(v_fused), s));
+  int q_by_position = rows_by_position != 0;
+  if (ctx->q_gather_src) {
+    // zero-copy host step: the rows R of the host-resident q_new are gathered (bulk copies over PCIe) into a compact device
+    // buffer; a5 then reads q compactly while a4 above read k_new / v_new by position
+    QCF_CUDA(ctx, launch_gather_rows(ctx, b, sel_nn, n_sel, ctx->q_gather_src, ctx->q_gather_dst,
+                                     ctx->lay.hq * ctx->lay.d * 2, s));
+    q_new = ctx->q_gather_dst;
+    q_by_position = 0;
+  }
   if (ctx->profiling && ctx->ev_valid) cudaEventRecord(ctx->ev[4], s);
-  QCF_CUDA(ctx, launch_attn(ctx, b, sel_nn, n_sel, static_cast<const __nv_bfloat16*>(q_new), rows_by_position != 0,
+  QCF_CUDA(ctx, launch_attn(ctx, b, sel_nn, n_sel, static_cast<const __nv_bfloat16*>(q_new), q_by_position,
                             static_cast<const __nv_bfloat16*>(k_fused), static_cast<const __nv_bfloat16*>(v_fused),
                             static_cast<__nv_bfloat16*>(out), lse, s));
   return QCF_OK;
@@ -574,13 +607,42 @@ qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer
   QCF_CUDA(ctx, S.k_f.reserve(fused_bytes + 16)); QCF_CUDA(ctx, S.v_f.reserve(fused_bytes + 16));
   QCF_CUDA(ctx, S.q_probe.reserve(probe_bytes + 16)); QCF_CUDA(ctx, S.scores.reserve(score_bytes + 16));
   QCF_CUDA(ctx, S.sel.reserve(sel_bytes + 16)); QCF_CUDA(ctx, S.n_sel.reserve(B * sizeof(int32_t)));
-  QCF_CUDA(ctx, S.q_new.reserve(qnew_bytes + 16)); QCF_CUDA(ctx, S.k_new.reserve(fused_bytes + 16));
-  QCF_CUDA(ctx, S.v_new.reserve(fused_bytes + 16)); QCF_CUDA(ctx, S.out.reserve(qnew_bytes + 16));
+  // Position-indexed fresh rows: only the rows in R = P u U (~rho of them) are ever read, but P is decided on the device by
+  // a3, so a staged upload has to move ALL of q_new / k_new / v_new (60 % of the step's H2D bytes at config 4).  When the three
+  // host buffers are pinned AND mapped into the device's address space (cudaHostAlloc / cudaHostRegister under unified
+  // addressing — what torch.pin_memory gives), the a4 and a5 kernels read the rows they need straight from host memory
+  // over PCIe instead: zero-copy gather, only |R| rows cross the bus.
+  const void *zq = nullptr, *zk = nullptr, *zv = nullptr;
+  bool zero_copy = h->rows_by_position != 0;
+  if (zero_copy) {
+    const void* hp[3] = {h->q_new, h->k_new, h->v_new};
+    const void** zp[3] = {&zq, &zk, &zv};
+    for (int i = 0; i < 3 && zero_copy; ++i) {
+      cudaPointerAttributes at{};
+      if (cudaPointerGetAttributes(&at, hp[i]) != cudaSuccess || at.type != cudaMemoryTypeHost || at.devicePointer == nullptr) {
+        cudaGetLastError();                        // pageable memory: not an error, just the staged path
+        zero_copy = false;
+      } else {
+        *zp[i] = at.devicePointer;
+      }
+    }
+  }
+  QCF_CUDA(ctx, S.q_new.reserve(qnew_bytes + 16));                 // staged copy, or the compact gather destination
+  if (!zero_copy) {
+    QCF_CUDA(ctx, S.k_new.reserve(fused_bytes + 16));
+    QCF_CUDA(ctx, S.v_new.reserve(fused_bytes + 16));
+  }
+  QCF_CUDA(ctx, S.out.reserve(qnew_bytes + 16));
   if (h->lse) QCF_CUDA(ctx, S.lse.reserve(B * b->t_stride * L.hq * sizeof(float) + 16));
 
-  // uploads: PIC pool rows, probe, fresh rows; scores / sel when the caller carries them across layers
-  QCF_CUDA(ctx, cudaMemcpyAsync(S.k_pool.p, h->k_pool, pool_bytes, cudaMemcpyHostToDevice, s));
-  QCF_CUDA(ctx, cudaMemcpyAsync(S.v_pool.p, h->v_pool, pool_bytes, cudaMemcpyHostToDevice, s));
+  // uploads: the PIC pool rows the batch READS (merged intervals: chunks no request references stay on the host — at config 4
+  // the 16 requests touch ~100 of the pool's 256 chunks), probe, fresh rows; scores / sel when the caller carries them across
+  // layers.  One cudaMemcpyAsync per interval and tensor.
+  for (int i = 0; i < b->n_pool_iv; ++i) {
+    const size_t off = static_cast<size_t>(b->h_pool_iv[2 * i]) * kv_row, len = static_cast<size_t>(b->h_pool_iv[2 * i + 1]) * kv_row;
+    QCF_CUDA(ctx, cudaMemcpyAsync(static_cast<char*>(S.k_pool.p) + off, static_cast<const char*>(h->k_pool) + off, len, cudaMemcpyHostToDevice, s));
+    QCF_CUDA(ctx, cudaMemcpyAsync(static_cast<char*>(S.v_pool.p) + off, static_cast<const char*>(h->v_pool) + off, len, cudaMemcpyHostToDevice, s));
+  }
   if (h->is_critical_layer) QCF_CUDA(ctx, cudaMemcpyAsync(S.q_probe.p, h->q_probe, probe_bytes, cudaMemcpyHostToDevice, s));
   if (h->is_critical_layer && h->accumulate) {
     QCF_REQUIRE(ctx, h->scores != nullptr, "qcf_layer_step_host: scores is NULL with accumulate");
@@ -590,17 +652,24 @@ qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer
     QCF_CUDA(ctx, cudaMemcpyAsync(S.sel.p, h->sel, sel_bytes, cudaMemcpyHostToDevice, s));
     QCF_CUDA(ctx, cudaMemcpyAsync(S.n_sel.p, h->n_sel, B * sizeof(int32_t), cudaMemcpyHostToDevice, s));
   }
-  QCF_CUDA(ctx, cudaMemcpyAsync(S.q_new.p, h->q_new, qnew_bytes, cudaMemcpyHostToDevice, s));
-  QCF_CUDA(ctx, cudaMemcpyAsync(S.k_new.p, h->k_new, fused_bytes, cudaMemcpyHostToDevice, s));
-  QCF_CUDA(ctx, cudaMemcpyAsync(S.v_new.p, h->v_new, fused_bytes, cudaMemcpyHostToDevice, s));
+  if (!zero_copy) {
+    QCF_CUDA(ctx, cudaMemcpyAsync(S.q_new.p, h->q_new, qnew_bytes, cudaMemcpyHostToDevice, s));
+    QCF_CUDA(ctx, cudaMemcpyAsync(S.k_new.p, h->k_new, fused_bytes, cudaMemcpyHostToDevice, s));
+    QCF_CUDA(ctx, cudaMemcpyAsync(S.v_new.p, h->v_new, fused_bytes, cudaMemcpyHostToDevice, s));
+  }
 
   qcf_layer_args d = *h;
   d.k_pool = S.k_pool.p; d.v_pool = S.v_pool.p; d.k_fused = S.k_f.p; d.v_fused = S.v_f.p;
   d.q_probe = S.q_probe.p; d.scores = static_cast<float*>(S.scores.p);
   d.sel = static_cast<int32_t*>(S.sel.p); d.n_sel = static_cast<int32_t*>(S.n_sel.p);
-  d.q_new = S.q_new.p; d.k_new = S.k_new.p; d.v_new = S.v_new.p; d.out = S.out.p;
+  d.q_new = zero_copy ? zq : S.q_new.p; d.k_new = zero_copy ? zk : S.k_new.p; d.v_new = zero_copy ? zv : S.v_new.p;
+  d.out = S.out.p;
+  ctx->q_gather_src = zero_copy ? zq : nullptr;
+  ctx->q_gather_dst = S.q_new.p;
   d.lse = h->lse ? static_cast<float*>(S.lse.p) : nullptr;
-  if (qcf_status st = qcf_layer_step(ctx, b, &d, stream)) return st;
+  const qcf_status st_step = qcf_layer_step(ctx, b, &d, stream);
+  ctx->q_gather_src = nullptr;
+  if (st_step) return st_step;
 
   // only the |R_b| = k_b + Lq_b rows the step wrote are read back (k_b is known on the host: floor(rho N_b) when the step
   // selects, the caller's n_sel otherwise)

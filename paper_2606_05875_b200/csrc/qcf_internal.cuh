@@ -85,6 +85,8 @@ struct qcf_ctx {
   unsigned int* dec_counters;
   // host staging for qcf_layer_step_host
   struct HostStage* stage;
+  const void* q_gather_src;   // != nullptr during a zero-copy host step: position-indexed q_new in device-mapped host memory
+  void* q_gather_dst;         //   ... and the device buffer its rows R are gathered into (compact) before a5
   // profiling
   int profiling;
   static constexpr int kEvRing = 512;   // profiled steps kept between two qcf_get_stage_ms calls
@@ -107,6 +109,9 @@ struct qcf_batch {
   int64_t total_ctx;
   int32_t repo_blocks;     // total reposition work items
   int64_t pool_row_end;    // max over chunks of chunk_row + chunk_len: rows of the pool the batch reads (host-side validation)
+  int64_t* h_pool_iv;      // [2 * n_pool_iv] merged (first row, row count) intervals of the pool rows the batch reads
+  int32_t n_pool_iv;
+  int64_t pool_rows_touched;   // sum of the interval lengths
   int32_t* h_n_ctx;        // [batch]
   int32_t* h_n_query;      // [batch]
 };
@@ -135,6 +140,9 @@ cudaError_t launch_anchor_scores(const qcf_ctx*, const qcf_batch*, const __nv_bf
 cudaError_t launch_scatter(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                            const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, int rows_by_position,
                            __nv_bfloat16* k_f, __nv_bfloat16* v_f, cudaStream_t);
+// rows R_b of a position-indexed source (may be device-mapped host memory) -> compact rows in R order
+cudaError_t launch_gather_rows(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
+                               const void* src_by_pos, void* dst_compact, int row_bytes, cudaStream_t);
 // sel == nullptr: dense mode (rows 0..N+Lq-1 at their own positions, q indexed by position).
 cudaError_t launch_attn(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                         const __nv_bfloat16* q, int rows_by_position, const __nv_bfloat16* k_f,

@@ -86,7 +86,66 @@ __global__ void __launch_bounds__(256) scatter_kernel(BatchDev bd, int row_vec, 
   }
 }
 
+// Zero-copy gather for the host-side step (qcf_layer_step_host): the position-indexed q_new lives in pinned, device-mapped
+// HOST memory and only the rows of R are needed, so each row travels over PCIe as bulk async copies of <= 4 KB pieces
+// (host -> shared -> device), landing COMPACT in R order (row r of the destination = position R_b[r] of the source) — the
+// layout the attention kernel reads with q_by_position = 0.  Per-thread 16-byte loads from host memory reach ~12 GB/s
+// (32-byte PCIe read requests); bulk copies reach the link rate (~50 GB/s, measured on a4 with host-resident k_new / v_new).
+__global__ void __launch_bounds__(32) gather_rows_tma_kernel(BatchDev bd, uint32_t row_bytes, uint32_t piece_bytes,
+                                                             const int32_t* sel, const int32_t* n_sel,
+                                                             const unsigned char* src_by_pos, unsigned char* dst_compact) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  __shared__ __align__(8) unsigned long long s_bar[kScatterSlots];
+  const int lane = threadIdx.x;
+  const int b = blockIdx.y;
+  const int N = bd.n_ctx[b], Lq = bd.n_query[b];
+  if (lane < kScatterSlots) ptx::mbar_init(smem_u32(&s_bar[lane]), 1);
+  ptx::fence_barrier_init();
+  pdl_trigger();
+  __syncwarp();
+  pdl_wait();
+  const int ns = __ldcg(n_sel + b);
+  const int pieces = static_cast<int>(row_bytes / piece_bytes);
+  const long long n_items = static_cast<long long>(ns + Lq) * pieces;
+  const size_t base = static_cast<size_t>(b) * bd.t_stride;
+  const uint32_t bar = smem_u32(&s_bar[lane & (kScatterSlots - 1)]);
+  const uint32_t buf = smem_u32(smem) + static_cast<uint32_t>(lane & (kScatterSlots - 1)) * piece_bytes;
+  uint32_t phase = 0;
+  for (long long w0 = static_cast<long long>(blockIdx.x) * kScatterSlots; w0 < n_items; w0 += static_cast<long long>(gridDim.x) * kScatterSlots) {
+    const long long w = w0 + lane;
+    if (lane < kScatterSlots && w < n_items) {
+      const int r = static_cast<int>(w / pieces), piece = static_cast<int>(w % pieces);
+      const int p = r < ns ? __ldcg(sel + static_cast<size_t>(b) * bd.n_stride + r) : N + (r - ns);
+      const size_t off = static_cast<size_t>(piece) * piece_bytes;
+      ptx::mbar_arrive_expect_tx(bar, piece_bytes);
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(buf), "l"(src_by_pos + (base + p) * row_bytes + off), "r"(piece_bytes), "r"(bar) : "memory");
+      ptx::mbar_wait(bar, phase);
+      phase ^= 1u;
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                   ::"l"(dst_compact + (base + r) * row_bytes + off), "r"(buf), "r"(piece_bytes) : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    }
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_gather_rows(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                               const void* src_by_pos, void* dst_compact, int row_bytes, cudaStream_t stream) {
+  if (b->batch == 0 || b->t_stride == 0) return cudaSuccess;
+  uint32_t piece = 4096;
+  while (row_bytes % piece) piece >>= 1;                  // row_bytes is a multiple of 16
+  const long long max_items = static_cast<long long>(b->t_stride) * (row_bytes / piece);
+  long long blocks = (max_items + kScatterSlots - 1) / kScatterSlots;
+  if (blocks > ctx->n_sm * 16) blocks = ctx->n_sm * 16;
+  const size_t smem = static_cast<size_t>(kScatterSlots) * piece;
+  if (smem > 48 * 1024) cudaFuncSetAttribute(gather_rows_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+  return launch_pdl(ctx->pdl, gather_rows_tma_kernel, dim3(static_cast<unsigned>(blocks), b->batch), dim3(32), smem, stream, b->dev,
+                    static_cast<uint32_t>(row_bytes), piece, sel, n_sel, static_cast<const unsigned char*>(src_by_pos),
+                    static_cast<unsigned char*>(dst_compact));
+}
 
 cudaError_t launch_scatter(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
                            const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, int rows_by_position,

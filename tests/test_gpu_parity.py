@@ -436,12 +436,16 @@ def test_layer_step_profiling_and_noncritical():
     assert torch.equal(sel0, dw.sel) and torch.equal(out0, dw.out)
 
 
-def test_layer_step_host_matches_device():
+@pytest.mark.parametrize("pin", [True, False])
+def test_layer_step_host_matches_device(pin):
+    """qcf_layer_step_host: pinned (device-mapped) host buffers take the zero-copy path — only the pool rows the batch reads
+    are uploaded, the a4 kernel and a bulk-copy gather read the rows of R straight from host memory — pageable buffers are
+    staged through full uploads.  Both must reproduce the device-resident step bit for bit."""
     _, device = _binding()
     wl, ctx, dw = _setup("t_batch")
     ctx.qcf_layer_step(dw.batch, dw.layer_args())
     torch.cuda.synchronize()
-    hw = device.DeviceWorkload(wl, ctx, device="cpu", pin=True)
+    hw = device.DeviceWorkload(wl, ctx, device="cpu", pin=pin)
     args = hw.layer_args()
     args.k_fused, args.v_fused = hw.k_fused.data_ptr(), hw.v_fused.data_ptr()
     ctx.qcf_layer_step_host(hw.batch, args, hw.pool_rows)
