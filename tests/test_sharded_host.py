@@ -76,3 +76,19 @@ def test_score_exchange_buffer_size_is_header_plus_slots():
     assert binding.qcf_score_exchange_bytes(8, 16 * 8192) == 256 + 8 * 16 * 8192 * 4
     assert binding.qcf_score_exchange_bytes(0, 10) == -1 and binding.qcf_score_exchange_bytes(65, 10) == -1
     assert binding.qcf_score_exchange_bytes(2, -1) == -1
+
+
+def _bench_worker(rank, world, port):
+    import torch.distributed as dist
+    import bench
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    # the replica mode of bench.py (N > 1): every rank times its own replica, the line reports the MAX over ranks
+    got = bench.max_over_ranks([10.0 + rank, 5.0 - rank, 7.0], dist, "cpu")
+    assert got == [10.0 + world - 1, 5.0, 7.0]
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_bench_takes_the_max_over_ranks_two_gloo_ranks():
+    import torch.multiprocessing as mp
+    mp.spawn(_bench_worker, args=(2, 29743), nprocs=2, join=True)
