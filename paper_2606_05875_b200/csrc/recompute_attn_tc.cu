@@ -649,6 +649,7 @@ cudaError_t launch_attn(const qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
   // of the 126 MB L2 — two consecutive groups overlap at their boundary; whole requests when more than one fits.
   const int n_units = L.hkv * b->batch;
   const double unit_bytes = static_cast<double>(b->t_stride) * L.d * 2.0 * 2.0;
+  // (16 / 24 / 48 / 96 MB measured: a5 at c4 x 16 2.89 / 2.86 / 2.84 / 2.97 ms, c5 2.55 / 2.59 / 2.55 / 2.61 ms)
   int unit_grp = static_cast<int>(48.0 * 1024 * 1024 / unit_bytes);
   if (unit_grp >= L.hkv) unit_grp -= unit_grp % L.hkv;
   if (unit_grp < 1) unit_grp = 1;
