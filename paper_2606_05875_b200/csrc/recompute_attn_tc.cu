@@ -53,7 +53,7 @@ constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (
 //     the 512 the unit could do), so serialising the groups halves the MUFU rate, and a shared issuer blocks one item on
 //     the other's P; two independent CTAs per SM remain the best arrangement found;
 //   * halving the K/V loads (timing experiment, wrong results): c2 unchanged, c5 -9 %: L2 -> SM traffic is not the limiter;
-//   * a persistent work-list kernel (recompute_attn_ptc.cu);
+//   * a persistent work-list kernel (device-built work list, split-KV partials merged by the last arriver; removed from the tree);
 //   * S = Q K^T for PAIRS of key tiles as one 128 x 128 x 16 chain into a single 128-column S buffer (the TMEM budget of two
 //     CTAs per SM leaves no room to double-buffer it): c2 75.8 -> 90.1 us, c5 2.51 -> 2.90 ms — the serialised
 //     QK -> softmax -> PV chain costs more than the cheaper MMA saves;
