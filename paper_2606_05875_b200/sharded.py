@@ -56,15 +56,24 @@ def share_exchange_buffers(mine, rank: int, world: int, group=None):
     from torch.multiprocessing.reductions import reduce_tensor
     if world == 1:
         return [mine]
+    import torch
     handles = [None] * world
-    dist.all_gather_object(handles, reduce_tensor(mine), group=group)
+    dist.all_gather_object(handles, (mine.device.index, reduce_tensor(mine)), group=group)
     peers = []
     for p in range(world):
         if p == rank:
             peers.append(mine)
-        else:
-            fn, args = handles[p]
-            peers.append(fn(*args))
+            continue
+        dev_p, (fn, args) = handles[p]
+        if dev_p != mine.device.index:
+            # the kernels dereference the peer's buffer directly: peer access must be on (NVLink / NVSwitch P2P)
+            if not torch.cuda.can_device_access_peer(mine.device.index, dev_p):
+                raise RuntimeError("GPU %d cannot access GPU %d: the fused score exchange needs peer access" %
+                                   (mine.device.index, dev_p))
+            err = torch.cuda.cudart().cudaDeviceEnablePeerAccess(dev_p, 0)
+            if int(err) not in (0, 704):                      # 704: cudaErrorPeerAccessAlreadyEnabled
+                raise RuntimeError("cudaDeviceEnablePeerAccess(%d) failed: %s" % (dev_p, err))
+        peers.append(fn(*args))
     return peers
 
 
