@@ -215,14 +215,16 @@ def test_layer_step_through_a_nccl_group_of_one():
 
 # ----------------------------------------------------------------------------------------------- two processes, one GPU, CUDA IPC
 
-def _ipc_rank(rank, world, name, q_bufs, q_res, barrier):
-    """One rank of the fused-exchange step in its own PROCESS (own CUDA context).  Phases are ordered on the host so that
-    no kernel ever waits on a flag another process has not written yet (B200_PROFILING.md: ranks that spin on one another
-    must not share a GPU)."""
-    import numpy as np
+def _ipc_rank(rank, world, name, port, q_res):
+    """One rank of the fused-exchange step in its own PROCESS (own CUDA context).  Rendezvous exactly as production does it
+    (sharded.share_exchange_buffers: CUDA IPC handles carried by torch.distributed, here a gloo group); phases are ordered on
+    the host so that no kernel ever waits on a flag another process has not written yet (B200_PROFILING.md: ranks that
+    spin on one another must not share a GPU)."""
     import torch
+    import torch.distributed as dist
     from paper_2606_05875_b200 import device, inputs, sharded
     torch.cuda.set_device(0)
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
     wl = inputs.make_workload(name)
     cfg = wl.cfg
     st = sharded.HeadShardedStep(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, max(cfg.batch, 1),
@@ -230,27 +232,21 @@ def _ipc_rank(rank, world, name, q_bufs, q_res, barrier):
     dw = device.DeviceWorkload(inputs.shard_heads(wl, rank, world), st.ctx)
     slot = dw.batch.batch * dw.batch.n_stride
     mine = sharded.HeadShardedStep.alloc_exchange_buffer(world, slot)
-    for p in range(world):                        # my buffer to every peer: torch.multiprocessing maps it with cudaIpc*
-        if p != rank:
-            q_bufs[p].put((rank, mine))
-    peers = {rank: mine}
-    while len(peers) < world:
-        r, t = q_bufs[rank].get(timeout=120)
-        peers[r] = t
-    st.enable_fused_exchange([peers[p] for p in range(world)], slot)
-    barrier.wait(timeout=120)
+    st.enable_fused_exchange(sharded.share_exchange_buffers(mine, rank, world), slot)     # peers mapped with cudaIpc*
+    dist.barrier()
     for turn in range(world):                     # a2 of one rank at a time (peer stores + flag release), host-ordered
         if turn == rank:
             st.score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
                            q_probe=dw.q_probe, scores=dw.scores)
             torch.cuda.synchronize()
-        barrier.wait(timeout=120)
+        dist.barrier()
     st.fuse_phase(dw.batch, scores=None, sel=dw.sel, n_sel=dw.n_sel, q_new=dw.q_new, k_new=dw.k_new, v_new=dw.v_new,
                   k_fused=dw.k_fused, v_fused=dw.v_fused, out=dw.out, ratio=cfg.ratio)      # a3 acquires flags already set
     torch.cuda.synchronize()
     q_res.put((rank, dw.n_sel.cpu().numpy(), dw.sel.cpu().numpy(), st.exchanged_scores(dw.batch).cpu().numpy(),
                dw.out.cpu().view(torch.int16).numpy()))
-    barrier.wait(timeout=120)                     # keep the exported buffers alive until every peer is done
+    dist.barrier()                                # keep the exported buffers alive until every peer is done
+    dist.destroy_process_group()
 
 
 def test_fused_exchange_two_processes_one_gpu_cuda_ipc():
@@ -261,10 +257,8 @@ def test_fused_exchange_two_processes_one_gpu_cuda_ipc():
     import torch.multiprocessing as mp
     name, world = "t_mid", 2
     ctx = mp.get_context("spawn")
-    q_bufs = [ctx.Queue() for _ in range(world)]
     q_res = ctx.Queue()
-    barrier = ctx.Barrier(world)
-    procs = [ctx.Process(target=_ipc_rank, args=(r, world, name, q_bufs, q_res, barrier)) for r in range(world)]
+    procs = [ctx.Process(target=_ipc_rank, args=(r, world, name, 29747, q_res)) for r in range(world)]
     for p in procs:
         p.start()
     try:
