@@ -446,6 +446,9 @@ def test_layer_step_host_matches_device(pin):
     ctx.qcf_layer_step(dw.batch, dw.layer_args())
     torch.cuda.synchronize()
     hw = device.DeviceWorkload(wl, ctx, device="cpu", pin=pin)
+    # chunks shared by several requests are uploaded once: the batch knows the union of the pool rows it reads
+    used = sorted({int(i) for r in wl.requests for i in r.chunk_ids})
+    assert hw.batch.pool_rows_touched == sum(wl.pool_k[i].shape[0] for i in used) <= hw.pool_rows
     args = hw.layer_args()
     args.k_fused, args.v_fused = hw.k_fused.data_ptr(), hw.v_fused.data_ptr()
     ctx.qcf_layer_step_host(hw.batch, args, hw.pool_rows)
