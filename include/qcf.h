@@ -390,6 +390,27 @@ QCF_API qcf_status qcf_stack_first_token(qcf_stack* s, const void* hidden, int32
 QCF_API qcf_status qcf_decode_attn(qcf_ctx* ctx, const void* q, const void* k_cache, const void* v_cache, int32_t n_keys,
                                    void* out, float* lse, void* stream);
 
+/* qcf_decode_attn_static — qcf_decode_attn for callers that cannot allocate device memory.  Same operation, same kernel,
+ * same arguments and result (bit-identical to qcf_decode_attn for the same layout on the same GPU), but no qcf_ctx:
+ * qcf_create cudaMallocs the kernel's split-KV workspace, and that is exactly what some callers may not do — an op
+ * plugged into a serving engine whose pool allocator already owns all of HBM, code inside a region its framework has
+ * declared allocation-free, a monitoring tool that must leave the allocator untouched.  Here the workspace is a fixed
+ * array inside the library image (about 2.1 MiB of device memory on every GPU that loads libqcf.so, held until the
+ * process exits), and the call itself makes no cudaMalloc / cudaFree and uses no allocating library routine: it is one
+ * 256-byte cudaMemsetAsync (the arrival counters) plus one kernel launch on `stream`.
+ *   layout : host; Hq * head_dim <= 8192 and Hkv <= 64 (what the fixed workspace holds; beyond it the call fails with
+ *            QCF_ERR_WORKSPACE and launches nothing — use qcf_create + qcf_decode_attn there), head_dim 64 or 128,
+ *            Hq / Hkv in {1,2,4,8,16}; softmax_scale 0 -> 1/sqrt(d); rope_theta is not used.  n_keys >= 1, no upper limit.
+ *   q, k_cache, v_cache, out, lse : as for qcf_decode_attn; the caller owns them.
+ * First call on each device: with that device current, the library looks up the array's device address and the SM count
+ * (a few driver queries, no allocation) and keeps them; make that first call outside any stream capture.
+ * One workspace per GPU, shared by every caller and thread: two calls whose kernels can overlap on the GPU (different
+ * streams, no ordering between them) race on it and both results are undefined; calls on one stream, or ordered by
+ * events, are fine.  Each call clears the counters it needs; the rest of the array is overwritten before it is read.
+ * Errors: returned as a status; the message is qcf_last_error(NULL) on the calling thread. */
+QCF_API qcf_status qcf_decode_attn_static(const qcf_layout* layout, const void* q, const void* k_cache, const void* v_cache,
+                                          int32_t n_keys, void* out, float* lse, void* stream);
+
 /* qcf_stack_decode — n_new greedy tokens, one at a time through every layer:
  *   token i (i = 0: *token_in, the token qcf_stack_first_token produced; else tokens_out[i-1]) is embedded, sits at request
  *   position pos0 + i, and per layer: RMSNorm -> QKV projection -> QK-norm + RoPE at that position -> its K/V APPENDED as

@@ -23,7 +23,7 @@ EXPORTS = (
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards", "qcf_debug_set",
     "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
-    "qcf_decode_attn", "qcf_stack_decode", "qcf_score_exchange_bytes", "qcf_set_score_exchange",
+    "qcf_decode_attn", "qcf_decode_attn_static", "qcf_stack_decode", "qcf_score_exchange_bytes", "qcf_set_score_exchange",
 )
 
 QCF_EPI_STORE, QCF_EPI_ADD_RESIDUAL, QCF_EPI_SWIGLU = 0, 1, 2
@@ -127,6 +127,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_stack_fuse": (i32, [vp, vp, vp, C.POINTER(qcf_fuse_args), vp]),
         "qcf_stack_first_token": (i32, [vp, vp, i32, vp, vp, vp, vp, vp]),
         "qcf_decode_attn": (i32, [vp, vp, vp, vp, i32, vp, vp, vp]),
+        "qcf_decode_attn_static": (i32, [C.POINTER(qcf_layout), vp, vp, vp, i32, vp, vp, vp]),
         "qcf_stack_decode": (i32, [vp, vp, i32, i32, C.POINTER(vp), C.POINTER(vp), vp, vp, vp, vp, vp]),
     }
     for name, (res, args) in sigs.items():
@@ -158,6 +159,18 @@ def _stream(stream) -> Optional[int]:
 
 def qcf_score_exchange_bytes(n_shards: int, slot_elems: int) -> int:
     return int(load_library().qcf_score_exchange_bytes(int(n_shards), int(slot_elems)))
+
+
+def qcf_decode_attn_static(n_q_heads: int, n_kv_heads: int, head_dim: int, q, k_cache, v_cache, n_keys: int, out, lse=None,
+                           softmax_scale: float = 0.0, stream=None) -> None:
+    """qcf_decode_attn without a Context: for callers that must not allocate device memory (the kernel's workspace is a
+    fixed array inside libqcf.so; limits and sharing rules in include/qcf.h).  Marshals the arguments, nothing else."""
+    lib = load_library()
+    lay = qcf_layout(int(n_q_heads), int(n_kv_heads), int(head_dim), 0.0, float(softmax_scale))
+    st = lib.qcf_decode_attn_static(C.byref(lay), _ptr(q), _ptr(k_cache), _ptr(v_cache), int(n_keys), _ptr(out), _ptr(lse),
+                                    _stream(stream))
+    if st != QCF_OK:
+        raise QcfError(st, (lib.qcf_last_error(None) or b"").decode())
 
 
 def qcf_n_select(n_ctx: int, ratio: float) -> int:

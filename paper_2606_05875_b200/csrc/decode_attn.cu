@@ -13,6 +13,8 @@
 // Split partials (m, l, o) go to a workspace; the LAST CTA of a kv-head (arrival counter) merges them in split order
 // (bit-reproducible), normalises and stores bf16.
 #include <cmath>
+#include <mutex>
+#include <string>
 
 #include "qcf_internal.cuh"
 #include "sm100_ptx.cuh"
@@ -303,3 +305,115 @@ cudaError_t launch_decode_attn(const qcf_ctx* ctx, const __nv_bfloat16* q, const
 }
 
 }  // namespace qcf
+
+// ------------------------------------------------------------------------------------------------------------------------
+// qcf_decode_attn_static (include/qcf.h) — the same decode attention for callers that may not allocate device memory.
+//
+// qcf_decode_attn needs a qcf_ctx, and qcf_create cudaMallocs the split-KV workspace of the kernel above.  Some users of
+// this library are not in a position to do that: a plugin or custom op running inside a serving engine that has handed
+// all of HBM to its own pool allocator (a cudaMalloc from inside it fails or fragments the pool), code running under a
+// framework's "no allocation here" region (memory-planned or about-to-be-captured sections), and tools that must not
+// disturb the allocator state they observe.  For them the workspace below lives in the library image itself: a file-scope
+// __device__ array that every GPU which loads libqcf.so carries from module load until the process exits.
+//
+// Layout of the array (offsets are multiples of 256 B):
+//   [0, kStaticPartO)              split partial outputs   [Hkv][kDecodeSplitsMax][G][d] fp32
+//   [kStaticPartO, +kStaticPartMl) split (max, sum) pairs  [Hkv][kDecodeSplitsMax][G][2] fp32
+//   [.., +kStaticCounters)         per-kv-head arrival counters (must be zero when a launch starts)
+// Sized for Hq * d <= kStaticMaxHeadElems and Hkv <= kStaticMaxKvHeads: 2 MiB + 64 KiB + 256 B per GPU.
+namespace qcf {
+namespace {
+
+constexpr int kStaticMaxHeadElems = 8192;                       // Hq * d, e.g. 64 heads x 128
+constexpr int kStaticMaxKvHeads = 64;
+constexpr size_t kStaticPartO = static_cast<size_t>(kDecodeSplitsMax) * kStaticMaxHeadElems * sizeof(float);
+constexpr size_t kStaticPartMl = static_cast<size_t>(kDecodeSplitsMax) * (kStaticMaxHeadElems / 64) * 2 * sizeof(float);
+constexpr size_t kStaticCounters = 256;                         // kStaticMaxKvHeads x 4 B
+constexpr size_t kStaticBytes = kStaticPartO + kStaticPartMl + kStaticCounters;
+static_assert(kStaticPartO % 256 == 0 && kStaticPartMl % 256 == 0, "sub-buffers keep the array's 256-byte alignment");
+static_assert(kStaticMaxKvHeads * sizeof(unsigned int) <= kStaticCounters, "counter block too small");
+
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+// In host code `g_static_scratch` is only a handle for the runtime's symbol table, NOT a device address: the per-device
+// address comes from cudaGetSymbolAddress with that device current, once, and is remembered here.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDev {
+  bool ready;
+  unsigned char* base;      // device address of g_static_scratch on this device
+  int n_sm;
+};
+StaticDev g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;
+
+}  // namespace
+}  // namespace qcf
+
+qcf_status qcf_decode_attn_static(const qcf_layout* lay, const void* q, const void* k_cache, const void* v_cache, int32_t n_keys,
+                                  void* out, float* lse, void* stream) {
+  using namespace qcf;
+  auto bad = [](qcf_status st, const std::string& msg) { return set_error(nullptr, st, "qcf_decode_attn_static: " + msg); };
+  if (!lay) return bad(QCF_ERR_INVALID_ARG, "layout is NULL");
+  if (lay->n_q_heads < 1 || lay->n_kv_heads < 1 || lay->n_q_heads % lay->n_kv_heads != 0)
+    return bad(QCF_ERR_UNSUPPORTED, "n_kv_heads must divide n_q_heads");
+  if (lay->head_dim != 64 && lay->head_dim != 128) return bad(QCF_ERR_UNSUPPORTED, "head_dim must be 64 or 128");
+  const int g = lay->n_q_heads / lay->n_kv_heads;
+  if (!(g == 1 || g == 2 || g == 4 || g == 8 || g == 16)) return bad(QCF_ERR_UNSUPPORTED, "group size Hq/Hkv must be 1, 2, 4, 8 or 16");
+  if (static_cast<long long>(lay->n_q_heads) * lay->head_dim > kStaticMaxHeadElems || lay->n_kv_heads > kStaticMaxKvHeads)
+    return bad(QCF_ERR_WORKSPACE,
+               "layout exceeds the built-in workspace (Hq * head_dim <= " + std::to_string(kStaticMaxHeadElems) + ", Hkv <= " +
+                   std::to_string(kStaticMaxKvHeads) + "); use qcf_create + qcf_decode_attn for larger layers");
+  if (!(lay->softmax_scale >= 0.0f)) return bad(QCF_ERR_INVALID_ARG, "softmax_scale must be >= 0");
+  if (n_keys < 1) return bad(QCF_ERR_INVALID_ARG, "n_keys must be >= 1 (the token's own K/V row is part of the cache)");
+  if (!q || !k_cache || !v_cache || !out) return bad(QCF_ERR_INVALID_ARG, "NULL tensor pointer");
+  if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k_cache) | reinterpret_cast<uintptr_t>(v_cache) |
+       reinterpret_cast<uintptr_t>(out)) & 15u)
+    return bad(QCF_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
+
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return bad(QCF_ERR_UNSUPPORTED, std::string("no CUDA device: ") + cudaGetErrorString(e));
+  if (dev < 0 || dev >= kStaticMaxDevices) return bad(QCF_ERR_UNSUPPORTED, "device ordinal beyond " + std::to_string(kStaticMaxDevices - 1));
+  StaticDev sd;
+  {
+    // First call on this device: resolve the array's address THERE (the device is current) and read the SM count.
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDev& slot = g_static_dev[dev];
+    if (!slot.ready) {
+      int major = 0, n_sm = 0;
+      if ((e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev)) != cudaSuccess ||
+          (e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+        return bad(QCF_ERR_CUDA, std::string("cudaDeviceGetAttribute: ") + cudaGetErrorString(e));
+      if (major != 10) return bad(QCF_ERR_UNSUPPORTED, "this library is built for sm_100a only");
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_static_scratch);
+      if (e != cudaSuccess || !p)
+        return bad(QCF_ERR_CUDA, std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e));
+      slot.base = static_cast<unsigned char*>(p);
+      slot.n_sm = n_sm;
+      slot.ready = true;
+    }
+    sd = slot;
+  }
+
+  // The launcher above reads only these fields of a ctx; this one lives on the host stack and owns nothing.
+  qcf_ctx view{};
+  view.lay = Layout{lay->n_q_heads, lay->n_kv_heads, lay->head_dim, g, lay->rope_theta,
+                    lay->softmax_scale > 0.f ? lay->softmax_scale : 1.0f / std::sqrt(static_cast<float>(lay->head_dim))};
+  view.device = dev;
+  view.n_sm = sd.n_sm;
+  view.pdl = 0;                                                    // plain launch: ordered after the memset below
+  view.dec_part_o = reinterpret_cast<float*>(sd.base);
+  view.dec_part_ml = reinterpret_cast<float*>(sd.base + kStaticPartO);
+  view.dec_counters = reinterpret_cast<unsigned int*>(sd.base + kStaticPartO + kStaticPartMl);
+
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  // The array keeps whatever the previous call (of any thread, any layout) left.  The partials are fully rewritten before
+  // they are read; the arrival counters must start at zero, and a launch that died half-way would have left them dirty.
+  e = cudaMemsetAsync(view.dec_counters, 0, kStaticCounters, s);
+  if (e != cudaSuccess) return bad(QCF_ERR_CUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(e));
+  e = launch_decode_attn(&view, static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(k_cache),
+                         static_cast<const __nv_bfloat16*>(v_cache), n_keys, static_cast<__nv_bfloat16*>(out), lse, s);
+  if (e != cudaSuccess) return bad(QCF_ERR_CUDA, std::string("launch: ") + cudaGetErrorString(e));
+  return QCF_OK;
+}
