@@ -162,22 +162,35 @@ QCF_API qcf_status qcf_set_head_shards(qcf_ctx* ctx, int32_t n_shards);
 
 /* The same step with the score exchange FUSED into a2 instead of a collective call between two launches (SURVEY.md
  * section 8(f).4): every rank owns an exchange buffer of qcf_score_exchange_bytes(n_shards, slot_elems) bytes, laid out
- *     [64 x uint32 flags][n_shards slots x slot_elems fp32],     slot_elems >= B * n_stride of every batch used,
+ *     [64 x uint32 flags][64 x uint32 acks][2 slot sets x n_shards slots x slot_elems fp32],
+ *     slot_elems >= B * n_stride of every batch used,
  * and `peer_bufs[p]` (host array [n_shards]) is rank p's buffer AS MAPPED INTO THIS PROCESS (its own allocation for
  * p == rank; cudaIpcOpenMemHandle / peer access over NVLink for the others).  After this call, on this ctx:
- *   qcf_score        besides writing `scores` as before, the combine CTAs store this rank's (accumulated) partial
- *                    I_rank(t) straight into slot `rank` of EVERY rank's buffer (plain st.global on peer pointers), and a
- *                    one-thread tail kernel then publishes a monotonically increasing epoch in flag[rank] of every
- *                    buffer with a system-scope release — no NCCL call, no host involvement;
+ *   qcf_score        is epoch e (e counts this ctx's exchanging qcf_score calls from 1).  Besides writing `scores` as
+ *                    before, the combine CTAs store this rank's (accumulated) partial I_rank(t) straight into slot `rank`
+ *                    of slot set (e & 1) of EVERY rank's buffer (plain st.global on peer pointers), and a one-thread tail
+ *                    kernel then publishes e in flag[rank] of every buffer with a system-scope release — no NCCL call, no
+ *                    host involvement.  Before it starts, a one-warp head kernel waits until every peer has acknowledged
+ *                    the newest selection epoch <= e - 2 (see below);
  *   qcf_select_topk  waits (system-scope acquire, bounded: a missing peer traps after ~2 s instead of hanging) until all
- *                    n_shards flags of ITS OWN buffer have reached the current epoch, then ranks the element-wise sum
- *                    of the n_shards slots, added in slot order (every rank forms bit-identical sums and selects the
- *                    same P); its `scores` argument is ignored.
- * Ranks must issue the same sequence of exchanging qcf_score calls (the epoch counts them).  n_shards == 1 or
- * peer_bufs == NULL turns the exchange off.  Not CUDA-graph capturable (the epoch is a launch argument).
- * Unmeasured on > 1 GPU in this repository (one GPU per box); tested with two contexts on one GPU and with two
- * PROCESSES sharing one GPU through CUDA IPC handles, their phases ordered on the host so that no kernel ever spins on
- * a flag another process has yet to write. */
+ *                    n_shards flags of ITS OWN buffer have reached the current epoch e, then ranks the element-wise sum
+ *                    of the n_shards slots of slot set (e & 1), added in slot order (every rank forms bit-identical sums
+ *                    and selects the same P); its `scores` argument is ignored.  A one-thread tail kernel then publishes e
+ *                    in ack[rank] of every buffer: "this rank has finished reading epoch e".
+ * Protocol invariant (what makes back-to-back steps safe when ranks drift apart): a rank overwrites slot set (e & 1),
+ * last written at epoch e - 2, only after every peer has acknowledged the newest selection at an epoch <= e - 2 — so no
+ * selection that could still be reading that set is outstanding — while the selection of epoch e - 1, if a slower peer has
+ * yet to run it, reads the OTHER set.  A rank may therefore run up to one exchanging qcf_score ahead of its slowest peer's
+ * selection; further ahead it waits.  Flags and acks only ever increase.
+ * Rules for the caller: (1) the buffers are ZEROED before they are shared (qcf_set_score_exchange clears nothing: a faster
+ * peer may already have published into this rank's buffer); no rank issues an exchanging call before every rank's buffer
+ * is zeroed and mapped (sharded.share_exchange_buffers ends with a barrier).  (2) All ranks issue the same sequence of
+ * exchanging qcf_score / qcf_select_topk calls (the epoch counts the former).  (3) Selecting twice at the same epoch is
+ * allowed only while no rank has moved past the next epoch (only the first selection's ack is distinguishable).
+ * n_shards == 1 or peer_bufs == NULL turns the exchange off.  Not CUDA-graph capturable (the epoch is a launch argument).
+ * Unmeasured on > 1 GPU in this repository (one GPU per box); tested with two contexts on one GPU — including one rank
+ * running a whole step ahead of the other's selection — and with two PROCESSES sharing one GPU through CUDA IPC handles,
+ * their phases ordered on the host so that no kernel ever spins on a flag another process has yet to write. */
 QCF_API int64_t qcf_score_exchange_bytes(int32_t n_shards, int64_t slot_elems);
 QCF_API qcf_status qcf_set_score_exchange(qcf_ctx* ctx, int32_t rank, int32_t n_shards, void* const* peer_bufs,
                                           int64_t slot_elems);

@@ -134,6 +134,7 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->q_gather_src = nullptr; c->q_gather_dst = nullptr;
   c->pdl = 1; c->gemm_mt = 0; c->attn_cluster = 0;
   c->exch_rank = 0; c->exch_world = 1; c->exch_slot_elems = 0; c->exch_peers = nullptr; c->exch_epoch = 0;
+  c->exch_sel_epoch[0] = c->exch_sel_epoch[1] = 0;
   c->ratio_hint = 0.3;
   c->head_shards = 1;
   c->profiling = 0; c->ev_valid = false;
@@ -365,15 +366,24 @@ qcf_status qcf_score(qcf_ctx* ctx, const qcf_batch* b, const void* q_probe, cons
   QCF_REQUIRE(ctx, k_fused && scores, "qcf_score: NULL tensor pointer");
   QCF_REQUIRE(ctx, q_probe || b->q_stride == 0, "qcf_score: q_probe is NULL");
   QCF_REQUIRE(ctx, aligned16(q_probe) && aligned16(k_fused), "qcf_score: pointers must be 16-byte aligned");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (ctx->exch_world > 1) {
     QCF_REQUIRE(ctx, static_cast<long long>(b->batch) * b->n_stride <= ctx->exch_slot_elems,
                 "qcf_score: the batch does not fit a slot of the score exchange buffers");
-    ctx->exch_epoch++;
+    // This call is epoch e = exch_epoch + 1 and overwrites the slot set of epoch e - 2.  Every peer must have finished the
+    // selections that read it: the newest selection epoch <= e - 2 of the (common) call sequence must be acknowledged.
+    const unsigned int e = ctx->exch_epoch + 1;
+    const unsigned int need = ctx->exch_sel_epoch[0] + 2 <= e ? ctx->exch_sel_epoch[0] : ctx->exch_sel_epoch[1];
+    if (need > 0) QCF_CUDA(ctx, launch_exchange_wait(ctx, need, s));
+    ctx->exch_epoch = e;                       // read by the two launches below; taken back if either fails
   }
-  QCF_CUDA(ctx, launch_score(ctx, b, static_cast<const __nv_bfloat16*>(q_probe),
-                             static_cast<const __nv_bfloat16*>(k_fused), scores, accumulate != 0,
-                             static_cast<cudaStream_t>(stream)));
-  if (ctx->exch_world > 1) QCF_CUDA(ctx, launch_exchange_flags(ctx, static_cast<cudaStream_t>(stream)));
+  cudaError_t err = launch_score(ctx, b, static_cast<const __nv_bfloat16*>(q_probe), static_cast<const __nv_bfloat16*>(k_fused),
+                                 scores, accumulate != 0, s);
+  if (err == cudaSuccess && ctx->exch_world > 1) err = launch_exchange_flags(ctx, s);
+  if (err != cudaSuccess) {
+    if (ctx->exch_world > 1) ctx->exch_epoch--;
+    return cuda_fail(ctx, err, "qcf_score");
+  }
   return QCF_OK;
 }
 
@@ -386,6 +396,14 @@ qcf_status qcf_select_topk(qcf_ctx* ctx, const qcf_batch* b, const float* scores
   QCF_REQUIRE(ctx, ((scores || ctx->exch_world > 1) && sel) || b->n_stride == 0, "qcf_select_topk: NULL tensor pointer");
   ctx->ratio_hint = ratio;
   QCF_CUDA(ctx, launch_topk(ctx, b, scores, ratio, sel, n_sel, static_cast<cudaStream_t>(stream)));
+  if (ctx->exch_world > 1) {
+    // tell the peers that this rank is done reading the slots of this epoch (they may overwrite them two epochs on)
+    QCF_CUDA(ctx, launch_exchange_ack(ctx, static_cast<cudaStream_t>(stream)));
+    if (ctx->exch_sel_epoch[0] != ctx->exch_epoch) {
+      ctx->exch_sel_epoch[1] = ctx->exch_sel_epoch[0];
+      ctx->exch_sel_epoch[0] = ctx->exch_epoch;
+    }
+  }
   return QCF_OK;
 }
 
@@ -525,7 +543,7 @@ qcf_status qcf_debug_set(qcf_ctx* ctx, int32_t knob, int32_t value) {
 
 int64_t qcf_score_exchange_bytes(int32_t n_shards, int64_t slot_elems) {
   if (n_shards < 1 || n_shards > 64 || slot_elems < 0) return -1;
-  return static_cast<int64_t>(kExchHeaderElems) * 4 + static_cast<int64_t>(n_shards) * slot_elems * 4;
+  return static_cast<int64_t>(kExchHeaderElems) * 4 + 2 * static_cast<int64_t>(n_shards) * slot_elems * 4;
 }
 
 qcf_status qcf_set_score_exchange(qcf_ctx* ctx, int32_t rank, int32_t n_shards, void* const* peer_bufs, int64_t slot_elems) {
@@ -542,9 +560,10 @@ qcf_status qcf_set_score_exchange(qcf_ctx* ctx, int32_t rank, int32_t n_shards, 
   for (int p = 0; p < 64; ++p) ctx->exch_peers_host[p] = p < n_shards ? static_cast<float*>(peer_bufs[p]) : nullptr;
   QCF_CUDA(ctx, cudaMemcpy(ctx->exch_peers, ctx->exch_peers_host, 64 * sizeof(float*), cudaMemcpyHostToDevice));
   ctx->exch_rank = rank; ctx->exch_world = n_shards; ctx->exch_slot_elems = slot_elems;
+  // Epochs count from 1 and the caller hands over ZEROED buffers: nothing is cleared here, because a faster peer may
+  // already have published its first epoch into this rank's buffer by the time this rank gets to this call.
   ctx->exch_epoch = 0;
-  // flags of the own buffer start at 0 (epochs count from 1)
-  QCF_CUDA(ctx, cudaMemset(peer_bufs[rank], 0, kExchHeaderElems * 4));
+  ctx->exch_sel_epoch[0] = ctx->exch_sel_epoch[1] = 0;
   return QCF_OK;
 }
 

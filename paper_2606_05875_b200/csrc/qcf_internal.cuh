@@ -71,6 +71,7 @@ struct qcf_ctx {
   float* exch_peers_host[64];
   float** exch_peers;          // device copy
   unsigned int exch_epoch;     // incremented by every exchanging qcf_score; the flag value peers wait for
+  unsigned int exch_sel_epoch[2];  // the two most recent distinct epochs an exchanging qcf_select_topk ran at ([0] newest)
   // workspace (device)
   float* stats_m;        // score pass-1 partial row max      [max_batch][Hq*max_query][kScoreSplits]
   float* stats_l;        // score pass-1 partial row sum-exp
@@ -131,9 +132,18 @@ cudaError_t launch_score(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* 
                          float* scores, int accumulate, cudaStream_t);
 cudaError_t launch_topk(const qcf_ctx*, const qcf_batch*, const float* scores, double ratio, int32_t* sel,
                         int32_t* n_sel, cudaStream_t, int ceil_mode = 0);
+// Exchange buffer of a rank (include/qcf.h, qcf_set_score_exchange):
+//   words [0, 64)    flag[p]: newest epoch whose scores rank p has stored into THIS buffer     (written by p's a2 tail)
+//   words [64, 128)  ack[p] : newest epoch at which rank p has finished a selection (a3)      (written by p's a3 tail)
+//   then 2 slot sets (epoch parity) x n_shards slots x slot_elems fp32
+constexpr int kExchHeaderElems = 128;
+constexpr int kExchAckOffset = 64;
 // after a2 on an exchanging ctx: publish `epoch` in flag[rank] of every peer's exchange buffer (system-scope release)
 cudaError_t launch_exchange_flags(const qcf_ctx*, cudaStream_t);
-constexpr int kExchHeaderElems = 64;   // 64 x 4 B of flags in front of the slots of an exchange buffer
+// before a2: wait until every peer's ack in this rank's own buffer has reached `need` (bounded spin, then trap)
+cudaError_t launch_exchange_wait(const qcf_ctx*, unsigned int need, cudaStream_t);
+// after a3: publish `epoch` in ack[rank] of every peer's exchange buffer (system-scope release)
+cudaError_t launch_exchange_ack(const qcf_ctx*, cudaStream_t);
 // G_i(r) of Eq. 14 for every chunk row of the batch (rule 0: sink, 1: knorm) into scores[B][n_stride]
 cudaError_t launch_anchor_scores(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool, int rule, int accumulate,
                                  float* scores, cudaStream_t);

@@ -66,7 +66,8 @@ struct ScoreArgs {
   unsigned int* counters;
   float* scores; int accumulate;
   // fused exchange of the KV-head-sharded step: the combined value also goes to slot exch_rank of every rank's buffer
-  float* const* exch_peers; int exch_rank, exch_world; long long exch_slot_elems;
+  // (slot set exch_parity = epoch & 1: the other set still holds the previous epoch, which a slower peer may be ranking)
+  float* const* exch_peers; int exch_rank, exch_world, exch_parity; long long exch_slot_elems;
 };
 
 template <int D, int PASS>
@@ -406,7 +407,8 @@ score_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
           *dst = nv;
           if (a.exch_world > 1) {
             // this rank's partial of Eq. 18, straight into every rank's exchange buffer (peer memory: NVLink / IPC)
-            const size_t off = kExchHeaderElems + static_cast<size_t>(a.exch_rank) * a.exch_slot_elems + static_cast<size_t>(b) * bd.n_stride + key;
+            const size_t off = kExchHeaderElems + static_cast<size_t>(a.exch_parity * a.exch_world + a.exch_rank) * a.exch_slot_elems +
+                               static_cast<size_t>(b) * bd.n_stride + key;
             for (int p = 0; p < a.exch_world; ++p) a.exch_peers[p][off] = nv;
           }
         }
@@ -480,10 +482,43 @@ __global__ void exchange_flag_kernel(float* const* peers, int rank, int world, u
   }
 }
 
+// The reader's half of the protocol.  ack: one thread behind a3 on the same stream — every slot read of this rank's
+// selection at `epoch` has been performed; tell every peer.  wait: one thread per peer in front of a2 — this rank is about
+// to overwrite the slot set it last wrote two epochs ago, so every peer must have finished the selections that read it.
+__global__ void exchange_ack_kernel(float* const* peers, int rank, int world, unsigned int epoch) {
+  __threadfence_system();
+  for (int p = 0; p < world; ++p) {
+    unsigned int* ack = reinterpret_cast<unsigned int*>(peers[p]) + kExchAckOffset + rank;
+    asm volatile("st.release.sys.global.u32 [%0], %1;" ::"l"(ack), "r"(epoch) : "memory");
+  }
+}
+
+__global__ void exchange_wait_kernel(const float* own, int world, unsigned int need) {
+  if (static_cast<int>(threadIdx.x) >= world) return;
+  const unsigned int* ack = reinterpret_cast<const unsigned int*>(own) + kExchAckOffset + threadIdx.x;
+  const long long t0 = clock64();
+  unsigned int v;
+  do {
+    asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(ack) : "memory");
+    if (static_cast<int>(v - need) >= 0) break;
+    if (clock64() - t0 > 4000000000LL) __trap();                  // a peer that never selects is a trap, not a hang
+  } while (true);
+}
+
 }  // namespace
 
 cudaError_t launch_exchange_flags(const qcf_ctx* ctx, cudaStream_t stream) {
   exchange_flag_kernel<<<1, 1, 0, stream>>>(ctx->exch_peers, ctx->exch_rank, ctx->exch_world, ctx->exch_epoch);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_exchange_ack(const qcf_ctx* ctx, cudaStream_t stream) {
+  exchange_ack_kernel<<<1, 1, 0, stream>>>(ctx->exch_peers, ctx->exch_rank, ctx->exch_world, ctx->exch_epoch);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_exchange_wait(const qcf_ctx* ctx, unsigned int need, cudaStream_t stream) {
+  exchange_wait_kernel<<<1, 64, 0, stream>>>(ctx->exch_peers_host[ctx->exch_rank], ctx->exch_world, need);
   return cudaGetLastError();
 }
 
@@ -548,6 +583,7 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
   a.counters = ctx->counters;
   a.scores = scores; a.accumulate = accumulate;
   a.exch_peers = ctx->exch_peers; a.exch_rank = ctx->exch_rank; a.exch_world = ctx->exch_world; a.exch_slot_elems = ctx->exch_slot_elems;
+  a.exch_parity = static_cast<int>(ctx->exch_epoch & 1u);
   return L.d == 128 ? launch<128>(ctx, b, tm_q, tm_k, a, row_tiles, key_tiles, stream)
                     : launch<64>(ctx, b, tm_q, tm_k, a, row_tiles, key_tiles, stream);
 }

@@ -23,7 +23,8 @@ __device__ __forceinline__ uint32_t order_key(float f) {
 // order, of `world` slots of this rank's exchange buffer, each written by one rank's a2; flag[p] >= epoch says rank p's
 // slot is complete.
 struct Exch {
-  const float* buf;        // nullptr: plain scores
+  const float* buf;        // nullptr: plain scores; else this rank's exchange buffer (flags in front)
+  const float* slots;      // slot 0 of the slot set of this epoch's parity
   int world;
   long long slot_elems;
   unsigned int epoch;
@@ -66,7 +67,7 @@ __global__ void __launch_bounds__(kThreads) topk_kernel(BatchDev bd, const float
   // score of position i: plain, or the slot sum in fixed order
   auto score_at = [&](int i) -> float {
     if (!EXCH) return __ldcg(s + i);
-    const float* p = ex.buf + kExchHeaderElems + static_cast<size_t>(b) * bd.n_stride + i;
+    const float* p = ex.slots + static_cast<size_t>(b) * bd.n_stride + i;
     float acc = __ldcg(p);
     for (int q = 1; q < ex.world; ++q) acc += __ldcg(p + static_cast<size_t>(q) * ex.slot_elems);
     return acc;
@@ -181,12 +182,13 @@ cudaError_t launch_topk(const qcf_ctx* ctx, const qcf_batch* b, const float* sco
   // per device / context, so set on every launch (as the other launchers do) rather than once per process
   cudaFuncSetAttribute(topk_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
   cudaFuncSetAttribute(topk_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 49152 * 4);
-  Exch ex{nullptr, 1, 0, 0u};
+  Exch ex{nullptr, nullptr, 1, 0, 0u};
   if (ctx->exch_world > 1 && !ceil_mode) {     // (the anchor ranking of Phase I is never sharded)
     ex.buf = ctx->exch_peers_host[ctx->exch_rank];
     ex.world = ctx->exch_world;
     ex.slot_elems = ctx->exch_slot_elems;
     ex.epoch = ctx->exch_epoch;
+    ex.slots = ex.buf + kExchHeaderElems + static_cast<size_t>(ex.epoch & 1u) * ex.world * ex.slot_elems;
     return launch_pdl(ctx->pdl, topk_kernel<true>, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode, ex);
   }
   return launch_pdl(ctx->pdl, topk_kernel<false>, dim3(b->batch), dim3(kThreads), smem, stream, b->dev, scores, ratio, sel, n_sel, n_cached, ceil_mode, ex);

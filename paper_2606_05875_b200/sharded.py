@@ -57,6 +57,7 @@ def share_exchange_buffers(mine, rank: int, world: int, group=None):
     if world == 1:
         return [mine]
     import torch
+    torch.cuda.synchronize(mine.device)       # the zero fill of `mine` has run before any peer can store into it
     handles = [None] * world
     dist.all_gather_object(handles, (mine.device.index, reduce_tensor(mine)), group=group)
     peers = []
@@ -74,6 +75,8 @@ def share_exchange_buffers(mine, rank: int, world: int, group=None):
             if int(err) not in (0, 704):                      # 704: cudaErrorPeerAccessAlreadyEnabled
                 raise RuntimeError("cudaDeviceEnablePeerAccess(%d) failed: %s" % (dev_p, err))
         peers.append(fn(*args))
+    # nobody starts an exchanging call before every rank holds every mapping (include/qcf.h, rule (1))
+    dist.barrier(group=group)
     return peers
 
 
@@ -95,7 +98,8 @@ class HeadShardedStep:
     # ---- fused exchange (include/qcf.h, qcf_set_score_exchange)
     @staticmethod
     def alloc_exchange_buffer(world: int, slot_elems: int, device="cuda"):
-        """This rank's exchange buffer: [64 flags][world slots x slot_elems] fp32, zeroed.  Share it with the peers
+        """This rank's exchange buffer: [64 flags][64 acks][2 slot sets x world slots x slot_elems] fp32, zeroed (the
+        library requires that and clears nothing itself).  Share it with the peers
         (same process: pass the tensor; other processes: send it through torch.multiprocessing, which maps it with CUDA
         IPC; other GPUs: enable peer access and pass the pointer)."""
         import torch
@@ -109,13 +113,15 @@ class HeadShardedStep:
         self.fused = self.world > 1
         self._exch = list(peer_bufs)
         self.slot_elems = int(slot_elems)
+        self._epoch = 0                                # mirrors the ctx's count of exchanging qcf_score calls
         if self.fused:
             self.ctx.qcf_set_score_exchange(self.rank, self.world, self._exch, slot_elems)
 
     def exchanged_scores(self, b: binding.Batch):
         """The summed scores [B][n_stride] this rank's a3 ranks (slot order), for inspection."""
         buf = self._exch[self.rank]
-        slots = buf[64: 64 + self.world * self.slot_elems].view(self.world, self.slot_elems)[:, : b.batch * b.n_stride]
+        first = 128 + (self._epoch & 1) * self.world * self.slot_elems      # slot set of the newest epoch's parity
+        slots = buf[first: first + self.world * self.slot_elems].view(self.world, self.slot_elems)[:, : b.batch * b.n_stride]
         acc = slots[0].clone()
         for p in range(1, self.world):
             acc += slots[p]
@@ -133,6 +139,8 @@ class HeadShardedStep:
         self.ctx.qcf_rope_reposition(b, k_pool, v_pool, k_fused, v_fused, stream)
         if is_critical_layer:
             self.ctx.qcf_score(b, q_probe, k_fused, scores, accumulate, stream)
+            if self.fused and b.total_ctx > 0:
+                self._epoch += 1
 
     def fuse_phase(self, b: binding.Batch, *, scores, sel, n_sel, q_new, k_new, v_new, k_fused, v_fused, out, lse=None,
                    ratio: float = 0.0, rows_by_position: bool = True, select_now: bool = True, stream=None):

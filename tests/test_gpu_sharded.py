@@ -128,6 +128,75 @@ def test_head_sharded_step_matches_unsharded_oracle(name, world, exchange):
             assert torch.equal(sel_again[b, :kb], dws[0].sel[b, :kb])
 
 
+def _swap_probe(wl):
+    """Same requests with ANOTHER probe: the query rows of q_new stand in for q_probe (same shape, same positions)."""
+    import copy
+    wl2 = copy.copy(wl)
+    wl2.requests = [copy.copy(r) for r in wl.requests]
+    for r in wl2.requests:
+        r.q_probe = np.ascontiguousarray(r.q_new[r.n_ctx: r.n_ctx + r.n_query])
+    return wl2
+
+
+@pytest.mark.parametrize("name", ["t_mid", "t_batch"])
+def test_fused_exchange_rank_running_a_step_ahead(name):
+    """The write-after-read case of the fused exchange (include/qcf.h, protocol invariant): rank A runs a1 + a2 of step i AND
+    of step i + 1 (another probe, so other scores) before rank B has run a3 of step i.  With one slot per rank, A's second a2
+    would overwrite what B is about to rank and the ranks would silently select different P.  With the slot sets indexed by
+    epoch parity B still ranks step i's scores: B's P_i equals A's P_i and the oracle's on step-i inputs; both ranks then
+    select the same P_{i+1}, the oracle's on step-(i+1) inputs.  A third step makes A's a2 pass the acknowledgement wait."""
+    _, device, sharded = _mods()
+    wl = inputs.make_workload(name)
+    wl2 = _swap_probe(wl)
+    cfg = wl.cfg
+    world = 2
+    steps, dws = _ranks(wl, world)
+    dws2 = [device.DeviceWorkload(inputs.shard_heads(wl2, rank, world), st.ctx) for rank, st in enumerate(steps)]
+    slot = dws[0].batch.batch * dws[0].batch.n_stride
+    bufs = [sharded.HeadShardedStep.alloc_exchange_buffer(world, slot) for _ in range(world)]
+    for st in steps:
+        st.enable_fused_exchange(bufs, slot)
+    A, B = 0, 1
+
+    def score(rank, dw):
+        steps[rank].score_phase(dw.batch, k_pool=dw.k_pool, v_pool=dw.v_pool, k_fused=dw.k_fused, v_fused=dw.v_fused,
+                                q_probe=dw.q_probe, scores=dw.scores)
+
+    def select(rank, dw):
+        steps[rank].ctx.qcf_select_topk(dw.batch, None, cfg.ratio, dw.sel, dw.n_sel)
+
+    score(A, dws[A]); score(B, dws[B])                 # step i on both ranks
+    select(A, dws[A])                                  # A: a3 of step i ...
+    score(A, dws2[A])                                  # ... and already a1 + a2 of step i + 1 (B has not selected yet)
+    select(B, dws[B])                                  # B: a3 of step i — must still see step i's scores
+    score(B, dws2[B])
+    select(A, dws2[A]); select(B, dws2[B])             # step i + 1 on both
+    score(A, dws[A])                                   # step i + 2: A's a2 waits for B's ack of step i (already there)
+    score(B, dws[B])
+    sel3 = torch.zeros_like(dws[A].sel)
+    n3 = torch.zeros_like(dws[A].n_sel)
+    steps[A].ctx.qcf_select_topk(dws[A].batch, None, cfg.ratio, sel3, n3)
+    torch.cuda.synchronize()
+    for step_wl, step_dws in ((wl, dws), (wl2, dws2)):
+        for b, r in enumerate(step_wl.requests):
+            k_pic = [O.widen_bf16(step_wl.pool_k[i]) for i in r.chunk_ids]
+            ref = O.layer_step(k_pic, [O.widen_bf16(step_wl.pool_v[i]) for i in r.chunk_ids], cfg.rope_theta,
+                               O.widen_bf16(r.q_probe), cfg.ratio, O.widen_bf16(r.q_new), O.widen_bf16(r.k_new),
+                               O.widen_bf16(r.v_new))
+            k = int(step_dws[A].n_sel[b])
+            assert k == len(ref["sel"]) and int(step_dws[B].n_sel[b]) == k
+            sel_a = step_dws[A].sel[b, :k].cpu().numpy().astype(np.int64)
+            assert np.array_equal(step_dws[B].sel[b, :k].cpu().numpy(), sel_a), "the ranks selected different P"
+            _check_selection(sel_a, ref["scores"], k)
+    # the two probes really rank differently (else the test would pass with the hazard in place)
+    assert any(not torch.equal(dws[A].sel[b, : int(dws[A].n_sel[b])], dws2[A].sel[b, : int(dws2[A].n_sel[b])])
+               for b in range(dws[A].B))
+    # step i + 2 repeats step i's inputs: same selection
+    for b in range(dws[A].B):
+        kb = int(n3[b])
+        assert kb == int(dws[A].n_sel[b]) and torch.equal(sel3[b, :kb], dws[A].sel[b, :kb])
+
+
 def test_head_sharded_full_size_c2_matches_the_unsharded_step():
     """BASELINE configs[1] at full size, two shards, against the UNSHARDED CUDA step on the same inputs (itself checked
     against the oracle in tests/test_gpu_parity.py): the summed partial scores agree to fp32 rounding, the selection is

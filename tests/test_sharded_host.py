@@ -69,11 +69,11 @@ def test_score_all_reduce_two_gloo_ranks():
 
 
 def test_score_exchange_buffer_size_is_header_plus_slots():
-    """include/qcf.h, qcf_score_exchange_bytes: 64 uint32 flags in front of n_shards slots of slot_elems fp32 (pure host
-    arithmetic of the C ABI, callable without a GPU)."""
+    """include/qcf.h, qcf_score_exchange_bytes: 64 uint32 flags + 64 uint32 acks in front of TWO slot sets (epoch parity)
+    of n_shards slots of slot_elems fp32 (pure host arithmetic, no device needed)."""
     from paper_2606_05875_b200 import binding
-    assert binding.qcf_score_exchange_bytes(2, 1000) == 64 * 4 + 2 * 1000 * 4
-    assert binding.qcf_score_exchange_bytes(8, 16 * 8192) == 256 + 8 * 16 * 8192 * 4
+    assert binding.qcf_score_exchange_bytes(2, 1000) == 128 * 4 + 2 * 2 * 1000 * 4
+    assert binding.qcf_score_exchange_bytes(8, 16 * 8192) == 512 + 2 * 8 * 16 * 8192 * 4
     assert binding.qcf_score_exchange_bytes(0, 10) == -1 and binding.qcf_score_exchange_bytes(65, 10) == -1
     assert binding.qcf_score_exchange_bytes(2, -1) == -1
 
