@@ -286,17 +286,17 @@ typedef struct {
  * chained on `stream` with no host synchronisation. */
 QCF_API qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* args, void* stream);
 
-/* pool_rows: rows of host->k_pool / v_pool; every chunk of the batch must lie inside them (QCF_ERR_INVALID_ARG otherwise).
- * Only the pool rows some request of the batch reads are uploaded (qcf_batch_info.pool_rows_touched rows per tensor).
- * With rows_by_position != 0 and q_new / k_new / v_new in pinned, device-mapped host memory (cudaHostAlloc,
- * cudaHostRegister, torch.pin_memory) those three buffers are not uploaded at all: the a4 and a5 kernels read the |R_b| rows
- * they need straight from host memory (zero-copy gather; P is only known on the device after a3).  Pageable buffers are
- * staged through a full upload as before.
- * Same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe
- * and fresh rows, runs qcf_layer_step on the context's internal device buffers, downloads the |R_b| written rows of `out`, `sel`,
- * `n_sel` (and the fused cache if k_fused / v_fused are non-NULL), and synchronises `stream` before
- * returning.  Pointer fields of `host` are host pointers with the same shapes; `pool_rows` is the number of
- * rows of host->k_pool / v_pool.  Device staging buffers are allocated on first use and kept by the ctx. */
+/* The same step with every tensor in HOST memory (pinned memory recommended): uploads the PIC pool rows, probe and fresh
+ * rows, runs qcf_layer_step on the context's internal device buffers, downloads the |R_b| written rows of `out`, `sel`,
+ * `n_sel` (and the fused cache if k_fused / v_fused are non-NULL), and synchronises `stream` before returning.  Pointer
+ * fields of `host` are host pointers with the same shapes.  Device staging buffers are allocated on first use and kept
+ * by the ctx.
+ *   pool_rows: rows of host->k_pool / v_pool; every chunk of the batch must lie inside them (QCF_ERR_INVALID_ARG otherwise).
+ *   Only the pool rows some request of the batch reads are uploaded (qcf_batch_info.pool_rows_touched rows per tensor).
+ *   With rows_by_position != 0 and q_new / k_new / v_new in pinned, device-mapped host memory (cudaHostAlloc,
+ *   cudaHostRegister, torch.pin_memory) those three buffers are not uploaded at all: the a4 and a5 kernels read the |R_b|
+ *   rows they need straight from host memory (zero-copy gather; P is only known on the device after a3).  Pageable
+ *   buffers are staged through a full upload. */
 QCF_API qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* host,
                                        int64_t pool_rows, void* stream);
 
@@ -326,7 +326,12 @@ QCF_API qcf_status qcf_debug_set(qcf_ctx* ctx, int32_t knob, int32_t value);
  *            QCF_EPI_ADD_RESIDUAL : c = residual + acc   (residual [M][N] bf16; residual == c allowed)
  *            QCF_EPI_SWIGLU       : w holds (gate_j, up_j) rows INTERLEAVED (row 2j = W_g[j], 2j+1 = W_u[j]);
  *                                   c[M][N/2] = silu(acc[2j]) * acc[2j+1]
- * All dev pointers 16-byte aligned; K % 8 == 0, N % 8 == 0 (N % 16 == 0 for SWIGLU).  M, N, K tails are handled. */
+ * All dev pointers 16-byte aligned; K % 8 == 0, N % 8 == 0 (N % 16 == 0 for SWIGLU).  M, N, K tails are handled.
+ * Not invariant to M in the last bit: M == 1 (a decoding row) runs a weight-streaming GEMV whose fp32 sums are formed in
+ * another order than the tensor-core tiles used for M > 1, so one row computed alone and the same row inside a larger batch
+ * can differ by one bf16 rounding (both are within the stated tolerance of the exact product).  Likewise the decode path
+ * folds RMSNorm into the GEMV prologue ((x * inv_rms) * gain rounded to bf16 once, the same expression as the prefill's
+ * RMSNorm kernel); decode == last row of a one-token-longer prefill holds within the free-running bound, not bit for bit. */
 typedef enum { QCF_EPI_STORE = 0, QCF_EPI_ADD_RESIDUAL = 1, QCF_EPI_SWIGLU = 2 } qcf_epilogue;
 QCF_API qcf_status qcf_linear(qcf_ctx* ctx, const void* a, const void* w, const void* residual, void* c, int32_t M,
                               int32_t N, int32_t K, int32_t epilogue, void* stream);
@@ -432,6 +437,8 @@ QCF_API qcf_status qcf_decode_attn_static(const qcf_layout* layout, const void* 
  *   token_in : dev int32 [1];  pos0 = rows already in every cache (N + Lq after qcf_stack_fuse / qcf_stack_prefill)
  *   k_cache, v_cache : host arrays [L] of dev [>= pos0 + n_new][Hkv][d] — the caches qcf_stack_fuse filled (KV^Fuse), with
  *                      room for the appended rows;  pos0 + n_new <= max_pos of qcf_stack_create
+ *   Limits: hidden, ffn and Hq * head_dim <= 115712 (the row a GEMV multiplies is staged whole in shared memory), else
+ *   QCF_ERR_UNSUPPORTED; Hq / Hkv in {1,2,4,8,16} as for every ctx.
  *   logits : dev [n_new][vocab] fp32;  tokens_out : dev int32 [n_new]
  * Launch-only on `stream` (token ids never return to the host between steps). */
 QCF_API qcf_status qcf_stack_decode(qcf_stack* s, const int32_t* token_in, int32_t pos0, int32_t n_new,

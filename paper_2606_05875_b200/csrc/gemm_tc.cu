@@ -277,7 +277,7 @@ cudaError_t launch_gemm(const qcf_ctx* ctx, const __nv_bfloat16* a, const __nv_b
                         cudaStream_t stream) {
   if (M <= 0 || N <= 0) return cudaSuccess;
   // one row (decoding): a pure weight stream — the warp-per-row GEMV, not a 128-row MMA tile with 127 zero rows
-  if (M == 1 && ctx->gemm_mt == 0 && N % 2 == 0 && K % 8 == 0 && K <= 48 * 1024)
+  if (M == 1 && ctx->gemm_mt == 0 && N % 2 == 0 && K % 8 == 0 && K <= kGemvMaxK)
     return launch_gemv(ctx, a, w, nullptr, 0.f, residual, c, N, K, epilogue, stream);
   // Skinny problems (one row block: the 64-row probe GEMMs of stage 1) stream 34-200 MB of weights and are bound by how
   // many SMs pull them: 128 x 64 tiles give 4x the CTAs of 128 x 256 tiles and an 8-deep ring keeps ~100 KB in flight per SM.

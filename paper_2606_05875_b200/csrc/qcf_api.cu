@@ -131,7 +131,6 @@ qcf_status qcf_create(qcf_ctx** out, const qcf_layout* lay, int32_t max_batch, i
   c->counters = nullptr;
   c->dec_part_o = c->dec_part_ml = nullptr; c->dec_counters = nullptr;
   c->stage = nullptr;
-  c->q_gather_src = nullptr; c->q_gather_dst = nullptr;
   c->pdl = 1; c->gemm_mt = 0; c->attn_cluster = 0;
   c->exch_rank = 0; c->exch_world = 1; c->exch_slot_elems = 0; c->exch_peers = nullptr; c->exch_epoch = 0;
   c->exch_sel_epoch[0] = c->exch_sel_epoch[1] = 0;
@@ -262,10 +261,12 @@ qcf_status qcf_batch_create(qcf_ctx* ctx, const qcf_request* reqs, int32_t batch
     qb->n_pool_iv = static_cast<int32_t>(flat.size() / 2);
     qb->pool_rows_touched = touched;
     qb->h_pool_iv = static_cast<int64_t*>(std::malloc(sizeof(int64_t) * (flat.empty() ? 1 : flat.size())));
+    if (!qb->h_pool_iv) { qcf_batch_destroy(qb); return fail(ctx, QCF_ERR_WORKSPACE, "qcf_batch_create: out of host memory"); }
     if (!flat.empty()) std::memcpy(qb->h_pool_iv, flat.data(), sizeof(int64_t) * flat.size());
   }
   qb->h_n_ctx = static_cast<int32_t*>(std::malloc(sizeof(int32_t) * (batch > 0 ? batch : 1)));
   qb->h_n_query = static_cast<int32_t*>(std::malloc(sizeof(int32_t) * (batch > 0 ? batch : 1)));
+  if (!qb->h_n_ctx || !qb->h_n_query) { qcf_batch_destroy(qb); return fail(ctx, QCF_ERR_WORKSPACE, "qcf_batch_create: out of host memory"); }
   if (batch > 0) {
     std::memcpy(qb->h_n_ctx, n_ctx.data(), sizeof(int32_t) * batch);
     std::memcpy(qb->h_n_query, n_query.data(), sizeof(int32_t) * batch);
@@ -426,9 +427,14 @@ qcf_status qcf_anchor_rank(qcf_ctx* ctx, const qcf_batch* b, const void* k_pool,
   return QCF_OK;
 }
 
-qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
-                              const void* q_new, const void* k_new, const void* v_new, int32_t rows_by_position,
-                              void* k_fused, void* v_fused, void* out, float* lse, void* stream) {
+namespace {
+
+// a4 + a5.  q_gather_src != nullptr (the zero-copy host step only): q_new is position-indexed in device-mapped HOST memory;
+// its rows R are first gathered into the compact device buffer q_gather_dst, which a5 then reads.
+qcf_status recompute_attn_impl(qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                               const void* q_new, const void* k_new, const void* v_new, int32_t rows_by_position,
+                               void* k_fused, void* v_fused, void* out, float* lse, const void* q_gather_src,
+                               void* q_gather_dst, void* stream) {
   if (qcf_status st = check_ctx_batch(ctx, b)) return st;
   if (b->batch == 0 || b->t_stride == 0) return QCF_OK;
   QCF_REQUIRE(ctx, n_sel != nullptr, "qcf_recompute_attn: n_sel is NULL");
@@ -444,12 +450,11 @@ qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
                                static_cast<const __nv_bfloat16*>(v_new), rows_by_position != 0,
                                static_cast<__nv_bfloat16*>(k_fused), static_cast<__nv_bfloat16*>(v_fused), s));
   int q_by_position = rows_by_position != 0;
-  if (ctx->q_gather_src) {
+  if (q_gather_src) {
     // zero-copy host step: the rows R of the host-resident q_new are gathered (bulk copies over PCIe) into a compact device
     // buffer; a5 then reads q compactly while a4 above read k_new / v_new by position
-    QCF_CUDA(ctx, launch_gather_rows(ctx, b, sel_nn, n_sel, ctx->q_gather_src, ctx->q_gather_dst,
-                                     ctx->lay.hq * ctx->lay.d * 2, s));
-    q_new = ctx->q_gather_dst;
+    QCF_CUDA(ctx, launch_gather_rows(ctx, b, sel_nn, n_sel, q_gather_src, q_gather_dst, ctx->lay.hq * ctx->lay.d * 2, s));
+    q_new = q_gather_dst;
     q_by_position = 0;
   }
   if (ctx->profiling && ctx->ev_valid) cudaEventRecord(ctx->ev[4], s);
@@ -457,6 +462,15 @@ qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* s
                             static_cast<const __nv_bfloat16*>(k_fused), static_cast<const __nv_bfloat16*>(v_fused),
                             static_cast<__nv_bfloat16*>(out), lse, s));
   return QCF_OK;
+}
+
+}  // namespace
+
+qcf_status qcf_recompute_attn(qcf_ctx* ctx, const qcf_batch* b, const int32_t* sel, const int32_t* n_sel,
+                              const void* q_new, const void* k_new, const void* v_new, int32_t rows_by_position,
+                              void* k_fused, void* v_fused, void* out, float* lse, void* stream) {
+  return recompute_attn_impl(ctx, b, sel, n_sel, q_new, k_new, v_new, rows_by_position, k_fused, v_fused, out, lse, nullptr,
+                             nullptr, stream);
 }
 
 qcf_status qcf_full_prefill_attn(qcf_ctx* ctx, const qcf_batch* b, const void* q, const void* k, const void* v,
@@ -485,7 +499,10 @@ qcf_status qcf_decode_attn(qcf_ctx* ctx, const void* q, const void* k_cache, con
   return QCF_OK;
 }
 
-qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* a, void* stream) {
+namespace {
+
+qcf_status layer_step_impl(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* a, const void* q_gather_src,
+                           void* q_gather_dst, void* stream) {
   if (qcf_status st = check_ctx_batch(ctx, b)) return st;
   QCF_REQUIRE(ctx, a != nullptr, "qcf_layer_step: args is NULL");
   if (a->select_now) QCF_REQUIRE(ctx, a->ratio >= 0.0 && a->ratio <= 1.0, "qcf_layer_step: ratio must be in [0, 1]");
@@ -503,8 +520,8 @@ qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args
     if (qcf_status st = qcf_select_topk(ctx, b, a->scores, a->ratio, a->sel, a->n_sel, stream)) return st;
   if (prof) cudaEventRecord(ctx->ev[3], s);
   ctx->ev_valid = prof;      // lets qcf_recompute_attn record ev[4] between a4 and a5
-  qcf_status st = qcf_recompute_attn(ctx, b, a->sel, a->n_sel, a->q_new, a->k_new, a->v_new, a->rows_by_position,
-                                     a->k_fused, a->v_fused, a->out, a->lse, stream);
+  qcf_status st = recompute_attn_impl(ctx, b, a->sel, a->n_sel, a->q_new, a->k_new, a->v_new, a->rows_by_position,
+                                      a->k_fused, a->v_fused, a->out, a->lse, q_gather_src, q_gather_dst, stream);
   if (st) { ctx->ev_valid = false; return st; }
   if (prof) {
     if (b->batch == 0 || b->t_stride == 0) cudaEventRecord(ctx->ev[4], s);
@@ -513,6 +530,12 @@ qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args
   }
   ctx->ev_valid = false;
   return QCF_OK;
+}
+
+}  // namespace
+
+qcf_status qcf_layer_step(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer_args* a, void* stream) {
+  return layer_step_impl(ctx, b, a, nullptr, nullptr, stream);
 }
 
 qcf_status qcf_set_head_shards(qcf_ctx* ctx, int32_t n_shards) {
@@ -683,12 +706,8 @@ qcf_status qcf_layer_step_host(qcf_ctx* ctx, const qcf_batch* b, const qcf_layer
   d.sel = static_cast<int32_t*>(S.sel.p); d.n_sel = static_cast<int32_t*>(S.n_sel.p);
   d.q_new = zero_copy ? zq : S.q_new.p; d.k_new = zero_copy ? zk : S.k_new.p; d.v_new = zero_copy ? zv : S.v_new.p;
   d.out = S.out.p;
-  ctx->q_gather_src = zero_copy ? zq : nullptr;
-  ctx->q_gather_dst = S.q_new.p;
   d.lse = h->lse ? static_cast<float*>(S.lse.p) : nullptr;
-  const qcf_status st_step = qcf_layer_step(ctx, b, &d, stream);
-  ctx->q_gather_src = nullptr;
-  if (st_step) return st_step;
+  if (qcf_status st_step = layer_step_impl(ctx, b, &d, zero_copy ? zq : nullptr, S.q_new.p, stream)) return st_step;
 
   // only the |R_b| = k_b + Lq_b rows the step wrote are read back (k_b is known on the host: floor(rho N_b) when the step
   // selects, the caller's n_sel otherwise)

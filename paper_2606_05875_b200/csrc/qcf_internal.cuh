@@ -86,8 +86,6 @@ struct qcf_ctx {
   unsigned int* dec_counters;
   // host staging for qcf_layer_step_host
   struct HostStage* stage;
-  const void* q_gather_src;   // != nullptr during a zero-copy host step: position-indexed q_new in device-mapped host memory
-  void* q_gather_dst;         //   ... and the device buffer its rows R are gathered into (compact) before a5
   // profiling
   int profiling;
   static constexpr int kEvRing = 512;   // profiled steps kept between two qcf_get_stage_ms calls
@@ -163,7 +161,8 @@ cudaError_t launch_decode_attn(const qcf_ctx*, const __nv_bfloat16* q, const __n
                                int n_keys, __nv_bfloat16* out, float* lse, cudaStream_t);
 cudaError_t launch_gemm(const qcf_ctx*, const __nv_bfloat16* a, const __nv_bfloat16* w, const __nv_bfloat16* residual,
                         __nv_bfloat16* c, int M, int N, int K, int epilogue, cudaStream_t);
-// one row: c[N] = epilogue(x[K] . w[N][K]^T); gain != nullptr: x is RMS-normalised with that gain first (rounded to bf16)
+constexpr int kGemvMaxK = 113 * 1024;   // x[K] bf16 must fit the 227 KB of shared memory a CTA can have
+// one row: c[N] = epilogue(x[K] . w[N][K]^T), N even, K % 8 == 0, K <= kGemvMaxK (cudaErrorInvalidValue otherwise); gain != nullptr: x is RMS-normalised with that gain first (rounded to bf16)
 cudaError_t launch_gemv(const qcf_ctx*, const __nv_bfloat16* x, const __nv_bfloat16* w, const __nv_bfloat16* gain, float eps,
                         const __nv_bfloat16* residual, __nv_bfloat16* c, int N, int K, int epilogue, cudaStream_t);
 cudaError_t launch_lm_head(const qcf_ctx*, const __nv_bfloat16* w_lm, const __nv_bfloat16* h, int vocab, int hidden, float* logits,

@@ -268,6 +268,9 @@ qcf_status qcf_stack_decode(qcf_stack* s, const int32_t* token_in, int32_t pos0,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const int hid = s->dims.hidden, ffn = s->dims.ffn, vocab = s->dims.vocab;
   const int qkv_n = (L.hq + 2 * L.hkv) * L.d;
+  // the decode layer is four weight-streaming GEMVs that keep their input row in shared memory
+  if (hid > kGemvMaxK || ffn > kGemvMaxK || L.hq * L.d > kGemvMaxK)
+    return set_error(ctx, QCF_ERR_UNSUPPORTED, "qcf_stack_decode: hidden, ffn and Hq * head_dim must be <= " + std::to_string(kGemvMaxK));
   const size_t kv_row = static_cast<size_t>(L.hkv) * L.d;
   auto bf = [](const void* p) { return static_cast<const __nv_bfloat16*>(p); };
   for (int i = 0; i < n_new; ++i) {

@@ -341,6 +341,9 @@ cudaError_t launch_lm_head(const qcf_ctx* ctx, const __nv_bfloat16* w_lm, const 
 cudaError_t launch_gemv(const qcf_ctx* ctx, const __nv_bfloat16* x, const __nv_bfloat16* w, const __nv_bfloat16* gain, float eps,
                         const __nv_bfloat16* residual, __nv_bfloat16* c, int N, int K, int epilogue, cudaStream_t stream) {
   if (N <= 0) return cudaSuccess;
+  // two output rows per warp, x staged whole in shared memory as 16-byte words: anything else is the caller's to route
+  // to the tiled GEMM (launch_gemm does) or to refuse (qcf_stack_decode does) — never a silently dropped row
+  if (N % 2 != 0 || K % 8 != 0 || K > kGemvMaxK) return cudaErrorInvalidValue;
   int blocks = (N / 2 + 7) / 8;
   if (blocks > ctx->n_sm * 8) blocks = ctx->n_sm * 8;
   const size_t smem = static_cast<size_t>(K) * 2;
