@@ -376,17 +376,17 @@ def measure_layer_config(name, ratio, steps, warmup, dev, dist, world, want_e2e,
         flops += device.attn_flops(cfg, n, pos)
     a5_ms = float(stage_ms[4])
     achieved = flops / (a5_ms * 1e-3) / 1e12
-    # burst peak for a kernel timed alone in a sub-millisecond step; sustained (power-capped) peak for a multi-ms kernel
-    # inside a long step (c4 / c5: the clocks record shows sw_power_cap during the timed region)
-    long_step = ms_per_step >= 1.0
-    peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) if long_step else peaks["bf16_tflops"])
+    # The kernel is a few ms inside a step that is timed for well under a second: by MEASURED_PEAKS.json's own definition the
+    # burst figure is the denominator (the sustained one is for kernels inside seconds-long steps).  The fraction of the
+    # sustained peak is printed beside it: under the power cap the clocks record shows, the truth lies between the two.
+    peak = float(peaks["bf16_tflops"])
+    sustained = float(peaks.get("bf16_tflops_sustained", peak))
     traffic, traffic_src = profile_traffic(cfg.name, "attn_tc_kernel")
     work = dw.algorithmic_work()
     roofline = {"kernel": "attn_tc_kernel (a5 recompute attention)", "bound": "tensor", "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
-                "peak_source": "%s %s" % (peak_kind, "bf16_tflops_sustained (multi-ms kernel inside a long, power-capped step)"
-                                          if long_step else "bf16_tflops (burst: sub-ms step, kernel timed alone between events)"),
-                "frac_of_burst_peak": achieved / float(peaks["bf16_tflops"]),
+                "peak_source": "%s bf16_tflops (burst: a ms-scale kernel in a sub-second timed region)" % peak_kind,
+                "frac_of_sustained_peak": achieved / sustained, "sustained_peak": sustained,
                 "algorithmic_flops_per_launch": flops, "algorithmic_bytes_per_launch": work["a5_bytes"], "ms_per_launch": a5_ms}
     hbm = float(peaks["hbm_gbs"])
     sm_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
@@ -472,10 +472,13 @@ def run_qcf(args) -> None:
     if sub == "all":
         # the other BASELINE configs, same code, fewer steps: one driver run reproduces every row of DESIGN.md §7
         cfgs = {}
-        for key, name, ratio in (("c2", "c2", None), ("c5", "c5", None), ("c4_rho0.1", "c4", 0.1), ("c4_rho0.5", "c4", 0.5)):
+        for key, name, ratio in (("c1", "c1", None), ("c2", "c2", None), ("c5", "c5", None), ("c4_rho0.1", "c4", 0.1), ("c4_rho0.5", "c4", 0.5)):
             s2 = ClockSampler(local); s2.start(); time.sleep(0.2)
             n_steps = max(10, min(args.steps, 50)) if ratio is None else 10        # configs[3] sweeps rho in {0.1, 0.3, 0.5}
-            r = measure_layer_config(name, ratio, n_steps, args.warmup, dev, dist, world, want_e2e=False, want_cpu=False)
+            try:
+                r = measure_layer_config(name, ratio, n_steps, args.warmup, dev, dist, world, want_e2e=False, want_cpu=False)
+            except Exception as e:                           # the headline number must survive a failing sub-record
+                r = {"error": "%s: %s" % (type(e).__name__, e)}
             r["clocks"] = s2.stop()
             cfgs[key] = r
         try:

@@ -44,9 +44,31 @@ def test_header_compiles_as_plain_c(tmp_path):
 
 
 def test_library_is_sm100a_with_expected_kernels():
+    """The shipped cubin is sm_100a and its kernels are what DESIGN.md says they are (profiles/r03_sass_census.md holds the
+    same census as a table): the contractions issue tcgen05.mma (UTCHMMA) with TMEM loads (LDTM) and TMA tensor loads
+    (UTMALDG), the streaming kernels move rows with bulk async copies (UBLKCP), and no legacy mma.sync (HMMA) exists."""
     from paper_2606_05875_b200 import binding
     out = subprocess.run(["cuobjdump", "-lelf", binding.LIB_PATH], capture_output=True, text=True).stdout
     assert "sm_100a" in out
+    sass = subprocess.run(["cuobjdump", "-sass", binding.LIB_PATH], capture_output=True, text=True).stdout
+    census = {}
+    for part in re.split(r"\n\s*Function : ", sass)[1:]:
+        name = part.split("\n", 1)[0].strip()
+        census[name] = {op: len(re.findall(r"\b" + op, part)) for op in ("UTCHMMA", "LDTM", "UTMALDG", "UBLKCP", "HMMA")}
+    assert len(census) >= 40
+
+    def of(kernel):
+        rows = [c for n, c in census.items() if re.search(r"\d+" + kernel + r"(I|E)", n)]
+        assert rows, kernel
+        return rows
+
+    for kernel in ("attn_tc_kernel", "score_tc_kernel", "gemm_tc_kernel"):
+        for c in of(kernel):
+            assert c["UTCHMMA"] > 0 and c["LDTM"] > 0 and c["UTMALDG"] > 0, (kernel, c)
+    for kernel in ("reposition_tma_kernel", "scatter_tma_kernel", "gather_rows_tma_kernel"):
+        for c in of(kernel):
+            assert c["UBLKCP"] > 0, (kernel, c)
+    assert sum(c["HMMA"] for c in census.values()) == 0, "a legacy mma.sync path crept in"
 
 
 def test_n_select_floor_rule(lib):
