@@ -18,10 +18,7 @@
 // Tiles are walked row-block fastest, so the CTAs of one wave share a handful of W tiles: every weight is read from
 // HBM once, A (<= 77 MB) stays in L2.
 // Epilogues: store | + residual (in place allowed) | SwiGLU over interleaved (gate, up) output columns.
-// Measured and dropped: 128 x 192 tiles where they quantise better (QKV at M = 3136: 4.05 waves of 256-wide tiles): 0.128 -> 0.137 ms;
-// split-K (fp32 partials in a workspace, last arriver reduces) for the 64-row probe GEMMs of stage 1,
-// which stream 34-200 MB of weights through 16-96 CTAs: down projection 79 -> 56 us, but QKV 25 -> 33 us and O 29 -> 42 us
-// (the partial write + fence + reduce costs more than the extra CTAs save), stage 1 as a whole 4.73 -> 4.62 ms.
+// (Tile shapes and split-K variants measured and dropped: DESIGN.md §9.4.)
 #include "qcf_internal.cuh"
 #include "sm100_ptx.cuh"
 

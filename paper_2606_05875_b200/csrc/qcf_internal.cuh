@@ -212,7 +212,8 @@ __device__ __forceinline__ int ld_ca_s32(const int32_t* p) {
   asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(v) : "l"(p));
   return v;
 }
-__device__ __forceinline__ uint4 ld_nc_v4(const void* p) {
+// coherent 128-bit load that does not allocate in L1 ("na"; NOT the non-coherent .nc path, see the PDL note above)
+__device__ __forceinline__ uint4 ld_na_v4(const void* p) {
   uint4 r;
   asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)

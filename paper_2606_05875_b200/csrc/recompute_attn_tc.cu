@@ -35,43 +35,9 @@ constexpr int kColO = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleSum = 256.0f;         // rescale when a tile's row sum (relative to the reference max) exceeds 2^8
-#ifndef QCF_ATTN_MUFU_PAIRS
-#define QCF_ATTN_MUFU_PAIRS 3
-#endif
-// Measured dead ends on this kernel (all parity-green, all slower on c2; kept out of the code):
-//   * two threads per row (8 softmax warps, 32 key columns each, barrier.red agreement per tile): 82 -> 92 us, and a lone
-//     CTA's tile step went 0.80 -> 0.89 us: the step is not sweep-bound — one warp-wide EX2 takes 8 cycles on its SMSP
-//     (16/clk/SM), so the 64 exponentials of a row are ~512 cycles however the row is divided;
-//   * splitting every item's keys over 2 / 4 CTAs (cluster + DSMEM merge, or global partials merged by the last
-//     arriver): 107 -> 127 / 158 us — at c2 the SMs are throughput-bound, a split only adds prologues and merge traffic
-//     (it does pay when the grid under-fills the machine: rho = 0, 16 items: 82 -> 53 us, hence the heuristic below);
-//   * a second CTA for only the 4-24 heaviest row tiles of each (request, kv-head) ("tail trim", partials merged through a
-//     global workspace): 82 -> 84-92 us — trimming the 81-step tail buys nothing, the SMs are throughput-bound;
-//   * ONE CTA per SM owning two items (the same row tile for two adjacent kv-heads: 512 TMEM columns, one producer, one
-//     issuer, two softmax groups), with or without FA-style turn taking between the groups on named barriers: c5 2675 ->
-//     3320-3400 us, c2 82 -> 127 us.  A lone warp does not saturate its SMSP's MUFU (a sweep alone takes ~1500 cycles, not
-//     the 512 the unit could do), so serialising the groups halves the MUFU rate, and a shared issuer blocks one item on
-//     the other's P; two independent CTAs per SM remain the best arrangement found;
-//   * halving the K/V loads (timing experiment, wrong results): c2 unchanged, c5 -9 %: L2 -> SM traffic is not the limiter;
-//   * a persistent work-list kernel (device-built work list, split-KV partials merged by the last arriver; removed from the tree);
-//   * S = Q K^T for PAIRS of key tiles as one 128 x 128 x 16 chain into a single 128-column S buffer (the TMEM budget of two
-//     CTAs per SM leaves no room to double-buffer it): c2 75.8 -> 90.1 us, c5 2.51 -> 2.90 ms — the serialised
-//     QK -> softmax -> PV chain costs more than the cheaper MMA saves;
-//   * pairing the heaviest tile of the first block round with the lightest of the second (equal pair sums): 75.8 -> 74.9 us;
-//   * one launch of 2-CTA clusters in which the heaviest 10-100 % of the items have their keys split over the pair and every
-//     other cluster carries two independent items: 75.8 -> 80.1 (10 %) ... 95.0 us (100 %).
-// What bounds it (microbenchmarks + knock-outs): a 128 x 64 x 16 SS MMA takes ~57 cycles, not the 32
-// its flops need (the 4 KB A read from shared memory; N = 128: 67, N = 256: 128, TS N = 128: 64), so one 64-key step is
-// 624 cycles of tensor pipe (8 SS + 4 TS), 82 % of peak at best.  A skeleton of this loop (MMAs and barrier handshakes
-// only) runs AT that floor with two CTAs per SM (607-631 cycles per step) and at 770-925 alone; the full kernel with the
-// loads, the exponentials and the S loads removed still takes 75.3 of its 75.8 us at c2: the step is bound by the tensor
-// pipe shared between the two CTAs plus ~0.1 us of sweep ALU work and ring barriers per CTA step, and the launch by the
-// heaviest tile's 81-step chain (3.3 us prologue + 81 x 0.80 us).
-// Of every 4 pairs, how many take MUFU.EX2 (the rest: packed polynomial on the FMA pipe).  Round 1 (before the elected-lane
-// issue fix, when the sweep was issue-bound) measured 4 -> 84 us, 3 -> 91 us on c2.  Re-measured in round 2 on the current
-// kernel: c2 76.7 vs 76.8 us (neutral), c4 x 16 2.84 -> 2.80 ms, c5 2.57 -> 2.49 ms with 3 — MUFU and tensor pipe are both
-// ~60 % busy (profiles/r02_c4.md), a quarter of the exponentials on the FMA pipe unloads the tighter of the two.
-constexpr int kMufuPairs = QCF_ATTN_MUFU_PAIRS;
+// Of every 4 exponential pairs, 3 take MUFU.EX2 and 1 the packed polynomial on the FMA pipe (MUFU and tensor pipe are both
+// ~60 % busy; this unloads the tighter one).  What bounds the kernel and the arrangements measured and rejected: DESIGN.md §9.4.
+constexpr int kMufuPairs = 3;
 
 // Two CTAs are resident per SM (96 KB of shared memory, 256 TMEM columns and <= 168 registers each).  Inside a CTA
 // S_{j+1} = Q K_{j+1}^T is issued before P_j V_j, so the softmax of tile j overlaps it; across the two CTAs the
@@ -145,7 +111,18 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   //              18.8 GB of DRAM traffic for 0.55 GB of cache, profiles/r02_c4_base.md);
   //   section B: tiles past the host's row-count hint `tiles_hint` (the selection size lives on the device), all units —
   //              normally empty, they retire under the tail.
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t sbase = smem_u32(smem);
+  auto bar = [&](int i) -> uint32_t { return sbase + S::oBar + 8 * i; };
   pdl_trigger();
+  // Everything that touches no predecessor data runs before the dependency wait, under the predecessor's tail: descriptor
+  // prefetch and barrier init.  (The TMEM allocation stays behind the wait: CTAs that find no work below return early.)
+  if (warp == 0 && lane == 0) {
+    prefetch_tensormap(&tm_k);
+    prefetch_tensormap(&tm_v);
+    for (int i = 0; i < S::kNumBar; ++i) mbar_init(bar(i), (i == kPReady || i == kPReady + 1 || i == kQFull) ? 128 : 1);
+    fence_barrier_init();
+  }
   pdl_wait();          // n_sel / sel below are written by the predecessors
   const int ncl = static_cast<int>(cluster_nctarank());
   const int crank = static_cast<int>(cluster_ctarank());
@@ -174,7 +151,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   if (t_idx >= n_tiles) return;
   const int tile = n_tiles - 1 - t_idx;
   const int ridx0 = tile * PT;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int* sel_b = dense ? nullptr : sel + static_cast<size_t>(b) * bd.n_stride;
   auto pos_of = [&](int r) -> int {          // request position of row r of R (padding rows: 0, never stored)
     if (r >= n_rows) return 0;
@@ -189,21 +165,10 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
   const int n_kt = kt_base + (crank < kt_rem ? 1 : 0);
   const int t_end = N + Lq;                  // rows >= t_end of the cache are padding
 
-  const uint32_t sbase = smem_u32(smem);
   const uint32_t sQ = sbase + S::oQ, sK = sbase + S::oK, sV = sbase + S::oV;
-  auto bar = [&](int i) -> uint32_t { return sbase + S::oBar + 8 * i; };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + S::oTmem);
 
-  if (warp == 0) {
-    if (lane == 0) {
-      prefetch_tensormap(&tm_k);
-      prefetch_tensormap(&tm_v);
-      for (int i = 0; i < S::kNumBar; ++i) mbar_init(bar(i), (i == kPReady || i == kPReady + 1 || i == kQFull) ? 128 : 1);
-      fence_barrier_init();
-    }
-  } else if (warp == 1) {
-    tmem_alloc<kTmemCols>(sbase + S::oTmem);
-  }
+  if (warp == 1) tmem_alloc<kTmemCols>(sbase + S::oTmem);
   // Q tile: the gathered rows are requested from global memory BEFORE the CTA-wide sync and land in shared memory after
   // it, signalled on their own barrier, so the producer's first K / V TMA loads (issued right after the sync) and the
   // TMEM allocation overlap the gather latency instead of queueing behind it.
@@ -219,7 +184,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tm_k, const __grid_constant__
     }
 #pragma unroll
     // coherent loads: in the stack path q is written by a predecessor this kernel's lifetime overlaps (PDL)
-    for (int c = 0; c < D / 8; ++c) qv[c] = src ? ld_nc_v4(src + c) : make_uint4(0u, 0u, 0u, 0u);
+    for (int c = 0; c < D / 8; ++c) qv[c] = src ? ld_na_v4(src + c) : make_uint4(0u, 0u, 0u, 0u);
   }
   tc_fence_before();
   __syncthreads();

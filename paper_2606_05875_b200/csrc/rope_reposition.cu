@@ -7,10 +7,6 @@
 #include "qcf_internal.cuh"
 #include "sm100_ptx.cuh"
 
-#ifndef QCF_REPO_TMA
-#define QCF_REPO_TMA 1
-#endif
-
 namespace qcf {
 
 namespace {
@@ -74,13 +70,13 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
   uint4 tv[4];
 #pragma unroll
   for (int u = 0; u < 4; ++u)
-    if (static_cast<int>(threadIdx.x + u * blockDim.x) < n_vec) tv[u] = ld_nc_v4(vs + threadIdx.x + u * blockDim.x);
+    if (static_cast<int>(threadIdx.x + u * blockDim.x) < n_vec) tv[u] = ld_na_v4(vs + threadIdx.x + u * blockDim.x);
   if (k_pool == nullptr) {
     // V-only stitch (the K of a critical layer was re-positioned ahead of time for scoring)
   } else if (identity) {
     for (int r = rsub; r < rows; r += rows_per_pass) {
-      const uint4 a = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0);
-      const uint4 b = ld_nc_v4(ks + static_cast<size_t>(r) * row_elems + e0 + D / 2);
+      const uint4 a = ld_na_v4(ks + static_cast<size_t>(r) * row_elems + e0);
+      const uint4 b = ld_na_v4(ks + static_cast<size_t>(r) * row_elems + e0 + D / 2);
       st_na_v4(kd + static_cast<size_t>(r) * row_elems + e0, a);
       st_na_v4(kd + static_cast<size_t>(r) * row_elems + e0 + D / 2, b);
     }
@@ -100,8 +96,8 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
     for (int it = 0; it < kMaxIter; ++it) {
       if (it < n_it) {
         const size_t r = rsub + it * rows_per_pass;
-        a[it] = ld_nc_v4(ks + r * row_elems + e0);
-        b[it] = ld_nc_v4(ks + r * row_elems + e0 + D / 2);
+        a[it] = ld_na_v4(ks + r * row_elems + e0);
+        b[it] = ld_na_v4(ks + r * row_elems + e0 + D / 2);
       }
     }
 #pragma unroll
@@ -126,7 +122,7 @@ __global__ void __launch_bounds__(512) reposition_kernel(BatchDev bd, int hkv, c
     uint4 t[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u)
-      if (i + u * blockDim.x < n_vec) t[u] = ld_nc_v4(vs + i + u * blockDim.x);
+      if (i + u * blockDim.x < n_vec) t[u] = ld_na_v4(vs + i + u * blockDim.x);
 #pragma unroll
     for (int u = 0; u < 4; ++u)
       if (i + u * blockDim.x < n_vec) st_na_v4(vd + i + u * blockDim.x, t[u]);
@@ -222,8 +218,7 @@ cudaError_t launch_reposition(const qcf_ctx* ctx, const qcf_batch* b, const __nv
   if (rpp < 1) rpp = 1;
   if (rpp > kRepoRows) rpp = kRepoRows;
   const int threads = slots * rpp;     // slots <= 512 is enforced at qcf_create
-#if QCF_REPO_TMA
-  {
+  {   // bulk-copy staged kernel whenever its work item fits shared memory; the register-staged kernel otherwise
     const size_t row_bytes = static_cast<size_t>(ctx->lay.hkv) * ctx->lay.d * 2;
     const size_t smem = kRepoRows * row_bytes * ((k_pool ? 1 : 0) + (v_pool ? 1 : 0));
     if (threads <= 256 && smem <= 200 * 1024) {
@@ -237,7 +232,6 @@ cudaError_t launch_reposition(const qcf_ctx* ctx, const qcf_batch* b, const __nv
       return launch_pdl(ctx->pdl, kern, dim3(b->repo_blocks), dim3(threads), smem, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
     }
   }
-#endif
   if (ctx->lay.d == 128)
     return launch_pdl(ctx->pdl, reposition_kernel<128>, dim3(b->repo_blocks), dim3(threads), 0, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);
   return launch_pdl(ctx->pdl, reposition_kernel<64>, dim3(b->repo_blocks), dim3(threads), 0, stream, b->dev, ctx->lay.hkv, k_pool, v_pool, k_f, v_f);

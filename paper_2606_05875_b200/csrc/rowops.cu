@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) embed_gather_kernel(const uint4* __restri
   const int tok = __ldg(tokens + rp(r));
   const uint4* src = embed + static_cast<size_t>(tok) * row_vec;
   uint4* dst = x + static_cast<size_t>(r) * row_vec;
-  for (int i = lane; i < row_vec; i += 32) dst[i] = ld_nc_v4(src + i);
+  for (int i = lane; i < row_vec; i += 32) dst[i] = ld_na_v4(src + i);
 }
 
 // y = x / sqrt(mean(x^2) + eps) * g      one warp per row; the row (<= 16 KB) is re-read from L1/L2 for the second sweep
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256) anchor_score_kernel(BatchDev bd, int row_
     const uint4* src = k_pool + (static_cast<size_t>(bd.chunk_row[c]) + r) * row_vec;
     float ss = 0.f;
     for (int i = lane; i < row_vec; i += 32) {
-      const uint4 v = ld_nc_v4(src + i);
+      const uint4 v = ld_na_v4(src + i);
       const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
       for (int k = 0; k < 4; ++k) { const float x = bf16lo(w[k]), y = bf16hi(w[k]); ss = fmaf(x, x, ss); ss = fmaf(y, y, ss); }
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(256) gemv_kernel(const uint4* __restrict__ w, 
   pdl_wait();                                   // x / residual are written by the predecessor kernel
   float ss = 0.f;
   for (int i = threadIdx.x; i < k8; i += blockDim.x) {
-    const uint4 v = ld_nc_v4(x + i);            // coherent (not .nc): see the PDL note in qcf_internal.cuh
+    const uint4 v = ld_na_v4(x + i);            // coherent (not .nc): see the PDL note in qcf_internal.cuh
     s_x[i] = v;
     if (NORM) {
       const uint32_t u[4] = {v.x, v.y, v.z, v.w};
@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(256) gemv_kernel(const uint4* __restrict__ w, 
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         const int i = i0 + 32 * u;
-        if (i < k8) { a0[u] = ld_nc_v4(w0 + i); a1[u] = ld_nc_v4(w1 + i); }
+        if (i < k8) { a0[u] = ld_na_v4(w0 + i); a1[u] = ld_na_v4(w1 + i); }
       }
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(256) lm_head_kernel(const uint4* __restrict__ 
     const uint4* src = w + static_cast<size_t>(v) * row_vec;
     float acc = 0.f;
     for (int i = lane; i < row_vec; i += 32) {
-      const uint4 a = ld_nc_v4(src + i), b = s_h[i];
+      const uint4 a = ld_na_v4(src + i), b = s_h[i];
       const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
 #pragma unroll
       for (int k = 0; k < 4; ++k) { acc = fmaf(bf16lo(aw[k]), bf16lo(bw[k]), acc); acc = fmaf(bf16hi(aw[k]), bf16hi(bw[k]), acc); }

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(256) scatter_kernel(BatchDev bd, int row_vec, 
       uint4 kk[4], vv[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u)
-        if (i + 32 * u < row_vec) { kk[u] = ld_nc_v4(k_new + src + i + 32 * u); vv[u] = ld_nc_v4(v_new + src + i + 32 * u); }
+        if (i + 32 * u < row_vec) { kk[u] = ld_na_v4(k_new + src + i + 32 * u); vv[u] = ld_na_v4(v_new + src + i + 32 * u); }
 #pragma unroll
       for (int u = 0; u < 4; ++u)
         if (i + 32 * u < row_vec) { k_f[dst + i + 32 * u] = kk[u]; v_f[dst + i + 32 * u] = vv[u]; }

@@ -32,13 +32,10 @@ constexpr int HC = BT / 2;          // S columns swept by one consumer thread
 constexpr int kTmemCols = 256;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kStaleSum = 1099511627776.0f;      // 2^40
-#ifndef QCF_SCORE_MUFU_PAIRS
-#define QCF_SCORE_MUFU_PAIRS 3
-#endif
 // Of every 4 pairs, how many take MUFU.EX2 (the rest: the packed polynomial on the FMA pipe).  Unlike attention (no P V, no
 // P packing) these sweeps are MUFU-bound — 128 x 128 exponentials against a 256-cycle MMA per tile — so a quarter of them
 // moves to the FMA pipe: a2 on c4 600 -> 530 us, c5 295 -> 262 us, c2 30.8 -> 29.1 us (a half: 570 / 273 / 29.6).
-constexpr int kMufuPairs = QCF_SCORE_MUFU_PAIRS;
+constexpr int kMufuPairs = 3;
 
 template <int D>
 struct Smem {
@@ -553,11 +550,7 @@ cudaError_t launch_score(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bflo
   }
   // pass 2: key tiles per CTA (kt).  Equal-sized CTAs run in rounds of `slots`; a launch wastes the empty part of its last
   // round and a fixed prologue per CTA (barriers, TMEM, combining the pass-1 partials into lse: ~0.3 of a tile walk).  Pick
-  // the kt <= 32 with the best (fill of the last round) x kt / (kt + 0.3).  Measured: c5 (8 pairs x 256 tiles) kt = 7 gives 296
-  // CTAs, exactly one round: a2 218 -> 202 us against the former 3 (688 CTAs, 2.3 rounds); c4 x 16 (128 pairs x 64 tiles)
-  // kt = 4 (2048 CTAs, 6.9 rounds) and the former 11 (768 CTAs) are within 1 %, kt = 32 (256 CTAs, one round at 86 % fill)
-  // is 7 % slower.  (Publishing lse from pass 1's last-arriving split so that pass 2 only loads it was also measured:
-  // c2 23.6 -> 25.6 us — a fence + atomic round trip at the end of every pass-1 CTA — and no gain at c4.)
+  // the kt <= 32 with the best (fill of the last round) x kt / (kt + 0.3).  (Measurements behind it: DESIGN.md §9.4.)
   int kt_per_cta = 1;
   {
     const int pairs = L.hkv * b->batch;
