@@ -598,6 +598,43 @@ def test_full_size_c4_batch16(ratio, k):
     for b in sorted(picks):
         assert _check_full_size(wl, dw, b, 40 + b) >= 64 + 128
     assert dw.n_sel.cpu().tolist() == [k] * 16                     # floor(rho * 8192), the seven pins of reading (g)
+    if ratio == 0.3:
+        for b in sorted(set(range(16)) - picks):                   # a2 + a3 of EVERY request of the headline batch
+            _check_scores_and_selection(wl, dw, b)
+
+
+def _check_scores_and_selection(wl, dw, b):
+    r, k_pic, v_pic = _oracle_inputs(wl, b)
+    n = r.n_ctx
+    k_ctx, _ = O.reposition(k_pic, v_pic, wl.cfg.rope_theta)
+    want_sc = O.score(O.widen_bf16(r.q_probe), k_ctx)
+    got32 = dw.scores[b, :n].cpu().numpy()
+    np.testing.assert_allclose(got32.astype(np.float64), want_sc, rtol=1e-2, atol=0)
+    k = int(dw.n_sel[b])
+    assert k == O.n_select(n, wl.cfg.ratio)
+    sel = dw.sel[b, :k].cpu().numpy().astype(np.int64)
+    _check_selection(sel, want_sc, k)
+    assert np.array_equal(sel, O.select_topk(got32, k))            # integer work on the GPU's own scores: bit-exact
+    return sel, want_sc
+
+
+def test_layer_step_host_full_size_c4_batch16_against_oracle():
+    """The end-to-end leg `bench.py` times (`e2e`: qcf_layer_step_host at configs[3], all 16 requests, pinned host buffers:
+    pool rows uploaded by interval, fresh rows read zero-copy by a4 and the q gather, |R| rows downloaded) checked against
+    the ORACLE, not against the device path: scores and selection of four requests in full, attention outputs and the fused
+    cache of the first and the last request on the declared row sample."""
+    _, device = _binding()
+    wl = inputs.make_workload("c4")
+    ctx = _ctx_for(wl.cfg)
+    hw = device.DeviceWorkload(wl, ctx, device="cpu", pin=True)
+    assert hw.B == 16
+    args = hw.layer_args()
+    args.k_fused, args.v_fused = hw.k_fused.data_ptr(), hw.v_fused.data_ptr()
+    ctx.qcf_layer_step_host(hw.batch, args, hw.pool_rows)            # synchronises the stream before returning
+    for b in (0, 15):
+        assert _check_full_size(wl, hw, b, 60 + b) >= 64 + 128
+    for b in (5, 10):
+        _check_scores_and_selection(wl, hw, b)
 
 
 def test_layer_step_host_rejects_chunks_outside_the_pool():
@@ -658,5 +695,5 @@ def test_layer_step_ragged_batch_parity():
         _check_selection(got_sel, want_sc, k)
         ref = O.layer_step(k_pic, v_pic, cfg.rope_theta, None, 0.0, O.widen_bf16(qn[i, : n + lq]), O.widen_bf16(kn[i, : n + lq]),
                            O.widen_bf16(vn[i, : n + lq]), sel=got_sel)
-        assert np.max(np.abs(_f64(out[i, : k + lq]) - ref["out"])) <= 2e-2
+        _assert_attn_close(_f64(out[i, : k + lq]), ref["out"])               # max-abs 2e-2 + per-vector relative
         assert np.array_equal(_f64(vf[i, : n + lq]), ref["v_fused"])
