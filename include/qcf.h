@@ -258,6 +258,20 @@ QCF_API qcf_status qcf_anchor_rank(qcf_ctx* ctx, const qcf_batch* chunks, const 
                                    float* scores, int32_t accumulate, int32_t select_now, int32_t* anchor_idx,
                                    int32_t* n_anchor, void* stream);
 
+/* Eq. 16: KV_i^A = KV_i^PIC[A_i] — the step between the ranking above and the anchor stitch (a1'):
+ * the anchor rows of every chunk are copied out of a layer's PIC pool into that layer's COMPACT anchor pool, chunk after
+ * chunk, anchors ascending inside a chunk — exactly the pool layout a chunk_pos batch reads (chunk i's "chunk" = its
+ * |A_i| anchor rows starting at row sum_{j<i} |A_j|).
+ *   chunks     : the one-chunk-per-request batch of qcf_anchor_rank (chunk_row = the chunk's first row in the PIC pool)
+ *   k_pool, v_pool     : dev [pool_rows][Hkv][d] bf16, this layer's PIC pool; either may be NULL (with its output)
+ *   anchor_idx, n_anchor : dev, as written by qcf_anchor_rank (chunk-local positions; counts)
+ *   k_anchor, v_anchor : dev [>= sum_i n_anchor[i]][Hkv][d] bf16, written; the caller sizes them (n_anchor[i] =
+ *                        ceil(r_a |c_i|) is known on the host).  Rows are byte copies; K keeps its chunk-local RoPE, which
+ *                        qcf_rope_reposition on the chunk_pos batch then moves to off_i + a (Eq. 15). */
+QCF_API qcf_status qcf_anchor_gather(qcf_ctx* ctx, const qcf_batch* chunks, const void* k_pool, const void* v_pool,
+                                     const int32_t* anchor_idx, const int32_t* n_anchor, void* k_anchor, void* v_anchor,
+                                     void* stream);
+
 /* ------------------------------------------------------------------------------------------------ a6 */
 
 /* Everything one layer needs, by name.  Pointers as documented at the stage entry points. */

@@ -22,7 +22,7 @@ EXPORTS = (
     "qcf_create", "qcf_destroy", "qcf_last_error", "qcf_version", "qcf_batch_create", "qcf_batch_destroy",
     "qcf_batch_get_info", "qcf_n_select", "qcf_rope_reposition", "qcf_score", "qcf_select_topk", "qcf_recompute_attn",
     "qcf_full_prefill_attn", "qcf_layer_step", "qcf_layer_step_host", "qcf_set_profiling", "qcf_get_stage_ms", "qcf_set_head_shards", "qcf_debug_set",
-    "qcf_anchor_rank", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
+    "qcf_anchor_rank", "qcf_anchor_gather", "qcf_linear", "qcf_stack_create", "qcf_stack_destroy", "qcf_stack_prefill", "qcf_stack_layer", "qcf_stack_fuse", "qcf_stack_first_token",
     "qcf_decode_attn", "qcf_decode_attn_static", "qcf_stack_decode", "qcf_score_exchange_bytes", "qcf_set_score_exchange",
 )
 
@@ -118,6 +118,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
         "qcf_set_score_exchange": (i32, [vp, i32, i32, C.POINTER(vp), i64]),
         "qcf_get_stage_ms": (i32, [vp, C.POINTER(C.c_float)]),
         "qcf_anchor_rank": (i32, [vp, vp, vp, i32, f64, vp, i32, i32, vp, vp, vp]),
+        "qcf_anchor_gather": (i32, [vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "qcf_linear": (i32, [vp, vp, vp, vp, vp, i32, i32, i32, i32, vp]),
         "qcf_stack_create": (i32, [vp, C.POINTER(qcf_stack_dims), C.POINTER(qcf_layer_weights), vp, i32, i32, i64,
                                    C.POINTER(vp)]),
@@ -259,6 +260,10 @@ class Context:
         self._check(self.lib.qcf_anchor_rank(self.handle, chunks.handle, _ptr(k_pool), int(rule), float(r_a), _ptr(scores),
                                              int(bool(accumulate)), int(bool(select_now)), _ptr(anchor_idx), _ptr(n_anchor),
                                              _stream(stream)))
+
+    def qcf_anchor_gather(self, chunks: Batch, k_pool, v_pool, anchor_idx, n_anchor, k_anchor, v_anchor, stream=None):
+        self._check(self.lib.qcf_anchor_gather(self.handle, chunks.handle, _ptr(k_pool), _ptr(v_pool), _ptr(anchor_idx),
+                                               _ptr(n_anchor), _ptr(k_anchor), _ptr(v_anchor), _stream(stream)))
 
     def qcf_linear(self, a, w, residual, c, M: int, N: int, K: int, epilogue: int = QCF_EPI_STORE, stream=None):
         self._check(self.lib.qcf_linear(self.handle, _ptr(a), _ptr(w), _ptr(residual), _ptr(c), M, N, K, epilogue,

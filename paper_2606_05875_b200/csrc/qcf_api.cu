@@ -427,6 +427,23 @@ qcf_status qcf_anchor_rank(qcf_ctx* ctx, const qcf_batch* b, const void* k_pool,
   return QCF_OK;
 }
 
+qcf_status qcf_anchor_gather(qcf_ctx* ctx, const qcf_batch* b, const void* k_pool, const void* v_pool, const int32_t* anchor_idx,
+                             const int32_t* n_anchor, void* k_anchor, void* v_anchor, void* stream) {
+  if (qcf_status st = check_ctx_batch(ctx, b)) return st;
+  QCF_REQUIRE(ctx, b->n_chunks <= b->batch && b->q_stride == 0, "qcf_anchor_gather: the batch must list one chunk per request and no query");
+  if (b->batch == 0 || b->n_stride == 0) return QCF_OK;
+  QCF_REQUIRE(ctx, anchor_idx && n_anchor, "qcf_anchor_gather: anchor_idx / n_anchor is NULL");
+  QCF_REQUIRE(ctx, (k_pool != nullptr) == (k_anchor != nullptr) && (v_pool != nullptr) == (v_anchor != nullptr),
+              "qcf_anchor_gather: a pool and its anchor pool must both be given or both be NULL");
+  QCF_REQUIRE(ctx, k_pool || v_pool, "qcf_anchor_gather: nothing to gather");
+  QCF_REQUIRE(ctx, aligned16(k_pool) && aligned16(v_pool) && aligned16(k_anchor) && aligned16(v_anchor),
+              "qcf_anchor_gather: pointers must be 16-byte aligned");
+  QCF_CUDA(ctx, launch_anchor_gather(ctx, b, static_cast<const __nv_bfloat16*>(k_pool), static_cast<const __nv_bfloat16*>(v_pool),
+                                     anchor_idx, n_anchor, static_cast<__nv_bfloat16*>(k_anchor),
+                                     static_cast<__nv_bfloat16*>(v_anchor), static_cast<cudaStream_t>(stream)));
+  return QCF_OK;
+}
+
 namespace {
 
 // a4 + a5.  q_gather_src != nullptr (the zero-copy host step only): q_new is position-indexed in device-mapped HOST memory;

@@ -145,6 +145,10 @@ cudaError_t launch_exchange_ack(const qcf_ctx*, cudaStream_t);
 // G_i(r) of Eq. 14 for every chunk row of the batch (rule 0: sink, 1: knorm) into scores[B][n_stride]
 cudaError_t launch_anchor_scores(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool, int rule, int accumulate,
                                  float* scores, cudaStream_t);
+// Eq. 16: rows chunk_row + anchor_idx[b][r] of the PIC pool -> compact anchor pool (chunk order); K and / or V
+cudaError_t launch_anchor_gather(const qcf_ctx*, const qcf_batch*, const __nv_bfloat16* k_pool, const __nv_bfloat16* v_pool,
+                                 const int32_t* anchor_idx, const int32_t* n_anchor, __nv_bfloat16* k_anchor,
+                                 __nv_bfloat16* v_anchor, cudaStream_t);
 cudaError_t launch_scatter(const qcf_ctx*, const qcf_batch*, const int32_t* sel, const int32_t* n_sel,
                            const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, int rows_by_position,
                            __nv_bfloat16* k_f, __nv_bfloat16* v_f, cudaStream_t);

@@ -159,6 +159,41 @@ __global__ void __launch_bounds__(256) anchor_score_kernel(BatchDev bd, int row_
   }
 }
 
+// Eq. 16: KV_i^A = KV_i^PIC[A_i].  Request b of the batch is chunk b (one chunk per request, as for the
+// ranking above); row chunk_row + anchor_idx[b][r] of the layer's PIC pool goes to row base_b + r of the compact anchor pool,
+// base_b = sum_{j<b} n_anchor[j] (chunk order, anchors ascending inside a chunk).  A pure row gather: one warp per row,
+// 128-bit coalesced loads and stores, K and V in the same pass.
+__global__ void __launch_bounds__(256) anchor_gather_kernel(BatchDev bd, int row_vec, const uint4* k_pool, const uint4* v_pool,
+                                                            const int32_t* anchor_idx, const int32_t* n_anchor,
+                                                            uint4* k_anchor, uint4* v_anchor) {
+  __shared__ long long s_base;
+  const int b = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int na = __ldcg(n_anchor + b);
+  if (warp == 0) {
+    long long acc = 0;
+    for (int j = lane; j < b; j += 32) acc += __ldcg(n_anchor + j);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) s_base = acc;
+  }
+  __syncthreads();
+  if (na <= 0 || bd.n_chunks == 0) return;
+  int c = b < bd.n_chunks ? b : bd.n_chunks - 1;              // the request's chunk, found by owner (empty requests own none)
+  while (c > 0 && bd.chunk_req[c] > b) --c;
+  while (c + 1 < bd.n_chunks && bd.chunk_req[c] < b) ++c;
+  const size_t src0 = static_cast<size_t>(bd.chunk_row[c]);
+  const size_t dst0 = static_cast<size_t>(s_base);
+  for (int r = blockIdx.x * 8 + warp; r < na; r += gridDim.x * 8) {
+    const int a = __ldcg(anchor_idx + static_cast<size_t>(b) * bd.n_stride + r);
+    const size_t src = (src0 + a) * row_vec, dst = (dst0 + r) * row_vec;
+    for (int i = lane; i < row_vec; i += 32) {
+      if (k_pool) st_na_v4(k_anchor + dst + i, ld_na_v4(k_pool + src + i));
+      if (v_pool) st_na_v4(v_anchor + dst + i, ld_na_v4(v_pool + src + i));
+    }
+  }
+}
+
 // Decoding pushes ONE row through the block: y[N] = x[K] . W[N][K]^T is a pure weight stream
 // (386 MB per layer at config 3, ~1 flop per byte), so it is a warp-per-output-row-pair GEMV, not a tensor-core tile:
 // x (optionally RMS-normalised with its gain on the way in, rounded to bf16 exactly as the batched path stores h) sits in
@@ -322,6 +357,18 @@ cudaError_t launch_anchor_scores(const qcf_ctx* ctx, const qcf_batch* b, const _
   if (b->batch == 0 || b->n_stride == 0) return cudaSuccess;
   anchor_score_kernel<<<dim3((b->n_stride + 7) / 8, b->batch), 256, 0, stream>>>(
       b->dev, ctx->lay.hkv * ctx->lay.d / 8, reinterpret_cast<const uint4*>(k_pool), rule, accumulate, scores);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_anchor_gather(const qcf_ctx* ctx, const qcf_batch* b, const __nv_bfloat16* k_pool, const __nv_bfloat16* v_pool,
+                                 const int32_t* anchor_idx, const int32_t* n_anchor, __nv_bfloat16* k_anchor,
+                                 __nv_bfloat16* v_anchor, cudaStream_t stream) {
+  if (b->batch == 0 || b->n_stride == 0) return cudaSuccess;
+  int bx = (b->n_stride + 7) / 8;
+  if (bx > 64) bx = 64;
+  anchor_gather_kernel<<<dim3(bx, b->batch), 256, 0, stream>>>(
+      b->dev, ctx->lay.hkv * ctx->lay.d / 8, reinterpret_cast<const uint4*>(k_pool), reinterpret_cast<const uint4*>(v_pool),
+      anchor_idx, n_anchor, reinterpret_cast<uint4*>(k_anchor), reinterpret_cast<uint4*>(v_anchor));
   return cudaGetLastError();
 }
 

@@ -535,6 +535,66 @@ def test_anchor_rank_parity(rule):
             assert len(np.intersect1d(got, O.select_topk(g2, k))) >= np.ceil(0.99 * k)
 
 
+@pytest.mark.parametrize("rule", ["sink", "knorm"])
+def test_phase1_rank_gather_stitch_through_the_c_abi(rule):
+    """Phase I closed inside the library (Eq. 14 -> Eq. 16 -> Eq. 15): qcf_anchor_rank picks A_i per chunk, qcf_anchor_gather
+    copies KV_i^PIC[A_i] into the compact anchor pool, qcf_rope_reposition on the chunk_pos batch stitches it.  Against the
+    oracle's anchor_stitch on the GPU's own anchor lists: the gathered V rows byte for byte (a pure row gather), the gathered K
+    rows byte for byte against the pool rows, and the stitched K within the a1 bound.  Rows past the last anchor untouched."""
+    binding = _binding()
+    wl = inputs.make_workload("t_ragged")                      # chunk lengths 131 / 64 / 1 / 257 / 77
+    cfg, r = wl.cfg, wl.requests[0]
+    ids = list(r.chunk_ids)
+    lens = [wl.pool_k[c].shape[0] for c in ids]
+    starts = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    ctx = binding.Context(cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.rope_theta, len(lens), 1024, 32)
+    chunks = ctx.batch([[ln] for ln in lens], [[int(x)] for x in starts[:-1]], [0] * len(lens))
+    pool_k, pool_v = _dev(np.concatenate([wl.pool_k[c] for c in ids], 0)), _dev(np.concatenate([wl.pool_v[c] for c in ids], 0))
+    B, Nn = len(lens), chunks.n_stride
+    scores = torch.zeros((B, Nn), device="cuda")
+    idx = torch.full((B, Nn), -1, dtype=torch.int32, device="cuda")
+    n_a = torch.zeros(B, dtype=torch.int32, device="cuda")
+    r_a = 0.1
+    code = binding.QCF_ANCHOR_SINK if rule == "sink" else binding.QCF_ANCHOR_KNORM
+    ctx.qcf_anchor_rank(chunks, pool_k, code, r_a, scores, idx, n_a)
+    counts = [O.n_anchor(ln, r_a) for ln in lens]               # known on the host: sizes the anchor pool
+    total = int(sum(counts))
+    hkv, d = cfg.n_kv_heads, cfg.head_dim
+    ak = torch.full((total + 3, hkv, d), 5.0, dtype=torch.bfloat16, device="cuda")
+    av = torch.full_like(ak, -5.0)
+    ctx.qcf_anchor_gather(chunks, pool_k, pool_v, idx, n_a, ak, av)
+    torch.cuda.synchronize()
+    assert n_a.cpu().tolist() == counts
+    a_idx = np.concatenate([idx[i, :c].cpu().numpy() for i, c in enumerate(counts)]).astype(np.int64)
+    a_ptr = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    k_pic = [O.widen_bf16(wl.pool_k[c]) for c in ids]
+    v_pic = [O.widen_bf16(wl.pool_v[c]) for c in ids]
+    k_exact, v_want, pos = O.anchor_stitch(k_pic, v_pic, a_idx, a_ptr, cfg.rope_theta, store_round=False)
+    assert len(pos) == total
+    assert np.array_equal(_f64(av[:total]), v_want)                                    # Eq. 16 on V: byte copy
+    k_rows = np.concatenate([k_pic[i][a_idx[a_ptr[i]: a_ptr[i + 1]]] for i in range(B)])
+    assert np.array_equal(_f64(ak[:total]), k_rows)                                    # Eq. 16 on K: byte copy (RoPE still local)
+    assert torch.all(ak[total:] == 5.0) and torch.all(av[total:] == -5.0)
+    # K-only and V-only calls write the same rows
+    ak2, av2 = torch.zeros_like(ak), torch.zeros_like(av)
+    ctx.qcf_anchor_gather(chunks, pool_k, None, idx, n_a, ak2, None)
+    ctx.qcf_anchor_gather(chunks, None, pool_v, idx, n_a, None, av2)
+    # Eq. 15: stitch the gathered pool at the chunks' ORIGINAL offsets
+    off = starts[:-1]
+    pb = ctx.batch([counts], [a_ptr[:-1]], [r.n_query], chunk_pos=[off])
+    kf = torch.zeros((1, pb.t_stride, hkv, d), dtype=torch.bfloat16, device="cuda")
+    vf = torch.zeros_like(kf)
+    ctx.qcf_rope_reposition(pb, ak, av, kf, vf)
+    torch.cuda.synchronize()
+    assert torch.equal(ak2[:total], ak[:total]) and torch.equal(av2[:total], av[:total])
+    half = d // 2
+    pair = np.hypot(k_exact[..., :half], k_exact[..., half:])
+    assert np.all(np.abs(_f64(kf[0, :total]) - k_exact) <= 0.5 * _ulp(k_exact) + 1e-6 * np.concatenate([pair, pair], -1) + 1e-30)
+    assert np.array_equal(_f64(vf[0, :total]), v_want)
+    with pytest.raises(binding.QcfError):
+        ctx.qcf_anchor_gather(chunks, pool_k, None, idx, n_a, None, None)             # a pool without its destination
+
+
 # ----------------------------------------------------------------------------------------------- config 3 at full size
 
 def test_stack_layer_full_size_c3_sampled():
