@@ -81,10 +81,13 @@ def n_cores() -> int:
 
 def profile_traffic(workload: str, kernel_substr: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel_substr` on `workload`, from the committed ncu
-    --set full summary profiles/r02_<workload>_kernels.csv (the .md beside it names the capture command).  None if the
-    summary or the kernel's row is absent — never a hard-coded number."""
-    path = os.path.join(ROOT, "profiles", "r02_%s_kernels.csv" % workload)
-    if not os.path.exists(path):
+    --set full summary profiles/r03_<workload>_kernels.csv (else the round-2 file; the .md beside it names the capture
+    command).  None if the summary or the kernel's row is absent — never a hard-coded number."""
+    for rnd in ("r03", "r02"):
+        path = os.path.join(ROOT, "profiles", "%s_%s_kernels.csv" % (rnd, workload))
+        if os.path.exists(path):
+            break
+    else:
         return None, None
     import csv
     with open(path, newline="") as f:
